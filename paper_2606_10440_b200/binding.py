@@ -1,0 +1,210 @@
+"""ctypes binding of include/astra.h.  Same call names as the C-ABI; marshalling only -- every
+step of the hot path runs in the CUDA kernels of csrc/astra_engine.cu."""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libastra_b200.so")
+
+EXPORTED_SYMBOLS = [
+    "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",
+    "astra_load_infragraph", "astra_load_collective", "astra_set_gpu",
+    "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
+    "astra_last_run_info",
+]
+
+FLAG_NO_WINDOW_SKIP = 1
+FLAG_WINDOW_1 = 2
+TS_NONE = np.uint64(0xFFFFFFFFFFFFFFFF)
+
+
+class AstraError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"astra error {code}: {msg}")
+        self.code = code
+
+
+class _Point(ctypes.Structure):
+    _fields_ = [("topo_id", ctypes.c_uint32), ("coll_id", ctypes.c_uint32),
+                ("gpu_id", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+
+
+class _Summary(ctypes.Structure):
+    _fields_ = [("status", ctypes.c_int32), ("n_steps", ctypes.c_uint32), ("n_links", ctypes.c_uint32),
+                ("window", ctypes.c_uint32), ("completion_cycle", ctypes.c_uint64),
+                ("total_lines", ctypes.c_uint64), ("busy_cycles", ctypes.c_uint64),
+                ("skipped_cycles", ctypes.c_uint64)]
+
+
+@dataclass
+class Summary:
+    status: int
+    n_steps: int
+    n_links: int
+    window: int
+    completion_cycle: int
+    total_lines: int
+    busy_cycles: int
+    skipped_cycles: int
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None):
+    """dlopen the engine.  Raises (loudly) when it has not been built; never falls back."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or _LIBPATH
+    if not os.path.exists(p):
+        raise FileNotFoundError(f"{p} not built: run `python -m paper_2606_10440_b200.build` "
+                                "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(p)
+    vp, u32, u64, i32 = ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int32
+    lib.astra_create.argtypes = [ctypes.POINTER(vp), i32, u64]
+    lib.astra_destroy.argtypes = [vp]
+    lib.astra_last_error.argtypes = [vp]
+    lib.astra_last_error.restype = ctypes.c_char_p
+    lib.astra_set_stream.argtypes = [vp, vp]
+    lib.astra_load_infragraph.argtypes = [vp, u32, u32, vp, vp, vp, vp, vp, ctypes.POINTER(u32)]
+    lib.astra_load_collective.argtypes = [vp, u32, u32, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(u32)]
+    lib.astra_set_gpu.argtypes = [vp, u32, u32, u32, u32, ctypes.POINTER(u32)]
+    lib.astra_run_batch.argtypes = [vp, u32, vp, u64]
+    lib.astra_run_batch_async.argtypes = [vp, u32, vp, u64]
+    lib.astra_sync.argtypes = [vp]
+    lib.astra_read_results.argtypes = [vp, u32, ctypes.POINTER(_Summary), vp, vp]
+    lib.astra_last_run_info.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u32), ctypes.POINTER(u64)]
+    for name in EXPORTED_SYMBOLS:
+        if name != "astra_last_error":
+            getattr(lib, name).restype = i32
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _u32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.uint32)
+
+
+class Engine:
+    """One astra_ctx.  Methods mirror the C calls one to one."""
+
+    def __init__(self, device: int = 0, flags: int = 0):
+        self._lib = load_library()
+        self._ctx = ctypes.c_void_p()
+        rc = self._lib.astra_create(ctypes.byref(self._ctx), device, flags)
+        if rc:
+            self._ctx = None
+            raise AstraError(rc, "astra_create failed (no usable CUDA device? there is no CPU fallback)")
+        self._points = None
+        self._n_points = 0
+
+    def _check(self, rc: int):
+        if rc:
+            raise AstraError(rc, (self._lib.astra_last_error(self._ctx) or b"").decode())
+
+    def close(self):
+        if self._ctx:
+            self._lib.astra_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def set_stream(self, cuda_stream_ptr: int):
+        self._check(self._lib.astra_set_stream(self._ctx, ctypes.c_void_p(cuda_stream_ptr)))
+
+    def load_infragraph(self, n_gpus, n_switches, node_latency, row_ptr, head, bw_q8, latency) -> int:
+        arrs = [_u32(node_latency), _u32(row_ptr), _u32(head), _u32(bw_q8), _u32(latency)]
+        out = ctypes.c_uint32()
+        self._check(self._lib.astra_load_infragraph(self._ctx, n_gpus, n_switches, *[_ptr(a) for a in arrs],
+                                                    ctypes.byref(out)))
+        return out.value
+
+    def load_collective(self, n_gpus, owner, dst, lines, cu_lo, cu_n, dep_ptr, dep_step, dep_kind) -> int:
+        arrs = [_u32(owner), _u32(dst), _u32(lines), _u32(cu_lo), _u32(cu_n), _u32(dep_ptr), _u32(dep_step),
+                np.ascontiguousarray(dep_kind, dtype=np.uint8)]
+        out = ctypes.c_uint32()
+        self._check(self._lib.astra_load_collective(self._ctx, n_gpus, len(arrs[0]), *[_ptr(a) for a in arrs],
+                                                    ctypes.byref(out)))
+        return out.value
+
+    def set_gpu(self, cus, wavefronts_per_cu, max_outstanding, hbm_lines_per_cycle) -> int:
+        out = ctypes.c_uint32()
+        self._check(self._lib.astra_set_gpu(self._ctx, cus, wavefronts_per_cu, max_outstanding,
+                                            hbm_lines_per_cycle, ctypes.byref(out)))
+        return out.value
+
+    def _marshal_points(self, points: Sequence[Tuple[int, int, int]]):
+        arr = (_Point * max(1, len(points)))()
+        for i, (t, c, g) in enumerate(points):
+            arr[i].topo_id, arr[i].coll_id, arr[i].gpu_id, arr[i].reserved = t, c, g, 0
+        return arr
+
+    def run_batch(self, points, max_cycles: int, asynchronous: bool = False):
+        if not isinstance(points, ctypes.Array):
+            self._n_points = len(points)
+            points = self._marshal_points(points)
+        self._points = points
+        fn = self._lib.astra_run_batch_async if asynchronous else self._lib.astra_run_batch
+        self._check(fn(self._ctx, self._n_points, ctypes.cast(points, ctypes.c_void_p), max_cycles))
+
+    def sync(self):
+        self._check(self._lib.astra_sync(self._ctx))
+
+    def read_results(self, point: int, want_steps: bool = True, want_links: bool = True):
+        s = _Summary()
+        self._check(self._lib.astra_read_results(self._ctx, point, ctypes.byref(s), None, None))
+        step_ts = np.zeros(max(1, 4 * s.n_steps), dtype=np.uint64) if want_steps else None
+        link_lines = np.zeros(max(1, s.n_links), dtype=np.uint64) if want_links else None
+        if want_steps or want_links:
+            self._check(self._lib.astra_read_results(self._ctx, point, ctypes.byref(s), _ptr(step_ts), _ptr(link_lines)))
+        summ = Summary(s.status, s.n_steps, s.n_links, s.window, s.completion_cycle, s.total_lines,
+                       s.busy_cycles, s.skipped_cycles)
+        return (summ,
+                step_ts[:4 * s.n_steps].reshape(s.n_steps, 4) if want_steps else None,
+                link_lines[:s.n_links] if want_links else None)
+
+    def last_run_info(self):
+        ms, n, b = ctypes.c_float(), ctypes.c_uint32(), ctypes.c_uint64()
+        self._check(self._lib.astra_last_run_info(self._ctx, ctypes.byref(ms), ctypes.byref(n), ctypes.byref(b)))
+        return ms.value, n.value, b.value
+
+    # convenience over the calls above: load a whole astra_inputs.Workload
+    def load_workload(self, w) -> List[Tuple[int, int, int]]:
+        tids = [self.load_infragraph(t.n_gpus, t.n_switches, t.node_latency, t.row_ptr, t.head, t.bw_q8, t.latency)
+                for t in w.topologies]
+        cids = [self.load_collective(c.n_gpus, c.owner, c.dst, c.lines, c.cu_lo, c.cu_n, c.dep_ptr, c.dep_step,
+                                     c.dep_kind) for c in w.collectives]
+        gids = [self.set_gpu(g.cus, g.wavefronts_per_cu, g.max_outstanding, g.hbm_lines_per_cycle) for g in w.gpus]
+        return [(tids[t], cids[c], gids[g]) for (t, c, g) in w.points]
+
+
+def simulate_workload(w, device: int = 0, flags: int = 0, indices=None):
+    """Load, run and read back a Workload.  Returns [(Summary, step_ts[S,4], link_lines[E])]."""
+    with Engine(device, flags) as eng:
+        pts = eng.load_workload(w)
+        if indices is not None:
+            pts = [pts[i] for i in indices]
+        eng.run_batch(pts, w.max_cycles)
+        return [eng.read_results(i) for i in range(len(pts))]

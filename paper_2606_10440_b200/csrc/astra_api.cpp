@@ -1,0 +1,312 @@
+// astra_api.cpp -- the C-ABI of include/astra.h: object tables, batch preparation (constant blob,
+// descriptors, cost-sorted queue, workspace sizing), launch, result read-back.
+// No exception crosses the ABI; every entry point returns an ASTRA_E* code.
+#include "astra_internal.h"
+#include "../../include/astra.h"
+
+#include <cuda_runtime_api.h>
+
+#include <algorithm>
+#include <cstring>
+#include <map>
+#include <new>
+#include <numeric>
+
+struct astra_ctx {
+    int device = 0;
+    u64 flags = 0;
+    std::string err;
+    cudaStream_t own_stream = nullptr, stream = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    std::vector<HostTopo> topos;
+    std::vector<HostColl> colls;
+    std::vector<HostGpu> gpus;
+    // prepared batch
+    bool prepared = false, ran = false, pending = false, results_cached = false;
+    std::vector<astra_point> batch_points;
+    u64 batch_max_cycles = 0;
+    std::vector<PointDesc> descs;
+    uint8_t *d_const = nullptr, *d_ws = nullptr, *d_results = nullptr;
+    PointDesc* d_points = nullptr;
+    u32 *d_order = nullptr, *d_queue = nullptr;
+    u64 const_bytes = 0, ws_stride = 0, ws_total = 0, results_bytes = 0;
+    u32 grid = 0, warps = 0;
+    std::vector<uint8_t> h_results;
+    float last_ms = 0.f;
+    u32 last_launches = 0;
+};
+
+static int32_t fail(astra_ctx* c, int32_t rc, const std::string& msg) { if (c) c->err = msg; return rc; }
+static int32_t cuda_fail(astra_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, e == cudaErrorMemoryAllocation ? ASTRA_ENOMEM : ASTRA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CUDA_TRY(ctx, call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(ctx, e_, what); } while (0)
+
+static void free_batch(astra_ctx* c) {
+    cudaFree(c->d_const); cudaFree(c->d_ws); cudaFree(c->d_results); cudaFree(c->d_points);
+    cudaFree(c->d_order); cudaFree(c->d_queue);
+    c->d_const = c->d_ws = c->d_results = nullptr; c->d_points = nullptr; c->d_order = c->d_queue = nullptr;
+    c->prepared = false; c->ran = false; c->results_cached = false;
+}
+
+extern "C" int32_t astra_create(astra_ctx** out, int32_t cuda_device, uint64_t flags) {
+    if (!out) return ASTRA_EINVAL;
+    *out = nullptr;
+    astra_ctx* c = new (std::nothrow) astra_ctx();
+    if (!c) return ASTRA_ENOMEM;
+    c->device = cuda_device; c->flags = flags;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || cuda_device < 0 || cuda_device >= n) { delete c; return ASTRA_ECUDA; }
+    if (cudaSetDevice(cuda_device) != cudaSuccess || cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) { delete c; return ASTRA_ECUDA; }
+    c->stream = c->own_stream;
+    *out = c;
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_destroy(astra_ctx* c) {
+    if (!c) return ASTRA_EINVAL;
+    cudaSetDevice(c->device);
+    if (c->pending) cudaStreamSynchronize(c->stream);
+    free_batch(c);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->own_stream) cudaStreamDestroy(c->own_stream);
+    delete c;
+    return ASTRA_OK;
+}
+
+extern "C" const char* astra_last_error(const astra_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+extern "C" int32_t astra_set_stream(astra_ctx* c, void* s) {
+    if (!c) return ASTRA_EINVAL;
+    if (c->pending) return fail(c, ASTRA_ESTATE, "a batch is still running");
+    c->stream = s ? (cudaStream_t)s : c->own_stream;
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_load_infragraph(astra_ctx* c, uint32_t n_gpus, uint32_t n_switches,
+                                         const uint32_t* node_latency, const uint32_t* row_ptr,
+                                         const uint32_t* head, const uint32_t* bw_q8, const uint32_t* latency,
+                                         uint32_t* out_id) {
+    if (!c) return ASTRA_EINVAL;
+    if (!node_latency || !row_ptr || !out_id) return fail(c, ASTRA_EINVAL, "null argument");
+    try {
+        HostTopo t;
+        t.G = n_gpus; t.NS = n_switches;
+        u64 V = (u64)n_gpus + n_switches;
+        if (V >= (1u << 24)) return fail(c, ASTRA_ELIMIT, "too many nodes");
+        t.node_lat.assign(node_latency, node_latency + V);
+        t.row_ptr.assign(row_ptr, row_ptr + V + 1);
+        u32 E = t.row_ptr[V];
+        if (E && (!head || !bw_q8 || !latency)) return fail(c, ASTRA_EINVAL, "null link arrays");
+        if (E >= (1u << 22)) return fail(c, ASTRA_ELIMIT, "too many links");
+        t.head.assign(head, head + E); t.bw.assign(bw_q8, bw_q8 + E); t.lat.assign(latency, latency + E);
+        std::string err;
+        int32_t rc = astra_build_topo(t, err);
+        if (rc) return fail(c, rc, err);
+        c->topos.push_back(std::move(t));
+        *out_id = (u32)c->topos.size() - 1;
+        return ASTRA_OK;
+    } catch (const std::bad_alloc&) { return fail(c, ASTRA_ENOMEM, "host allocation failed"); }
+      catch (...) { return fail(c, ASTRA_EINVAL, "unexpected error"); }
+}
+
+extern "C" int32_t astra_load_collective(astra_ctx* c, uint32_t n_gpus, uint32_t n_steps,
+                                         const uint32_t* owner, const uint32_t* dst, const uint32_t* lines,
+                                         const uint32_t* cu_lo, const uint32_t* cu_n,
+                                         const uint32_t* dep_ptr, const uint32_t* dep_step,
+                                         const uint8_t* dep_kind, uint32_t* out_id) {
+    if (!c) return ASTRA_EINVAL;
+    if (!dep_ptr || !out_id || (n_steps && (!owner || !dst || !lines || !cu_lo || !cu_n))) return fail(c, ASTRA_EINVAL, "null argument");
+    try {
+        HostColl h;
+        h.G = n_gpus; h.S = n_steps;
+        if (n_steps >= ASTRA_MAX_STEPS) return fail(c, ASTRA_ELIMIT, "too many steps");
+        h.owner.assign(owner, owner + n_steps); h.dst.assign(dst, dst + n_steps); h.lines.assign(lines, lines + n_steps);
+        h.cu_lo.assign(cu_lo, cu_lo + n_steps); h.cu_n.assign(cu_n, cu_n + n_steps);
+        h.dep_ptr.assign(dep_ptr, dep_ptr + n_steps + 1);
+        u32 nd = h.dep_ptr[n_steps];
+        if (nd && (!dep_step || !dep_kind)) return fail(c, ASTRA_EINVAL, "null dependency arrays");
+        h.dep_step.assign(dep_step, dep_step + nd); h.dep_kind.assign(dep_kind, dep_kind + nd);
+        std::string err;
+        int32_t rc = astra_build_coll(h, err);
+        if (rc) return fail(c, rc, err);
+        c->colls.push_back(std::move(h));
+        *out_id = (u32)c->colls.size() - 1;
+        return ASTRA_OK;
+    } catch (const std::bad_alloc&) { return fail(c, ASTRA_ENOMEM, "host allocation failed"); }
+      catch (...) { return fail(c, ASTRA_EINVAL, "unexpected error"); }
+}
+
+extern "C" int32_t astra_set_gpu(astra_ctx* c, uint32_t cus, uint32_t wpc, uint32_t k, uint32_t h, uint32_t* out_id) {
+    if (!c) return ASTRA_EINVAL;
+    if (!out_id) return fail(c, ASTRA_EINVAL, "null argument");
+    if (!cus || !wpc || !k || !h) return fail(c, ASTRA_EINVAL, "GPU parameters must be >= 1");
+    if ((u64)cus * wpc > ASTRA_MAX_WAVEFRONTS) return fail(c, ASTRA_ELIMIT, "cus * wavefronts_per_cu above ASTRA_MAX_WAVEFRONTS");
+    if (k > ASTRA_MAX_OUTSTANDING) return fail(c, ASTRA_ELIMIT, "max_outstanding above ASTRA_MAX_OUTSTANDING");
+    if (h > ASTRA_MAX_HBM_LINES) return fail(c, ASTRA_ELIMIT, "hbm_lines_per_cycle above ASTRA_MAX_HBM_LINES");
+    HostGpu g; g.C = cus; g.Wv = wpc; g.K = k; g.H = h;
+    c->gpus.push_back(g);
+    *out_id = (u32)c->gpus.size() - 1;
+    return ASTRA_OK;
+}
+
+static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_t max_cycles) {
+    free_batch(c);
+    Blob blob;
+    std::map<u32, std::vector<u64>> topo_off, coll_off;
+    c->descs.assign(n, PointDesc());
+    std::vector<double> cost(n, 0.0);
+    u64 roff = 0; u32 maxV = 1; u64 ws_max = 0;
+    for (u32 i = 0; i < n; i++) {
+        const astra_point& p = pts[i];
+        if (p.topo_id >= c->topos.size() || p.coll_id >= c->colls.size() || p.gpu_id >= c->gpus.size())
+            return fail(c, ASTRA_ESTATE, "design point references an unknown id");
+        const HostTopo& t = c->topos[p.topo_id];
+        const HostColl& h = c->colls[p.coll_id];
+        if (!topo_off.count(p.topo_id)) {
+            std::vector<u64> o(10);
+            o[0] = blob.add(t.row_ptr); o[1] = blob.add(t.in_ptr); o[2] = blob.add(t.in_link); o[3] = blob.add(t.leff);
+            o[4] = blob.add(t.bw); o[5] = blob.add(t.icand_ptr); o[6] = blob.add(t.icand); o[7] = blob.add(t.ocand_ptr);
+            o[8] = blob.add(t.ocand); o[9] = blob.add(t.next_link);
+            topo_off[p.topo_id] = o;
+        }
+        if (!coll_off.count(p.coll_id)) {
+            std::vector<u32> od(h.S);
+            for (u32 s = 0; s < h.S; s++) od[s] = (h.owner[s] << 16) | h.dst[s];
+            std::vector<u64> o(7);
+            o[0] = blob.add(od); o[1] = blob.add(h.lines); o[2] = blob.add(h.cu_lo); o[3] = blob.add(h.cu_n);
+            o[4] = blob.add(h.succ_ptr); o[5] = blob.add(h.succ); o[6] = blob.add(h.ndeps);
+            coll_off[p.coll_id] = o;
+        }
+        std::string err;
+        int32_t rc = astra_plan_point(t, h, c->gpus[p.gpu_id], c->flags, max_cycles, topo_off[p.topo_id].data(),
+                                      coll_off[p.coll_id].data(), blob, c->descs[i], cost[i], err);
+        if (rc) return fail(c, rc, "point " + std::to_string(i) + ": " + err);
+        PointDesc& P = c->descs[i];
+        P.r_step_ts = roff; roff += 32ull * P.S;
+        P.r_link_lines = roff; roff += 8ull * P.E;
+        P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
+        maxV = std::max(maxV, P.V);
+        ws_max = std::max(ws_max, P.ws_bytes);
+    }
+    c->results_bytes = roff ? roff : 16;
+    c->ws_stride = (ws_max + 255) & ~255ull;
+    c->warps = std::min<u32>(16, maxV);
+    std::string err;
+    u32 occ = 0, sms = 0;
+    int32_t rc = astra_engine_occupancy(c->warps, &occ, &sms, err);
+    if (rc) return fail(c, rc, err);
+    if (occ == 0) return fail(c, ASTRA_ECUDA, "kernel does not fit on an SM");
+    c->grid = std::max<u32>(1, std::min<u32>(n, occ * sms));
+    size_t free_b = 0, total_b = 0;
+    CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b), "cudaMemGetInfo");
+    u64 budget = (u64)(free_b * 0.85);
+    u64 fixed = blob.bytes.size() + c->results_bytes + n * sizeof(PointDesc) + n * 4 + 4096;
+    if (fixed + c->ws_stride > budget) return fail(c, ASTRA_ENOMEM, "batch does not fit in device memory");
+    while (c->grid > 1 && fixed + (u64)c->grid * c->ws_stride > budget) c->grid--;
+    c->ws_total = (u64)c->grid * c->ws_stride;
+    c->const_bytes = blob.bytes.size();
+
+    std::vector<u32> order(n);
+    std::iota(order.begin(), order.end(), 0u);
+    std::stable_sort(order.begin(), order.end(), [&](u32 a, u32 b) { return cost[a] > cost[b]; });
+
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_const, std::max<size_t>(16, blob.bytes.size())), "cudaMalloc const");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_ws, std::max<u64>(16, c->ws_total)), "cudaMalloc workspace");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_results, c->results_bytes), "cudaMalloc results");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_points, std::max<size_t>(16, n * sizeof(PointDesc))), "cudaMalloc points");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_order, std::max<size_t>(16, n * 4)), "cudaMalloc order");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_queue, 16), "cudaMalloc queue");
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_const, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, c->stream), "H2D const");
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_points, c->descs.data(), n * sizeof(PointDesc), cudaMemcpyHostToDevice, c->stream), "H2D points");
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_order, order.data(), n * 4, cudaMemcpyHostToDevice, c->stream), "H2D order");
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream), "H2D sync");     // host staging buffers die here
+    c->batch_points.assign(pts, pts + n);
+    c->batch_max_cycles = max_cycles;
+    c->prepared = true;
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_run_batch_async(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_t max_cycles) {
+    if (!c) return ASTRA_EINVAL;
+    if (n && !pts) return fail(c, ASTRA_EINVAL, "null points");
+    if (c->pending) return fail(c, ASTRA_ESTATE, "a batch is still running");
+    try {
+        CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
+        bool same = c->prepared && c->batch_points.size() == n && c->batch_max_cycles == max_cycles &&
+                    (n == 0 || std::memcmp(c->batch_points.data(), pts, n * sizeof(astra_point)) == 0);
+        if (!same) { int32_t rc = prepare(c, n, pts, max_cycles); if (rc) return rc; }
+        c->results_cached = false; c->ran = false;
+        CUDA_TRY(c, cudaEventRecord(c->ev0, c->stream), "event record");
+        c->last_launches = 0;
+        if (n) {
+            EngineLaunch L;
+            L.d_const = c->d_const; L.d_ws = c->d_ws; L.d_results = c->d_results; L.d_points = c->d_points;
+            L.d_order = c->d_order; L.d_queue = c->d_queue; L.n_points = n; L.ws_stride = c->ws_stride;
+            L.grid = c->grid; L.warps_per_cta = c->warps;
+            std::string err;
+            int32_t rc = astra_engine_launch(L, (void*)c->stream, err);
+            if (rc) return fail(c, rc, err);
+            c->last_launches = 1;
+        }
+        CUDA_TRY(c, cudaEventRecord(c->ev1, c->stream), "event record");
+        c->pending = true;
+        return ASTRA_OK;
+    } catch (const std::bad_alloc&) { return fail(c, ASTRA_ENOMEM, "host allocation failed"); }
+      catch (...) { return fail(c, ASTRA_EINVAL, "unexpected error"); }
+}
+
+extern "C" int32_t astra_sync(astra_ctx* c) {
+    if (!c) return ASTRA_EINVAL;
+    if (!c->pending) return ASTRA_OK;
+    c->pending = false;
+    CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream), "kernel execution");
+    CUDA_TRY(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1), "event elapsed");
+    c->ran = true;
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_run_batch(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_t max_cycles) {
+    int32_t rc = astra_run_batch_async(c, n, pts, max_cycles);
+    if (rc) return rc;
+    return astra_sync(c);
+}
+
+extern "C" int32_t astra_read_results(astra_ctx* c, uint32_t point, astra_summary* out, uint64_t* step_ts, uint64_t* link_lines) {
+    if (!c) return ASTRA_EINVAL;
+    if (c->pending) { int32_t rc = astra_sync(c); if (rc) return rc; }
+    if (!c->ran) return fail(c, ASTRA_ESTATE, "no batch has been run");
+    if (point >= c->descs.size()) return fail(c, ASTRA_ESTATE, "point index out of range");
+    try {
+        if (!c->results_cached) {
+            CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
+            c->h_results.resize(c->results_bytes);
+            CUDA_TRY(c, cudaMemcpy(c->h_results.data(), c->d_results, c->results_bytes, cudaMemcpyDeviceToHost), "D2H results");
+            c->results_cached = true;
+        }
+    } catch (const std::bad_alloc&) { return fail(c, ASTRA_ENOMEM, "host allocation failed"); }
+    const PointDesc& P = c->descs[point];
+    const uint8_t* base = c->h_results.data();
+    if (out) {
+        DeviceSummary s; std::memcpy(&s, base + P.r_summary, sizeof(s));
+        out->status = s.status; out->n_steps = s.n_steps; out->n_links = s.n_links; out->window = s.window;
+        out->completion_cycle = s.completion_cycle; out->total_lines = s.total_lines;
+        out->busy_cycles = s.busy_cycles; out->skipped_cycles = s.skipped_cycles;
+    }
+    if (step_ts) std::memcpy(step_ts, base + P.r_step_ts, 32ull * P.S);
+    if (link_lines) std::memcpy(link_lines, base + P.r_link_lines, 8ull * P.E);
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_last_run_info(astra_ctx* c, float* ms, uint32_t* launches, uint64_t* bytes) {
+    if (!c) return ASTRA_EINVAL;
+    if (c->pending) { int32_t rc = astra_sync(c); if (rc) return rc; }
+    if (ms) *ms = c->last_ms;
+    if (launches) *launches = c->last_launches;
+    if (bytes) *bytes = c->const_bytes + c->ws_total + c->results_bytes + c->descs.size() * sizeof(PointDesc);
+    return ASTRA_OK;
+}

@@ -1,0 +1,143 @@
+"""Parity proper: CUDA engine (through the C-ABI) == CPU oracle, bit for bit, on every integer
+output (completion cycle, four timestamps per step, lines per link).  Needs a B200."""
+import os
+
+import numpy as np
+import pytest
+
+from astra_inputs import GpuCfg, Workload, collectives as C, configs, topologies as T
+from oracle import oracle
+from tests.parity import check_workload, compare_point
+
+pytestmark = pytest.mark.gpu
+
+FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1 = 1, 2
+
+
+def _single(topo, coll, gpu, name="case", max_cycles=1 << 22):
+    w = Workload(name=name, max_cycles=max_cycles)
+    w.topologies.append(topo); w.collectives.append(coll); w.gpus.append(gpu)
+    w.points.append((0, 0, 0)); w.meta.append({})
+    return w
+
+
+def test_library_loaded_is_in_tree():
+    import paper_2606_10440_b200 as pkg
+    lib = pkg.load_library()
+    assert os.path.dirname(lib._name) == os.path.dirname(pkg.__file__)
+
+
+@pytest.mark.parametrize("k", [64, 2])
+def test_p1_hand_trace(k):
+    check_workload(_single(T.line(2, 256, 3), C.single_transfer(2, 0, 1, 5, 0, 1), GpuCfg(1, 1, k, 1)))
+
+
+def test_p2_p3():
+    check_workload(_single(T.line(2, 128, 3), C.single_transfer(2, 0, 1, 5, 0, 1), GpuCfg(1, 2, 64, 2)))
+    check_workload(_single(T.line(2, 1024, 7), C.single_transfer(2, 0, 1, 10, 0, 2), GpuCfg(2, 4, 64, 8)))
+
+
+def test_config1_bit_exact_and_pin():
+    gpu, _ = check_workload(configs.config1())
+    assert gpu[0][0].completion_cycle == 38623
+
+
+@pytest.mark.parametrize("cus", [1, 2, 8, 16, 64])
+def test_config1_cu_sweep(cus):
+    check_workload(configs.config1(cus))
+
+
+@pytest.mark.parametrize("seed", range(30))
+def test_random_small_workloads(seed):
+    """Random topologies (latencies down to 1 cycle -> 1-cycle windows), all three dep kinds."""
+    check_workload(configs.random_workload(seed, n_points=4, max_gpus=6, max_steps=24, max_lines=200))
+
+
+@pytest.mark.parametrize("flags", [FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_NO_WINDOW_SKIP | FLAG_WINDOW_1])
+def test_i8_skip_equivalence(flags):
+    """I8: outputs with idle-cycle / window skipping == without, and with a 1-cycle window."""
+    w = configs.random_workload(77, n_points=6, max_gpus=6, max_steps=24, max_lines=200)
+    check_workload(w, flags=flags)
+    check_workload(configs.config1(), flags=flags)
+
+
+def test_named_families_small():
+    gpu = GpuCfg(8, 2, 4, 6)
+    cases = [
+        (T.ring(8, 256, 9), C.ring_allreduce(8, 203, 8)[0]),
+        (T.torus2d(2, 4, 128, 7), C.direct_allreduce(8, 170, 8)),
+        (T.ring(8, 512, 5), C.double_binary_tree_allreduce(8, 157, 8)),
+        (T.torus2d(2, 4, 384, 11), C.halving_doubling_allreduce(8, 99, 8)),
+        (T.single_switch(4, 512, 6, 3), C.direct_allreduce(4, 120, 8)),
+        (T.nodes_fat_tree(2, 2, 2, 512, 5, 2, 128, 13, 1), C.hierarchical_allreduce(2, 2, 64, 8)),
+        (T.rail_optimized(2, 8, 512, 5, 2, 256, 9, 0), C.all_to_all(16, lambda g, d: 1 + (g * 7 + d * 3) % 9, 8)),
+    ]
+    for i, (topo, coll) in enumerate(cases):
+        check_workload(_single(topo, coll, gpu, name=f"family{i}"))
+
+
+def test_config2_all_22_points():
+    """BASELINE config 2 in the launch configuration bench.py times (one batch of 22 points)."""
+    gpu, _ = check_workload(configs.config2(), processes=8)
+    w = configs.config2()
+    for (summ, _, _), m in zip(gpu, w.meta):
+        n = m["lines"] // 8
+        if m["algo"] == "ring":
+            assert summ.completion_cycle == 14 * (350 + -(-n // 4)) + 350
+
+
+def test_config3_reduced():
+    """Config 3 topology and collective at 1/64 of the message size (oracle finishes in seconds)."""
+    check_workload(configs.config3(lines=32 * 1024 * 8))
+
+
+def test_config5_reduced():
+    check_workload(configs.config5(n_nodes=4), oracle_flags=oracle.FLAG_PRUNED_SCAN)
+
+
+def test_config4_sample():
+    """64 of the 4096 config-4 points (every point is independent): pruned-scan oracle."""
+    w = configs.config4(64)
+    check_workload(w, oracle_flags=oracle.FLAG_PRUNED_SCAN, processes=8)
+
+
+def test_i6_batch_independence():
+    """A point's result does not depend on its neighbours or on the batch order."""
+    from paper_2606_10440_b200 import simulate_workload
+    w = configs.config4(24)
+    a = simulate_workload(w)
+    order = list(reversed(range(24)))
+    b = simulate_workload(w, indices=order)
+    c = simulate_workload(w, indices=[5])
+    for j, i in enumerate(order):
+        assert a[i][0].completion_cycle == b[j][0].completion_cycle
+        assert (a[i][1] == b[j][1]).all() and (a[i][2] == b[j][2]).all()
+    assert (a[5][1] == c[0][1]).all()
+
+
+def test_watchdog_and_edge_cases():
+    from paper_2606_10440_b200 import Engine, AstraError
+    topo, coll, gpu = configs.config1().point(0)
+    w = _single(topo, coll, gpu, max_cycles=1000)
+    gpu_res, ora = check_workload(w)
+    assert gpu_res[0][0].status == 1
+    with Engine() as eng:
+        eng.run_batch([], 100)                                   # empty batch
+        with pytest.raises(AstraError) as ei:
+            eng.read_results(0)
+        assert ei.value.code == -6
+        t = eng.load_infragraph(topo.n_gpus, 0, topo.node_latency, topo.row_ptr, topo.head, topo.bw_q8, topo.latency)
+        c = eng.load_collective(coll.n_gpus, coll.owner, coll.dst, coll.lines, coll.cu_lo, coll.cu_n,
+                                coll.dep_ptr, coll.dep_step, coll.dep_kind)
+        g_small = eng.set_gpu(2, 2, 16, 8)                       # CU range [0,4) exceeds 2 CUs
+        with pytest.raises(AstraError) as ei:
+            eng.run_batch([(t, c, g_small)], 1000)
+        assert ei.value.code == -1
+        line3 = T.Topology.from_edges(3, 0, [0, 0, 0], [(0, 1, 256, 5), (1, 0, 256, 5)])
+        t3 = eng.load_infragraph(3, 0, line3.node_latency, line3.row_ptr, line3.head, line3.bw_q8, line3.latency)
+        c3 = C.single_transfer(3, 0, 2, 4, 0, 1)
+        c3id = eng.load_collective(3, c3.owner, c3.dst, c3.lines, c3.cu_lo, c3.cu_n, c3.dep_ptr, c3.dep_step, c3.dep_kind)
+        g1 = eng.set_gpu(1, 1, 4, 1)
+        with pytest.raises(AstraError) as ei:
+            eng.run_batch([(t3, c3id, g1)], 1000)
+        assert ei.value.code == -4                               # unreachable
