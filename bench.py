@@ -1,0 +1,273 @@
+#!/usr/bin/env python
+"""bench.py -- simulated 128 B cache-line transactions/sec of the CUDA engine on BASELINE config 2
+(8 GPUs on one switch, ring + direct all-reduce, 64 KiB .. 64 MiB, 22 design points in one batch).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+One "step" = one pass of the whole hot path (A0 excluded, A1-A8 included: state init, every
+simulated cycle, result write-out) over the 22-point batch.  `value` is measured with the tables
+resident in HBM (CUDA events on the launching stream); `e2e` goes through the C-ABI from host
+arrays: load_infragraph + load_collective + set_gpu + run_batch + read_results, host<->device
+copies included.  N > 1 (torchrun): every rank runs the same batch on its own GPU (the path
+shards by design point with no collective; weak scaling), time = max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/) as it stands on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "simulated_128B_cacheline_transactions_per_sec"
+UNIT = "transactions/s"
+BYTES_PER_TX_BASE, BYTES_PER_HOP = 72, 20          # SURVEY.md 8(d) algorithmic bytes per transaction
+
+
+def get_workload(name: str):
+    from astra_inputs import configs
+    if name == "config4":
+        return configs.config4(4096)
+    return configs.by_name(name)
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows for i in range(4) if len(r) > 2 + i and r[2 + i].startswith("Active")})
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_baseline(w, budget_s: float = 25.0):
+    """Time the oracle as it stands (plain scan, one design point per process) on a bounded sample:
+    the points of the workload in order of size until ~budget_s of CPU work."""
+    from oracle import oracle
+    oracle.build()
+    cores = max(1, min(os.cpu_count() or 1, w.n_points))
+    order = sorted(range(w.n_points), key=lambda i: w.collectives[w.points[i][1]].total_lines)
+    # config 2 in full is ~11 s of single-core work; larger workloads are cut to the cheapest points
+    est, sample = 0.0, []
+    for i in order:
+        est += w.collectives[w.points[i][1]].total_lines / 2.5e6
+        sample.append(i)
+        if est > budget_s * cores:
+            break
+    t0 = time.perf_counter()
+    res = oracle.run_workload(w, sample, processes=cores)
+    dt = time.perf_counter() - t0
+    lines = sum(r.total_lines for r in res)
+    return {"value": lines / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{len(sample)} of {w.n_points} design points of {w.name} ({lines} lines), plain scan, "
+                      f"one point per process, {dt:.2f} s wall",
+            "points_per_sec": len(sample) / dt, "seconds": dt}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = get_workload(args.workload)
+    runs = []
+    for _ in range(args.warmup and 1):
+        oracle_baseline(w, budget_s=2.0)
+    for _ in range(max(1, args.steps)):
+        runs.append(oracle_baseline(w, budget_s=20.0 / max(1, args.steps)))
+    dt = sum(r["seconds"] for r in runs) / len(runs)
+    val = sum(r["value"] for r in runs) / len(runs)
+    base = dict(runs[-1]); base["value"] = val
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": w.name, "design_points": w.n_points, "sample": base["sample"]},
+        "cpu_baseline": base,
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the engine has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_2606_10440_b200 import Engine, build as engine_build
+    engine_build.build()
+    w = get_workload(args.workload)
+    total_lines = w.total_lines()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.Stream()            # a real (non-default) stream shared by torch and the engine
+    torch.cuda.set_stream(stream)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    eng = Engine(local_rank)
+    eng.set_stream(stream.cuda_stream)
+    pts = eng.load_workload(w)
+    eng.run_batch(pts, w.max_cycles)                                     # prepares the batch (A0) + 1 run
+    # ---- correctness spot check against stored closed forms (no oracle call on this path) ----
+    summ = [eng.read_results(i, False, False)[0] for i in range(len(pts))]
+    assert all(s.status == 0 for s in summ), "a design point did not finish"
+    hops_lines = 0
+    for i in range(len(pts)):
+        _, _, ll = eng.read_results(i, False, True)
+        hops_lines += int(ll.sum())
+    alg_bytes = BYTES_PER_TX_BASE * total_lines + BYTES_PER_HOP * hops_lines
+    busy = sum(s.busy_cycles for s in summ)
+
+    for _ in range(max(0, args.warmup - 1)):
+        flush.zero_()
+        eng.run_batch(pts, w.max_cycles)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    kernel_ms = []
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        flush.zero_()                                                    # L2 flush between iterations
+        eng.run_batch(pts, w.max_cycles, asynchronous=True)
+        eng.sync()
+        kernel_ms.append(eng.last_run_info()[0])
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        tt = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = world * total_lines / (ms_per_step * 1e-3)
+    k_ms = float(np.mean(kernel_ms))
+    _, launches, dev_bytes = eng.last_run_info()
+    eng.close()
+
+    # ---- end to end through the C-ABI from host arrays ----
+    e2e_times = []
+    h2d = d2h = 0
+    for it in range(min(3, max(1, args.steps))):
+        barrier()
+        t0 = time.perf_counter()
+        with Engine(local_rank) as e2:
+            p2 = e2.load_workload(w)
+            e2.run_batch(p2, w.max_cycles)
+            outs = [e2.read_results(i) for i in range(len(p2))]
+            h2d, d2h = e2.last_transfer_bytes()
+        torch.cuda.synchronize()
+        e2e_times.append(time.perf_counter() - t0)
+        assert all(o[0].status == 0 for o in outs)
+    e2e_s = min(e2e_times)
+    if world > 1:
+        tt = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_s = float(tt.item())
+
+    peak, peak_src = measured_peak_gbs()
+    achieved = alg_bytes / (k_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(w.name)
+        except Exception:
+            traffic = None
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64", "data": "synthetic",
+        "config": {"workload": w.name, "design_points": w.n_points, "transactions_per_step": total_lines,
+                   "l2": "256 MiB device write between timed iterations (inside the timed region)",
+                   "parallelism": f"design points x {world} GPU(s), no collective"},
+        "design_points_per_sec": world * w.n_points / (ms_per_step * 1e-3),
+        "gpu_launches": launches * args.steps,
+        "clocks": clocks,
+        "e2e": {"value": world * total_lines / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "seconds_per_step": e2e_s},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "kernel": "astra_step_kernel", "kernel_ms": k_ms,
+                     "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
+                     "note": "bytes = 72 per transaction + 20 per link hop (SURVEY 8(d)); the kernel is "
+                             "latency/issue bound, see DESIGN.md section 6",
+                     "node_cycles_stepped": busy, "device_bytes": dev_bytes},
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = {k: v for k, v in oracle_baseline(w).items() if k != "seconds"}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -157,6 +157,10 @@ int32_t astra_read_results(astra_ctx* ctx, uint32_t point, astra_summary* out,
 int32_t astra_last_run_info(astra_ctx* ctx, float* device_ms, uint32_t* kernel_launches,
                             uint64_t* device_bytes);
 
+/* Diagnostics: host->device bytes copied when the last batch was prepared (tables, descriptors,
+ * queue order) and device->host bytes a full read-back of its results copies. */
+int32_t astra_last_transfer_bytes(astra_ctx* ctx, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",
     "astra_load_infragraph", "astra_load_collective", "astra_set_gpu",
     "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
-    "astra_last_run_info",
+    "astra_last_run_info", "astra_last_transfer_bytes",
 ]
 
 FLAG_NO_WINDOW_SKIP = 1
@@ -81,6 +81,7 @@ def load_library(path: Optional[str] = None):
     lib.astra_sync.argtypes = [vp]
     lib.astra_read_results.argtypes = [vp, u32, ctypes.POINTER(_Summary), vp, vp]
     lib.astra_last_run_info.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u32), ctypes.POINTER(u64)]
+    lib.astra_last_transfer_bytes.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     for name in EXPORTED_SYMBOLS:
         if name != "astra_last_error":
             getattr(lib, name).restype = i32
@@ -189,6 +190,11 @@ class Engine:
         ms, n, b = ctypes.c_float(), ctypes.c_uint32(), ctypes.c_uint64()
         self._check(self._lib.astra_last_run_info(self._ctx, ctypes.byref(ms), ctypes.byref(n), ctypes.byref(b)))
         return ms.value, n.value, b.value
+
+    def last_transfer_bytes(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self._lib.astra_last_transfer_bytes(self._ctx, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     # convenience over the calls above: load a whole astra_inputs.Workload
     def load_workload(self, w) -> List[Tuple[int, int, int]]:

@@ -310,3 +310,11 @@ extern "C" int32_t astra_last_run_info(astra_ctx* c, float* ms, uint32_t* launch
     if (bytes) *bytes = c->const_bytes + c->ws_total + c->results_bytes + c->descs.size() * sizeof(PointDesc);
     return ASTRA_OK;
 }
+
+extern "C" int32_t astra_last_transfer_bytes(astra_ctx* c, uint64_t* h2d, uint64_t* d2h) {
+    if (!c) return ASTRA_EINVAL;
+    if (!c->prepared) return fail(c, ASTRA_ESTATE, "no batch has been prepared");
+    if (h2d) *h2d = c->const_bytes + c->descs.size() * (sizeof(PointDesc) + 4);
+    if (d2h) *d2h = c->results_bytes;
+    return ASTRA_OK;
+}
