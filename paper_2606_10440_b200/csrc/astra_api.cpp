@@ -159,7 +159,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     std::map<u32, std::vector<u64>> topo_off, coll_off;
     c->descs.assign(n, PointDesc());
     std::vector<double> cost(n, 0.0);
-    u64 roff = 0; u32 maxV = 1; u64 ws_max = 0;
+    u64 roff = 0; u64 ws_max = 0;
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];
         if (p.topo_id >= c->topos.size() || p.coll_id >= c->colls.size() || p.gpu_id >= c->gpus.size())
@@ -167,16 +167,15 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         const HostTopo& t = c->topos[p.topo_id];
         const HostColl& h = c->colls[p.coll_id];
         if (!topo_off.count(p.topo_id)) {
-            std::vector<u64> o(10);
-            o[0] = blob.add(t.row_ptr); o[1] = blob.add(t.in_ptr); o[2] = blob.add(t.in_link); o[3] = blob.add(t.leff);
-            o[4] = blob.add(t.bw); o[5] = blob.add(t.icand_ptr); o[6] = blob.add(t.icand); o[7] = blob.add(t.ocand_ptr);
-            o[8] = blob.add(t.ocand); o[9] = blob.add(t.next_link);
+            std::vector<u64> o(ASTRA_N_TOPO_TABLES);
+            o[0] = blob.add(t.in_ptr); o[1] = blob.add(t.in_link); o[2] = blob.add(t.head); o[3] = blob.add(t.tail);
+            o[4] = blob.add(t.leff); o[5] = blob.add(t.bw); o[6] = blob.add(t.next_link);
             topo_off[p.topo_id] = o;
         }
         if (!coll_off.count(p.coll_id)) {
             std::vector<u32> od(h.S);
             for (u32 s = 0; s < h.S; s++) od[s] = (h.owner[s] << 16) | h.dst[s];
-            std::vector<u64> o(7);
+            std::vector<u64> o(ASTRA_N_COLL_TABLES);
             o[0] = blob.add(od); o[1] = blob.add(h.lines); o[2] = blob.add(h.cu_lo); o[3] = blob.add(h.cu_n);
             o[4] = blob.add(h.succ_ptr); o[5] = blob.add(h.succ); o[6] = blob.add(h.ndeps);
             coll_off[p.coll_id] = o;
@@ -189,12 +188,11 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         P.r_step_ts = roff; roff += 32ull * P.S;
         P.r_link_lines = roff; roff += 8ull * P.E;
         P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
-        maxV = std::max(maxV, P.V);
         ws_max = std::max(ws_max, P.ws_bytes);
     }
     c->results_bytes = roff ? roff : 16;
     c->ws_stride = (ws_max + 255) & ~255ull;
-    c->warps = std::min<u32>(16, maxV);
+    c->warps = 16;
     std::string err;
     u32 occ = 0, sms = 0;
     int32_t rc = astra_engine_occupancy(c->warps, &occ, &sms, err);

@@ -12,20 +12,21 @@ typedef uint64_t u64;
 // Flit: one 128 B line in flight, 64 bits.
 //   [0,20)  step id      [20,32) wavefront id within the owner GPU (cu*W + w)
 //   [32,38) outstanding-slot index inside the wavefront (ack addressing)
-//   [38,64) arrival cycle mod 2^26 (meaningful in link latency pipes only)
+//   [38,64) arrival cycle mod 2^26 (meaningful once the link has accepted the line)
 // ---------------------------------------------------------------------------------------------
 #define ASTRA_FLIT_TIME_SHIFT 38
+#define ASTRA_FLIT_PAYLOAD_MASK ((1ull << ASTRA_FLIT_TIME_SHIFT) - 1)
 #define ASTRA_TMASK26 0x3ffffffu
 #define ASTRA_T_INF 0xffffffffu
 #define ASTRA_NOTLOADED 0xffffffffu
 #define ASTRA_TS_NONE32 0xffffffffu
-#define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles (per-warp smem histogram)
-#define ASTRA_CAND_PAD 0xffffffffu        // padding entry in candidate tables
+#define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles (per-warp smem scratch)
+#define ASTRA_NW_MAX 256                  // ack window bins per point (smem counters)
 
-// Candidate table entry (per node, for in-links and out-links): link id, ceil(B), k.
-//   [10,32) link id   [5,10) ceil(bw)   [0,5) k
-// A link's block of candidates never straddles a 32-entry chunk.
-static inline u32 astra_cand_pack(u32 link, u32 ceilb, u32 k) { return (link << 10) | (ceilb << 5) | k; }
+// Link service kinds (R9): how the acceptance times of a FIFO are computed for a whole window.
+#define ASTRA_LK_INT     0u               // bw = B*256: B lines every cycle, no carried credit
+#define ASTRA_LK_PERIOD  1u               // 256 % bw == 0: one line every P = 256/bw cycles
+#define ASTRA_LK_GENERAL 2u               // any other bw: saturating credit walked entry by entry
 
 // Per design point descriptor.  c_* are byte offsets into the batch's constant blob, w_* byte
 // offsets into the workspace of the CTA slot running the point, r_* byte offsets into the results
@@ -34,28 +35,30 @@ struct PointDesc {
     u32 G, V, E, S;
     u32 C, Wv, K, H;
     u32 CW, nwords, slots, bmwords;
-    u32 logW, NW, kdiv_magic, n_rel_total;     // NW power of two; kdiv_magic = ceil(2^32 / K)
+    u32 logW, NW, kdiv_magic, NC;              // NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
     u32 flags, pad0;
     u64 max_cycles;
     u64 total_lines;
     u64 ws_bytes, ws_zero_bytes, ws_ff_off, ws_ff_bytes;
     // topology tables
-    u64 c_row_ptr, c_in_ptr, c_in_link, c_leff, c_bw, c_icand_ptr, c_icand, c_ocand_ptr, c_ocand, c_next_link;
+    u64 c_in_ptr, c_in_link, c_head, c_tail, c_leff, c_bw, c_next_link;
     // collective tables
     u64 c_step_od, c_lines, c_cu_lo, c_cu_n, c_succ_ptr, c_succ, c_ndeps;
     // plan tables (topology x collective x gpu)
     u64 c_step_q, c_step_r, c_first_link, c_step_alpha, c_cul_ptr, c_cul, c_rel_off, c_init_rel, c_init_rel_cnt;
-    u64 c_fifo_off, c_fifo_mask, c_pipe_off, c_pipe_mask, c_credit_cap;
+    u64 c_ev_off;
+    u64 c_ring_off, c_ring_mask, c_lkind, c_ceilb, c_lstate0_init, c_stage_off, c_mask_off, c_classoff;
+    u64 c_nd_cellcap, c_nd_mw, c_nd_injoff;
     // workspace: zero-initialised region
-    u64 w_fifo_head, w_fifo_tail, w_pipe_tail, w_pipe_tail_pub, w_pipe_head, w_pipe_tsnap, w_credit_time, w_link_lines;
-    u64 w_issued_cnt, w_deliv_cnt, w_ack_cnt, w_wf_busy, w_want, w_freeb, w_pend_cnt, w_rel_cnt;
-    u64 w_bitmap, w_bin_cnt, w_node_next, w_node_busy, w_node_acked;
+    u64 w_pipe_head, w_fifo_head, w_tail, w_lstate1, w_link_lines, w_masks;
+    u64 w_issued_cnt, w_t_issued, w_deliv_cnt, w_t_deliv, w_ack_cnt, w_t_ack, w_rel_time;
+    u64 w_wf_busy, w_want, w_bitmap, w_bin_cnt, w_ack_n, w_ev_cnt;
     // workspace: 0xff-initialised region
-    u64 w_t_release, w_t_issued, w_t_deliv, w_t_ack, w_wf_rem;
+    u64 w_wf_rem;
     // workspace: specially initialised
-    u64 w_credit, w_ndep_left, w_wf_cur, w_rel_list;
+    u64 w_lstate0, w_t_release, w_ndep_left, w_wf_cur, w_freeb, w_plist, w_pcnt;
     // workspace: uninitialised
-    u64 w_fifo_buf, w_pipe_buf, w_pend, w_pend_link, w_sel, w_ack_rec, w_ack_tmp, w_ack_sorted;   // ack_tmp / ack_sorted hold u64 entries
+    u64 w_ring, w_stage, w_sel, w_ack_rec, w_ack_tmp, w_ack_sorted, w_ev_list;
     // results
     u64 r_step_ts, r_link_lines, r_summary;
 };
@@ -74,7 +77,6 @@ struct HostTopo {
     std::vector<u32> in_ptr, in_link;
     std::vector<u32> next_link;       // [V*G], 0xffffffff = none
     std::vector<u32> dist;            // [V*G], 0xffffffff = unreachable
-    std::vector<u32> icand_ptr, icand, ocand_ptr, ocand;
     u32 min_leff = 0, max_leff = 0;
 };
 
@@ -95,13 +97,14 @@ struct Blob {                       // append-only byte buffer with 16-byte alig
     template <class T> u64 add(const std::vector<T>& v) { return add(v.data(), v.size() * sizeof(T)); }
 };
 
-struct PlanResult { int32_t rc = 0; std::string err; };
+#define ASTRA_N_TOPO_TABLES 7
+#define ASTRA_N_COLL_TABLES 7
 
 // loader entry points (astra_loader.cpp)
 int32_t astra_build_topo(HostTopo& t, std::string& err);
 int32_t astra_build_coll(HostColl& c, std::string& err);
 int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, u64 flags, u64 max_cycles,
-                         u64 topo_off[10], u64 coll_off[7], Blob& blob, PointDesc& out, double& cost,
+                         const u64* topo_off, const u64* coll_off, Blob& blob, PointDesc& out, double& cost,
                          std::string& err);
 
 // engine entry points (astra_engine.cu)

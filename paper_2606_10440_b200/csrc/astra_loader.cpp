@@ -1,8 +1,9 @@
 // astra_loader.cpp -- host loader of the engine (untimed prep):
 // validation (include/astra.h rules), min-latency routing with the (dst mod k) tie-break (R5,
-// PAPER.md:L221 "modular routing function"), candidate tables for the warp-parallel arrival and
-// acceptance phases, successor CSR of the step DAG (R3), per-CU in-order step lists and quota
-// split (R11), ring capacities, lookahead window, and the SoA workspace layout.
+// PAPER.md:L221 "modular routing function"), successor CSR of the step DAG (R3), per-CU in-order
+// step lists and quota split (R11), link ring capacities, link service kinds (R9), the per-window
+// staging cells that fix the same-cycle FIFO append order (R7/R8), the lookahead window, and the
+// SoA workspace layout.
 //
 // Independent of oracle/: the oracle routes with Bellman-Ford sweeps, this file with a heap
 // Dijkstra; they share no code.
@@ -94,27 +95,6 @@ int32_t astra_build_topo(HostTopo& t, std::string& err) {
                 }
         }
     }
-    // candidate tables: per node, for in-links (ceilB + 1 entries: the extra one peeks the next
-    // arrival) and out-links (ceilB entries); a link's block never straddles a 32-entry chunk.
-    auto build = [&](const std::vector<u32>& ptr, const std::vector<u32>* linkmap, u32 extra,
-                     std::vector<u32>& cptr, std::vector<u32>& cand) {
-        cptr.assign(V + 1, 0); cand.clear();
-        for (u32 v = 0; v < V; v++) {
-            cptr[v] = (u32)cand.size();
-            u32 pos = 0;
-            for (u32 i = ptr[v]; i < ptr[v + 1]; i++) {
-                u32 e = linkmap ? (*linkmap)[i] : i;
-                u32 ceilb = (t.bw[e] + 255) / 256;
-                u32 blk = ceilb + extra;
-                if ((pos & 31) + blk > 32) { u32 pad = 32 - (pos & 31); for (u32 j = 0; j < pad; j++) cand.push_back(ASTRA_CAND_PAD); pos += pad; }
-                for (u32 k = 0; k < blk; k++) cand.push_back(astra_cand_pack(e, ceilb, k));
-                pos += blk;
-            }
-        }
-        cptr[V] = (u32)cand.size();
-    };
-    build(t.in_ptr, &t.in_link, 1, t.icand_ptr, t.icand);
-    build(t.row_ptr, nullptr, 0, t.ocand_ptr, t.ocand);
     return ASTRA_OK;
 }
 
@@ -164,9 +144,17 @@ int32_t astra_build_coll(HostColl& c, std::string& err) {
 // ---------------------------------------------------------------------------------------------
 // Plan one design point: plan tables into the blob, workspace layout into the descriptor.
 // topo_off / coll_off are the blob offsets of the shared topology / collective tables.
+//
+// Staging cells (R7/R8).  The same-cycle append order into a link FIFO is fixed: transit lines
+// by ascending in-link id of the node, each in pipe order, then the node's own injections by
+// ascending wavefront id.  The engine gives every out-link of node v one cell per cycle of the
+// window with a FIXED slot layout: in-link i of v owns ceil(B_i) consecutive slots (a link
+// delivers at most ceil(B) lines per cycle), then H slots for injections (at most H issues per
+// GPU per cycle).  A line's slot is therefore known without any atomic allocation, and reading
+// a cell's occupied slots in slot order IS the FIFO order.
 // ---------------------------------------------------------------------------------------------
 int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, u64 flags, u64 max_cycles,
-                         u64 topo_off[10], u64 coll_off[7], Blob& blob, PointDesc& P, double& cost,
+                         const u64* topo_off, const u64* coll_off, Blob& blob, PointDesc& P, double& cost,
                          std::string& err) {
     std::memset(&P, 0, sizeof(P));
     const u32 G = t.G, V = t.V, E = t.E, S = c.S;
@@ -189,6 +177,8 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     }
     P.logW = logW;
     const u32 W = 1u << logW;
+    const u32 NC = W + 1;
+    P.NC = NC;
 
     std::vector<u32> step_q(S), step_r(S), first_link(S), step_alpha(S);
     u32 alpha_max = 1;
@@ -200,17 +190,19 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         u32 m = c.cu_n[s] * g.Wv;
         step_q[s] = c.lines[s] / m; step_r[s] = c.lines[s] % m;
     }
-    u32 nw = pow2ceil((u64)(alpha_max + W - 1) / W + 2);
-    P.NW = nw;
+    u64 nw64 = pow2ceil((u64)(alpha_max + W - 1) / W + 2);
+    if (nw64 > ASTRA_NW_MAX) { err = "route latency / lookahead window ratio above the engine limit"; return ASTRA_ELIMIT; }
+    P.NW = (u32)nw64;
 
-    // per-CU in-order step lists (R11) and per-owner release-list regions
-    std::vector<u32> cul_ptr((size_t)G * g.C + 1, 0), rel_off(G + 1, 0);
+    // per-CU in-order step lists (R11), per-owner release-list regions, per-GPU event-list regions
+    std::vector<u32> cul_ptr((size_t)G * g.C + 1, 0), rel_off(G + 1, 0), ev_off(G + 1, 0);
     for (u32 s = 0; s < S; s++) {
         for (u32 cu = c.cu_lo[s]; cu < c.cu_lo[s] + c.cu_n[s]; cu++) cul_ptr[(size_t)c.owner[s] * g.C + cu + 1]++;
         rel_off[c.owner[s] + 1]++;
+        ev_off[c.owner[s] + 1]++; ev_off[c.dst[s] + 1]++;     // one ACKED event at the owner, one DELIVERED at dst
     }
     for (size_t i = 0; i < (size_t)G * g.C; i++) cul_ptr[i + 1] += cul_ptr[i];
-    for (u32 i = 0; i < G; i++) rel_off[i + 1] += rel_off[i];
+    for (u32 i = 0; i < G; i++) { rel_off[i + 1] += rel_off[i]; ev_off[i + 1] += ev_off[i]; }
     std::vector<u32> cul(cul_ptr.back());
     {
         std::vector<u32> fill((size_t)G * g.C, 0);
@@ -223,7 +215,6 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     std::vector<u32> init_rel(S ? S : 1, 0), init_rel_cnt(G, 0);
     for (u32 s = 0; s < S; s++)
         if (c.ndeps[s] == 0) { u32 o = c.owner[s]; init_rel[rel_off[o] + init_rel_cnt[o]++] = s; }
-    P.n_rel_total = S;
 
     // ring capacities: lines that can sit in / fly over link e are bounded by the outstanding
     // lines of the owners routed through it.
@@ -248,57 +239,80 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
             for (u32 e : touched) { bound[e] += std::min<u64>(slots, via[e]); via[e] = 0; }
         }
     }
-    std::vector<u32> fifo_off(E), fifo_mask(E), pipe_off(E), pipe_mask(E), credit_cap(E);
-    u64 fifo_total = 0, pipe_total = 0;
+    // staging cells: slot layout per node, regions per link
+    std::vector<u32> nd_cellcap(V), nd_mw(V), nd_injoff(V), classoff(E, 0);
+    for (u32 v = 0; v < V; v++) {
+        u32 off = 0;
+        for (u32 i = t.in_ptr[v]; i < t.in_ptr[v + 1]; i++) {
+            u32 e = t.in_link[i];
+            classoff[e] = off;
+            off += (t.bw[e] + 255) / 256;
+        }
+        nd_injoff[v] = off;
+        nd_cellcap[v] = off + (v < G ? g.H : 0);
+        if (nd_cellcap[v] == 0) nd_cellcap[v] = 1;
+        nd_mw[v] = (nd_cellcap[v] + 31) / 32;
+    }
+    std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), credit_cap(E), lstate0(E), stage_off(E), mask_off(E);
+    u64 ring_total = 0, stage_total = 0, mask_total = 0;
     for (u32 e = 0; e < E; e++) {
         u32 ceilb = (t.bw[e] + 255) / 256;
+        ceilb_v[e] = ceilb;
         credit_cap[e] = ceilb * 256;
-        u32 fc = std::max<u32>(32, pow2ceil(bound[e]));
-        u64 pin = std::min<u64>(bound[e], (u64)ceilb * ((u64)t.leff[e] + W));
-        u32 pc = std::max<u32>(32, pow2ceil(pin));
-        if (fifo_total + fc >= (1ull << 32) || pipe_total + pc >= (1ull << 32)) { err = "ring space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
-        fifo_off[e] = (u32)fifo_total; fifo_mask[e] = fc - 1; fifo_total += fc;
-        pipe_off[e] = (u32)pipe_total; pipe_mask[e] = pc - 1; pipe_total += pc;
+        if (t.bw[e] % 256 == 0) { lkind[e] = ASTRA_LK_INT | ((t.bw[e] / 256) << 2); lstate0[e] = 0; }
+        else if (256 % t.bw[e] == 0) { lkind[e] = ASTRA_LK_PERIOD | ((256 / t.bw[e]) << 2); lstate0[e] = 0; }   // next accept not before cycle 0
+        else { lkind[e] = ASTRA_LK_GENERAL | (t.bw[e] << 2); lstate0[e] = credit_cap[e]; }
+        u32 rc = std::max<u32>(32, pow2ceil(bound[e]));
+        if (ring_total + rc >= (1ull << 32)) { err = "ring space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
+        ring_off[e] = (u32)ring_total; ring_mask[e] = rc - 1; ring_total += rc;
+        u32 v = t.tail[e];
+        u64 st = (u64)NC * nd_cellcap[v], mk = (u64)NC * nd_mw[v];
+        if (stage_total + st >= (1ull << 32)) { err = "staging space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
+        stage_off[e] = (u32)stage_total; stage_total += st;
+        mask_off[e] = (u32)mask_total; mask_total += mk;
     }
 
     // constant tables
-    P.c_row_ptr = topo_off[0]; P.c_in_ptr = topo_off[1]; P.c_in_link = topo_off[2]; P.c_leff = topo_off[3];
-    P.c_bw = topo_off[4]; P.c_icand_ptr = topo_off[5]; P.c_icand = topo_off[6]; P.c_ocand_ptr = topo_off[7];
-    P.c_ocand = topo_off[8]; P.c_next_link = topo_off[9];
+    P.c_in_ptr = topo_off[0]; P.c_in_link = topo_off[1]; P.c_head = topo_off[2]; P.c_tail = topo_off[3];
+    P.c_leff = topo_off[4]; P.c_bw = topo_off[5]; P.c_next_link = topo_off[6];
     P.c_step_od = coll_off[0]; P.c_lines = coll_off[1]; P.c_cu_lo = coll_off[2]; P.c_cu_n = coll_off[3];
     P.c_succ_ptr = coll_off[4]; P.c_succ = coll_off[5]; P.c_ndeps = coll_off[6];
     P.c_step_q = blob.add(step_q); P.c_step_r = blob.add(step_r); P.c_first_link = blob.add(first_link);
     P.c_step_alpha = blob.add(step_alpha); P.c_cul_ptr = blob.add(cul_ptr); P.c_cul = blob.add(cul);
     P.c_rel_off = blob.add(rel_off); P.c_init_rel = blob.add(init_rel); P.c_init_rel_cnt = blob.add(init_rel_cnt);
-    P.c_fifo_off = blob.add(fifo_off); P.c_fifo_mask = blob.add(fifo_mask);
-    P.c_pipe_off = blob.add(pipe_off); P.c_pipe_mask = blob.add(pipe_mask); P.c_credit_cap = blob.add(credit_cap);
+    P.c_ev_off = blob.add(ev_off);
+    P.c_ring_off = blob.add(ring_off); P.c_ring_mask = blob.add(ring_mask); P.c_lkind = blob.add(lkind);
+    P.c_ceilb = blob.add(ceilb_v); P.c_lstate0_init = blob.add(lstate0);
+    P.c_stage_off = blob.add(stage_off); P.c_mask_off = blob.add(mask_off); P.c_classoff = blob.add(classoff);
+    P.c_nd_cellcap = blob.add(nd_cellcap); P.c_nd_mw = blob.add(nd_mw); P.c_nd_injoff = blob.add(nd_injoff);
 
     // workspace layout
     u64 off = 0;
     auto take = [&](u64 bytes) { u64 o = off; off = (off + bytes + 15) & ~15ull; return o; };
     const u64 GW = (u64)G * CW;
+    const u32 nw = P.NW;
     // zero region
-    P.w_fifo_head = take(4ull * E); P.w_fifo_tail = take(4ull * E); P.w_pipe_tail = take(4ull * E);
-    P.w_pipe_tail_pub = take(4ull * E); P.w_pipe_head = take(4ull * E); P.w_pipe_tsnap = take(4ull * E);
-    P.w_credit_time = take(4ull * E); P.w_link_lines = take(4ull * E);
-    P.w_issued_cnt = take(4ull * S); P.w_deliv_cnt = take(4ull * S); P.w_ack_cnt = take(4ull * S);
-    P.w_wf_busy = take(8ull * GW); P.w_want = take(4ull * G * P.nwords); P.w_freeb = take(4ull * G * P.nwords);
-    P.w_pend_cnt = take(4ull * G); P.w_rel_cnt = take(4ull * G);
+    P.w_pipe_head = take(4ull * E); P.w_fifo_head = take(4ull * E); P.w_tail = take(4ull * E);
+    P.w_lstate1 = take(4ull * E); P.w_link_lines = take(4ull * E); P.w_masks = take(4ull * mask_total);
+    P.w_issued_cnt = take(4ull * S); P.w_t_issued = take(4ull * S); P.w_deliv_cnt = take(4ull * S);
+    P.w_t_deliv = take(4ull * S); P.w_ack_cnt = take(4ull * S); P.w_t_ack = take(4ull * S); P.w_rel_time = take(4ull * S);
+    P.w_wf_busy = take(8ull * GW); P.w_want = take(4ull * G * P.nwords);
     P.w_bitmap = take(4ull * G * nw * P.bmwords); P.w_bin_cnt = take(4ull * G * nw);
-    P.w_node_next = take(4ull * V); P.w_node_busy = take(8ull * V); P.w_node_acked = take(4ull * V);
+    P.w_ack_n = take(4ull * G); P.w_ev_cnt = take(4ull * G);
     P.ws_zero_bytes = off;
     // 0xff region
     P.ws_ff_off = off;
-    P.w_t_release = take(4ull * S); P.w_t_issued = take(4ull * S); P.w_t_deliv = take(4ull * S);
-    P.w_t_ack = take(4ull * S); P.w_wf_rem = take(4ull * GW);
+    P.w_wf_rem = take(4ull * GW);
     P.ws_ff_bytes = off - P.ws_ff_off;
     // specially initialised
-    P.w_credit = take(4ull * E); P.w_ndep_left = take(4ull * S); P.w_wf_cur = take(4ull * GW);
-    P.w_rel_list = take(4ull * (S ? S : 1));
+    P.w_lstate0 = take(4ull * E); P.w_t_release = take(4ull * S); P.w_ndep_left = take(4ull * S);
+    P.w_wf_cur = take(4ull * GW); P.w_freeb = take(4ull * G * P.nwords);
+    P.w_plist = take(4ull * (S ? S : 1)); P.w_pcnt = take(4ull * G);
     // uninitialised
-    P.w_fifo_buf = take(8ull * fifo_total); P.w_pipe_buf = take(8ull * pipe_total);
-    P.w_pend = take(8ull * G * g.H); P.w_pend_link = take(4ull * G * g.H); P.w_sel = take(4ull * G * g.H);
+    P.w_ring = take(8ull * ring_total); P.w_stage = take(8ull * stage_total);
+    P.w_sel = take(4ull * G * g.H);
     P.w_ack_rec = take(8ull * G * slots); P.w_ack_tmp = take(8ull * G * slots); P.w_ack_sorted = take(8ull * G * slots);
+    P.w_ev_list = take(4ull * (ev_off[G] ? ev_off[G] : 1));
     P.ws_bytes = off;
     return ASTRA_OK;
 }
