@@ -16,11 +16,17 @@ EXPORTED_SYMBOLS = [
     "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",
     "astra_load_infragraph", "astra_load_collective", "astra_set_gpu",
     "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
-    "astra_last_run_info", "astra_last_transfer_bytes",
+    "astra_last_run_info", "astra_last_transfer_bytes", "astra_read_diag",
 ]
 
 FLAG_NO_WINDOW_SKIP = 1
 FLAG_WINDOW_1 = 2
+
+
+def FLAG_GROUP(g: int) -> int:
+    """ASTRA_FLAG_GROUP(g): run every design point on a group of g CTAs."""
+    return (g & 0xFF) << 8
+
 TS_NONE = np.uint64(0xFFFFFFFFFFFFFFFF)
 
 
@@ -80,6 +86,7 @@ def load_library(path: Optional[str] = None):
     lib.astra_run_batch_async.argtypes = [vp, u32, vp, u64]
     lib.astra_sync.argtypes = [vp]
     lib.astra_read_results.argtypes = [vp, u32, ctypes.POINTER(_Summary), vp, vp]
+    lib.astra_read_diag.argtypes = [vp, u32, vp]
     lib.astra_last_run_info.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u32), ctypes.POINTER(u64)]
     lib.astra_last_transfer_bytes.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     for name in EXPORTED_SYMBOLS:
@@ -185,6 +192,11 @@ class Engine:
         return (summ,
                 step_ts[:4 * s.n_steps].reshape(s.n_steps, 4) if want_steps else None,
                 link_lines[:s.n_links] if want_links else None)
+
+    def read_diag(self, point: int) -> np.ndarray:
+        out = np.zeros(8, dtype=np.uint64)
+        self._check(self._lib.astra_read_diag(self._ctx, point, _ptr(out)))
+        return out
 
     def last_run_info(self):
         ms, n, b = ctypes.c_float(), ctypes.c_uint32(), ctypes.c_uint64()

@@ -6,25 +6,29 @@
 // node before a + Leff, and an ack cannot reach its owner before t_deliv + alpha >= t_deliv +
 // min Leff.  With W = 2^k <= min Leff, nothing a node does inside the window [kW, (k+1)W) can
 // influence another node inside the same window.  So simulated time advances a whole window at a
-// time, and inside a window every phase of rules R7-R12 is a data-parallel pass over ALL events
-// of the window instead of a serial walk over cycles:
+// time, every stage of a window is node-local, and inside a window every phase of rules R7-R12
+// is a data-parallel pass over ALL events of the window instead of a serial walk over cycles:
 //
-//   stage 1  arrivals (R7 A1)   one warp per link, 32 pipe entries per step: deliveries bump
-//            the step counters and post slot-addressed ack records; transit lines drop into the
-//            staging cell (out-link, cycle) at a slot fixed by (in-link, position) -- the FIFO
-//            append order of R8 without atomics or sorting.
-//            ack gather (R6, A3) one warp per GPU: this window's acks, counting-sorted by cycle,
-//            per-step ack counts and t_ack.
+//   stage 1  arrivals (R7 A1)   one warp per in-link, 32 pipe entries per step: deliveries bump
+//            the step counters and post slot-addressed ack records; a transit line either goes
+//            straight to the tail of the next link's ring (that link has a single feeder) or
+//            sets one bit in the (out-link, cycle) cell at a slot fixed by (in-link, position).
+//            ack gather (R6, A3) one warp per GPU: this window's acks, counting-sorted by cycle.
 //   stage 2  release + issue (R10-R13) one warp per GPU: dependency events of the window become
 //            timed releases; the fixed-priority HBM grant scan walks only the cycles of the
-//            window where something can change; issued lines drop into their staging cell.
-//   stage 3  link service (R9)  one warp per link: the occupied staging slots of the window, read
-//            in slot order, are the FIFO appends; acceptance times of the whole FIFO follow from
+//            window where something can change; issued lines are appended / recorded.
+//   stage 3  merge (R7/R8 append order) per out-link with several feeders: prefix sum of the
+//            cell popcounts = FIFO position of every slot; the feeders then write their lines
+//            straight to those positions.  No atomically allocated slot, no sort.
+//   stage 4  link service (R9)  one warp per link: acceptance times of the whole FIFO follow from
 //            a prefix-max scan (integer and 1/P bandwidths) or a credit walk (any other), and the
 //            accepted lines are stamped with their arrival cycle in the link's ring.
-//   stage 4  next non-idle window (A7): min over pending arrivals, acks, backlog and ready work.
+//   stage 5  next non-idle window (A7): min over pending arrivals, acks, backlog and ready work.
 //
-// One CTA simulates one design point at a time and pulls the next from a cost-sorted queue.
+// Hot per-node state (link cursors, cells, ready masks, wavefront records, step counters) lives
+// in shared memory whenever the loader could fit it (PointDesc::a_off placement flags); rings and
+// ack records stream through L2/HBM.  One CTA (or a group of CTAs, one node range each, with one
+// group barrier per window) simulates one design point and pulls the next from a cost-sorted queue.
 #include "astra_internal.h"
 #include "../../include/astra.h"
 
@@ -35,33 +39,40 @@
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
     u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, logW, W, NC, NWmask, NW, kmagic, tmax, flags;
+    u32 group, rank, v_lo, v_hi, g_lo, g_hi, e_lo, e_hi, i_lo, i_hi;
     u64 fullmask;
-    const u32 *in_ptr, *in_link, *head, *tail, *leff, *bw, *next_link;
-    const u32 *step_od, *lines, *cu_lo, *cu_n, *succ_ptr, *succ, *ndeps;
-    const u32 *step_q, *step_r, *first_link, *step_alpha, *cul_ptr, *cul, *rel_off, *init_rel, *init_rel_cnt, *ev_off;
-    const u32 *ring_off, *ring_mask, *lkind, *ceilb, *lstate0_init, *stage_off, *mask_off, *classoff;
-    const u32 *nd_cellcap, *nd_mw, *nd_injoff;
-    u32 *pipe_head, *fifo_head, *ltail, *lstate0, *lstate1, *link_lines, *masks;
-    u64 *ring, *stage;
-    u32 *t_release, *issued_cnt, *t_issued, *deliv_cnt, *t_deliv, *ack_cnt, *t_ack, *ndep_left, *rel_time;
-    u32 *wf_rem, *wf_cur; u64 *wf_busy;
-    u32 *want, *freeb, *sel, *plist, *pcnt, *ev_list, *ev_cnt, *ack_n;
-    u64 *ack_rec, *ack_tmp, *ack_sorted; u32 *bitmap, *bin_cnt;
-    u64 *r_step_ts, *r_link_lines; DeviceSummary *r_summary;
+#define X(n) const u32* n;
+    ASTRA_CONST_TABLES(X)
+#undef X
+#define X(n, t, i) t* n;
+    ASTRA_WS_ARRAYS(X)
+#undef X
+    u64 *r_step_ts, *r_link_lines, *r_diag; DeviceSummary* r_summary;
 };
 
 struct Ctl {   // per-CTA control block in shared memory
     u32 point;          // index into the order array
-    u32 acked;          // steps fully acked so far
+    u32 acked;          // steps fully acked by this CTA's GPUs since the last group reduction
     u32 completion;     // max t_ack
     u32 err;            // engine self-check flags
     u32 next_hint;      // min over everything pending of its next event time
     u32 decision;       // 0 = run window `next_k`, else 1 + status
     u32 next_k;
-    u32 pad;
+    u32 any_merged;     // some multi-feeder out-link received lines this window
+    u32 acked_total, pad;
     u64 busy, skipped;
-    u32 ackwin[ASTRA_NW_MAX];   // acks posted per future window bin
+    u64 clk[8];         // diagnostics: [0] windows, [1..4] SM clocks in stage groups, [5] init
 };
+
+__device__ const unsigned char k_arr_init[ASTRA_A_COUNT] = {
+#define X(n, t, i) i,
+    ASTRA_WS_ARRAYS(X)
+#undef X
+};
+
+// Arrays that the loader may place in shared OR global memory and that another CTA of a group may
+// have written: a volatile generic load (never served from a stale L1 line, legal on both spaces).
+__device__ __forceinline__ u32 ld_vol(const u32* p) { return *(const volatile u32*)p; }
 
 __device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
@@ -76,36 +87,56 @@ __device__ __forceinline__ int warp_incl_max(int v, u32 lane) {
     return v;
 }
 
-// Put one flit payload into the staging cell (out-link o, cycle t0 + d) at `slot` (R7/R8).
-__device__ __forceinline__ void stage_put(Ctx& c, u32 o, u32 v, u32 cb, u32 d, u32 slot, u64 payload) {
+// Mark slot `slot` of the cell (out-link o at node v, cycle t0 + d) occupied (R7/R8).
+__device__ __forceinline__ void cell_set(Ctx& c, Ctl& ctl, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
     u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
-    c.stage[(size_t)c.stage_off[o] + (size_t)ci * c.nd_cellcap[v] + slot] = payload;
-    atomicOr(&c.masks[(size_t)c.mask_off[o] + (size_t)ci * c.nd_mw[v] + (slot >> 5)], 1u << (slot & 31));
+    atomicOr(&c.masks[c.mask_off[o] + ci * c.nd_mw[v] + (slot >> 5)], 1u << (slot & 31));
+    c.dirty[o] = 1u;
+    ctl.any_merged = 1u;
+}
+// FIFO position, relative to the tail at the window start, of the line in slot `slot` of that cell.
+__device__ __forceinline__ u32 cell_pos(Ctx& c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
+    u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
+    const u32 mw = c.nd_mw[v];
+    const u32* words = c.masks + c.mask_off[o] + ci * mw;
+    u32 r = c.pre[c.pre_off[o] + d];
+    const u32 sw = slot >> 5;
+    for (u32 w = 0; w < sw; w++) r += __popc(words[w]);
+    return r + __popc(words[sw] & ((1u << (slot & 31)) - 1u));
 }
 
 // ---------------------------------------------------------------------------------------------
-// stage 1a: arrivals on link e during [t0, t0 + wlen)   (R7 A1)
+// stage 1a / 3b: arrivals on in-link stream i during [t0, t0 + wlen)   (R7 A1)
+// PASS 1 delivers, appends to single-feeder out-links and marks cells; PASS 3 (after the prefix
+// sums) writes the lines that go to multi-feeder out-links at their FIFO positions.
 // ---------------------------------------------------------------------------------------------
-__device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 wlen, u32 cb, u32 lane) {
-    const u32 lo = c.pipe_head[e], hi = c.fifo_head[e];
+template <int PASS>
+__device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 t0, u32 wlen, u32 cb, u32 lane) {
+    const u32 e = c.in_link[i];
+    const u32 lo = c.pipe_head[e];
+    u32 hi;
+    if (PASS == 1) hi = ld_vol(&c.fifo_head[e]);
+    else hi = lo + c.ndue[e];
     if (lo == hi) return;
     const u32 v = c.head[e];
     const u64* ring = c.ring + c.ring_off[e];
     const u32 rmask = c.ring_mask[e], coff = c.classoff[e];
+    if (PASS == 1 && lane == 0 && hi - lo > rmask + 1) atomicOr(&ctl.err, 1u);
     u32 carry_d = 0xffffffffu, carry_cnt = 0, idx = lo, ndue = 0, hint = ASTRA_T_INF;
+    bool any_p3 = false;
     for (;;) {
-        const u32 i = idx + lane;
-        const bool valid = (int32_t)(hi - i) > 0;
-        const u64 flit = valid ? ring[i & rmask] : 0ull;
+        const u32 ii = idx + lane;
+        const bool valid = (int32_t)(hi - ii) > 0;
+        const u64 flit = valid ? __ldcg(&ring[ii & rmask]) : 0ull;
         const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
         const bool due = valid && d < wlen;
         const u32 duemask = __ballot_sync(FULL, due);
-        if (valid && !due) hint = min(hint, t0 + d);
+        if (PASS == 1 && valid && !due) hint = min(hint, t0 + d);
         if (duemask) {
             // position of the line among the lines this link delivers in the same cycle
-            u32 r = 0, grp = 0;
+            u32 r = 0;
             if (due) {
-                grp = __match_any_sync(duemask, d);
+                const u32 grp = __match_any_sync(duemask, d);
                 r = __popc(grp & lanemask_lt()) + (d == carry_d ? carry_cnt : 0u);
             }
             const u32 last = 31 - __clz(duemask);
@@ -118,45 +149,74 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 wlen, u32 cb,
             const u32 dstg = od & 0xffffu;
             const bool deliver = due && dstg == v;
             const bool transit = due && !deliver;
-            if (transit) {
-                const u32 o = c.next_link[(size_t)v * c.G + dstg];
-                stage_put(c, o, v, cb, d, coff + r, flit & ASTRA_FLIT_PAYLOAD_MASK);
-            }
-            const u32 dmask = __ballot_sync(FULL, deliver);
-            if (dmask) {
-                bool completed = false;
-                if (deliver) {
-                    const u32 owner = od >> 16;
-                    const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
-                    const u32 ta = t0 + d + c.step_alpha[step];                       // R6
-                    const u32 bit = wf * c.K + slot;
-                    c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
-                    const u32 bin = (ta >> c.logW) & c.NWmask;
-                    atomicOr(&c.bitmap[(size_t)(owner * c.NW + bin) * c.bmwords + (bit >> 5)], 1u << (bit & 31));
-                    atomicAdd(&c.bin_cnt[owner * c.NW + bin], 1u);
-                    atomicAdd(&ctl.ackwin[bin], 1u);
-                    const u32 m = __match_any_sync(dmask, step);
-                    const u32 dmax = __reduce_max_sync(m, d);
-                    if ((m & lanemask_lt()) == 0) {
-                        const u32 dc = c.deliv_cnt[step] + __popc(m);
-                        c.deliv_cnt[step] = dc;
-                        if (dc == c.lines[step]) { c.t_deliv[step] = t0 + dmax; completed = true; }
+            u32 o = 0, moff = 0;
+            if (transit) { o = c.next_link[(size_t)v * c.G + dstg]; moff = c.mask_off[o]; }
+            const bool direct = transit && moff == ASTRA_NONE32;
+            const bool merged = transit && !direct;
+            if (PASS == 1) {
+                if (merged) { cell_set(c, ctl, o, v, cb, d, coff + r); any_p3 = true; }
+                const u32 dm = __ballot_sync(FULL, direct);
+                if (dm) {       // this stream is the only feeder of o: append in stream order
+                    u32 grp = 0, base = 0;
+                    if (direct) {
+                        grp = __match_any_sync(dm, o);
+                        base = c.run[o];
+                        const u32 pos = base + __popc(grp & lanemask_lt());
+                        c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] =
+                            (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+                    }
+                    __syncwarp();
+                    if (direct && (grp & lanemask_lt()) == 0) c.run[o] = base + __popc(grp);
+                    __syncwarp();
+                }
+                const u32 dmask = __ballot_sync(FULL, deliver);
+                if (dmask) {
+                    bool completed = false;
+                    if (deliver) {
+                        const u32 owner = od >> 16;
+                        const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
+                        const u32 ta = t0 + d + c.step_alpha[step];                       // R6
+                        const u32 bit = wf * c.K + slot;
+                        c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
+                        const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+                        atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
+                        const u32 mb = __match_any_sync(dmask, bin);
+                        if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+                        hint = min(hint, ta);
+                        const u32 m = __match_any_sync(dmask, step);
+                        const u32 dmax = __reduce_max_sync(m, d);
+                        if ((m & lanemask_lt()) == 0) {
+                            const u32 dc = c.deliv_cnt[step] + __popc(m);
+                            c.deliv_cnt[step] = dc;
+                            if (dc == c.lines[step]) { c.t_deliv[step] = t0 + dmax; completed = true; }
+                        }
+                    }
+                    if (completed) {      // DELIVERED event at GPU v (dst of the step)
+                        const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
+                        c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
                     }
                 }
-                if (completed) {      // DELIVERED event at GPU v (dst of the step)
-                    const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
-                    c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
-                }
+            } else if (merged) {
+                const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, coff + r);
+                c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] =
+                    (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
             }
             ndue += __popc(duemask);
         }
         if (duemask != FULL) break;
         idx += 32;
     }
-    hint = __reduce_min_sync(FULL, hint);
-    if (lane == 0) {
+    if (PASS == 1) {
+        hint = __reduce_min_sync(FULL, hint);
+        any_p3 = __any_sync(FULL, any_p3);
+        if (lane == 0) {
+            if (any_p3) c.ndue[e] = ndue;           // pass 3 walks the same entries again
+            else c.pipe_head[e] = lo + ndue;
+            if (hint != ASTRA_T_INF) atomicMin(&ctl.next_hint, hint);
+        }
+    } else if (lane == 0) {
         c.pipe_head[e] = lo + ndue;
-        if (hint != ASTRA_T_INF) atomicMin(&ctl.next_hint, hint);
+        c.ndue[e] = 0;
     }
 }
 
@@ -165,7 +225,18 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 wlen, u32 cb,
 // ---------------------------------------------------------------------------------------------
 __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
     const u32 bin = k & c.NWmask;
-    const u32 n = c.bin_cnt[g * c.NW + bin];
+    // earliest later window with acks pending for this GPU (A7)
+    {
+        u32 best = ASTRA_T_INF;
+        for (u32 j = 1 + lane; j < c.NW; j += 32)
+            if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
+        best = __reduce_min_sync(FULL, best);
+        if (lane == 0 && best != ASTRA_T_INF) {
+            const u64 tw = (u64)(k + best) << c.logW;
+            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
+        }
+    }
+    const u32 n = ld_vol(&c.bin_cnt[g * c.NW + bin]);
     if (lane == 0) c.ack_n[g] = n;
     if (n == 0) return;
     for (u32 i = lane; i <= wlen; i += 32) scnt[i] = 0;
@@ -178,7 +249,7 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
     u32 total = 0;
     for (u32 wb = 0; wb < c.bmwords; wb += 32) {
         const u32 wi = wb + lane;
-        u32 w = (wi < c.bmwords) ? bm[wi] : 0;
+        u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
         if (w) bm[wi] = 0;
         const u32 cnt = __popc(w);
         const u32 incl = warp_incl_scan(cnt, lane);
@@ -187,7 +258,7 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
         while (w) {
             const u32 b = __ffs(w) - 1; w &= w - 1;
             const u32 idx = wi * 32 + b;
-            const u64 rc = rec[idx];
+            const u64 rc = __ldcg(&rec[idx]);
             const u32 cyc = (u32)rc - t0;
             const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K (magic overflows for K == 1)
             const u32 slot = idx - wf * c.K;
@@ -229,16 +300,15 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
                     completed = true;
                     const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
                     c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
+                    completion = max(completion, tm);
                 }
             }
-            if (completed) completion = max(completion, max(c.t_ack[step], t0 + cmax));
         }
         acked_steps += __popc(__ballot_sync(FULL, completed));
     }
     completion = __reduce_max_sync(FULL, completion);
     if (lane == 0) {
         c.bin_cnt[g * c.NW + bin] = 0;
-        atomicSub(&ctl.ackwin[bin], total);
         if (total != n) atomicOr(&ctl.err, 2u);
         if (acked_steps) { atomicAdd(&ctl.acked, acked_steps); atomicMax(&ctl.completion, completion); }
     }
@@ -309,14 +379,19 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
         if (lane == 0 && nev) c.ev_cnt[g] = 0;
     }
     const u32 ack_n = c.ack_n[g];
-    u32 ack_pos = 0;
     const u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32* plist = c.plist + c.rel_off[g];
     u32* want = c.want + (size_t)g * c.nwords;
     u32* freeb = c.freeb + (size_t)g * c.nwords;
     u32* sel = c.sel + (size_t)g * c.H;
+    u64* inj = c.inj_list + c.inj_off[g];
+    const u32 inj_cap = c.inj_off[g + 1] - c.inj_off[g];
+    u32 n_inj = c.inj_n[g];
     const u32 injoff = c.nd_injoff[g];
-    u32 t_ack_next = ack_n ? t0 + ((u32)srt[0] >> 18) : ASTRA_T_INF;
+    // sorted acks are consumed from a register window of 32 entries
+    u32 ack_pos = 0, abase = 0;
+    u32 abuf = (lane < ack_n) ? (u32)srt[lane] : 0xffffffffu;       // low word: cyc << 18 | wf << 6 | slot
+    u32 t_ack_next = ack_n ? t0 + (__shfl_sync(FULL, abuf, 0) >> 18) : ASTRA_T_INF;
     u32 t_rel_next = ASTRA_T_INF;
     {
         const u32 np = c.pcnt[g];
@@ -337,15 +412,12 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
         // ---- slot return: acks due at t (R7 A3) ----
         if (t_ack_next == t) {
             const u32 cyc = t - t0;
-            while (ack_pos < ack_n) {
-                const u32 j = ack_pos + lane;
-                const u64 ent64 = (j < ack_n) ? srt[j] : ~0ull;
-                const u32 ent = (u32)ent64;
-                const bool now = (j < ack_n) && (ent >> 18) == cyc;
+            for (;;) {
+                const u32 j0 = ack_pos - abase;
+                const bool now = lane >= j0 && abase + lane < ack_n && (abuf >> 18) == cyc;
                 const u32 nm = __ballot_sync(FULL, now);
-                if (nm == 0) break;
                 if (now) {
-                    const u32 wf = (ent >> 6) & 0xfffu, slot = ent & 63u;
+                    const u32 wf = (abuf >> 6) & 0xfffu, slot = abuf & 63u;
                     // several acks of one wavefront may land in the same cycle
                     const u32 mw = __match_any_sync(nm, wf);
                     const u32 blo = __reduce_or_sync(mw, slot < 32 ? (1u << slot) : 0u);
@@ -361,10 +433,16 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
                     if ((mi & lanemask_lt()) == 0) freeb[wi] |= bits;
                 }
                 ack_pos += __popc(nm);
-                if (__popc(nm) < 32) break;
+                if (ack_pos - abase < 32 || ack_pos >= ack_n) break;
+                abase = ack_pos;                                     // register window exhausted: refill
+                abuf = (abase + lane < ack_n) ? (u32)srt[abase + lane] : 0xffffffffu;
             }
             __syncwarp();
-            t_ack_next = (ack_pos < ack_n) ? t0 + ((u32)srt[ack_pos] >> 18) : ASTRA_T_INF;
+            if (ack_pos >= ack_n) t_ack_next = ASTRA_T_INF;
+            else {
+                if (ack_pos - abase >= 32) { abase = ack_pos; abuf = (abase + lane < ack_n) ? (u32)srt[abase + lane] : 0xffffffffu; }
+                t_ack_next = t0 + (__shfl_sync(FULL, abuf, ack_pos - abase) >> 18);
+            }
         }
 
         // ---- phase C: releases that take effect at t (R10) ----
@@ -431,9 +509,11 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
             nsel += got; budget -= got;
         }
         __syncwarp();
+        const u32 d = t + 1 - t0;     // injected at t + 1 into the first-hop FIFO, after that cycle's transit lines (R7 A2)
         for (u32 b = 0; b < nsel; b += 32) {
             const u32 j = b + lane; const bool act = j < nsel;
-            u32 wf = 0, s = 0; bool full = false, keepw = true;
+            u32 wf = 0, s = 0, o = 0, moff = 0; bool full = false, keepw = true;
+            u64 payload = 0;
             if (act) {
                 wf = sel[j];
                 const size_t gw = (size_t)g * c.CW + wf;
@@ -445,12 +525,37 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
                 busy |= 1ull << slot;
                 c.wf_busy[gw] = busy;
                 full = (busy == c.fullmask);
-                // injected at t + 1 into the first-hop FIFO, after that cycle's transit lines (R7 A2)
-                stage_put(c, c.first_link[s], g, cb, t + 1 - t0, injoff + j, (u64)s | ((u64)wf << 20) | ((u64)slot << 32));
+                payload = (u64)s | ((u64)wf << 20) | ((u64)slot << 32);
+                o = c.first_link[s]; moff = c.mask_off[o];
                 if (rem == 0) { cur++; keepw = wf_advance(c, g, wf, cur, rem, t); c.wf_cur[gw] = cur; }
                 c.wf_rem[gw] = rem;
             }
             const u32 amask = __ballot_sync(FULL, act);
+            const bool direct = act && moff == ASTRA_NONE32;
+            const bool merged = act && !direct;
+            const u32 dm = __ballot_sync(FULL, direct);
+            if (dm) {            // this GPU is the only feeder of o: append in wavefront order
+                u32 grp = 0, base = 0;
+                if (direct) {
+                    grp = __match_any_sync(dm, o);
+                    base = c.run[o];
+                    const u32 pos = base + __popc(grp & lanemask_lt());
+                    c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = payload | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+                }
+                __syncwarp();
+                if (direct && (grp & lanemask_lt()) == 0) c.run[o] = base + __popc(grp);
+                __syncwarp();
+            }
+            const u32 mm = __ballot_sync(FULL, merged);
+            if (mm) {
+                if (merged) {
+                    cell_set(c, ctl, o, g, cb, d, injoff + j);
+                    const u32 p = n_inj + __popc(mm & lanemask_lt());
+                    if (p < inj_cap) inj[p] = payload | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
+                    else atomicOr(&ctl.err, 4u);
+                }
+                n_inj += __popc(mm);
+            }
             bool completed = false;
             if (act) {
                 const u32 ms = __match_any_sync(amask, s);
@@ -490,20 +595,21 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
         if (more) tn = min(tn, t + 1);
         t = tn;
     }
-    if (lane == 0 && t != ASTRA_T_INF) atomicMin(&ctl.next_hint, t);
+    if (lane == 0) {
+        c.inj_n[g] = n_inj;
+        if (t != ASTRA_T_INF) atomicMin(&ctl.next_hint, t);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
-// stage 3: link e over [t0, t1): FIFO appends of the window in slot order, acceptance times of
-// the whole FIFO (R9), arrival stamps.  `pre` is per-warp scratch of >= wlen + 1 words.
+// stage 3a: FIFO positions of the cells of multi-feeder out-link o: exclusive prefix over the
+// cell popcounts of the window (R7/R8: cycle by cycle, slot order inside a cycle).
 // ---------------------------------------------------------------------------------------------
-__device__ void link_window(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32* pre, u32 lane) {
-    const u32 wlen = t1 - t0;
-    const u32 v = c.tail[e];
-    const u32 cap = c.nd_cellcap[v], mw = c.nd_mw[v];
-    u32* masks = c.masks + c.mask_off[e];
-    const u64* stage = c.stage + c.stage_off[e];
-    // ---- appends per cycle of the window: exclusive prefix over the cells ----
+__device__ void link_prefix(Ctx& c, u32 o, u32 wlen, u32 cb, u32 lane) {
+    const u32 v = c.tail[o];
+    const u32 mw = c.nd_mw[v];
+    const u32* masks = c.masks + c.mask_off[o];
+    u32* pre = c.pre + c.pre_off[o];
     u32 n_new = 0;
     for (u32 b = 0; b < wlen; b += 32) {
         const u32 tau = b + lane; u32 cnt = 0;
@@ -515,15 +621,69 @@ __device__ void link_window(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32
         if (tau < wlen) pre[tau] = n_new + incl - cnt;
         n_new += __shfl_sync(FULL, incl, 31);
     }
-    const u32 fh = c.fifo_head[e], tl = c.ltail[e];
-    const u32 n_back = tl - fh;
-    if (n_new == 0 && n_back == 0) return;
-    if (lane == 0) pre[wlen] = n_new;
-    __syncwarp();
+    if (lane == 0) c.run[o] = c.ltail[o] + n_new;
+}
+
+// stage 3b: GPU g's recorded injections go to their FIFO positions; the ones that enter at the
+// first cycle of the next window stay recorded.
+__device__ void inject_place(Ctx& c, u32 g, u32 wlen, u32 cb, u32 lane) {
+    const u32 n = c.inj_n[g];
+    if (n == 0) return;
+    u64* inj = c.inj_list + c.inj_off[g];
+    const u32 injoff = c.nd_injoff[g];
+    u32 keep = 0;
+    for (u32 b = 0; b < n; b += 32) {
+        const u32 i = b + lane;
+        const bool act = i < n;
+        const u64 rec = act ? inj[i] : 0ull;
+        const u32 tf = (u32)(rec >> ASTRA_FLIT_TIME_SHIFT);
+        const u32 d = tf & 0x3ffu, j = (tf >> 10) & 0x3ffu;
+        const bool place = act && d < wlen;
+        const bool carry = act && !place;
+        if (place) {
+            const u32 o = c.first_link[(u32)rec & 0xfffffu];
+            const u32 pos = c.ltail[o] + cell_pos(c, o, g, cb, d, injoff + j);
+            c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+        }
+        const u32 cm = __ballot_sync(FULL, carry);
+        __syncwarp();
+        // records are in cycle order: the carried ones are the last; dst index <= src index
+        if (carry) inj[keep + __popc(cm & lanemask_lt())] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)(j << 10) << ASTRA_FLIT_TIME_SHIFT);
+        keep += __popc(cm);
+        __syncwarp();
+    }
+    if (lane == 0) c.inj_n[g] = keep;
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage 4: link e over [t0, t1): acceptance times of the whole FIFO (R9), arrival stamps.
+// ---------------------------------------------------------------------------------------------
+__device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32 lane) {
+    const u32 wlen = t1 - t0;
+    const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
+    if (c.dirty[e]) {                                        // consume the cells of the window
+        const u32 v = c.tail[e];
+        const u32 mw = c.nd_mw[v];
+        u32* masks = c.masks + c.mask_off[e];
+        for (u32 x = lane; x < wlen * mw; x += 32) {
+            u32 ci = cb + x / mw; if (ci >= c.NC) ci -= c.NC;
+            masks[ci * mw + x % mw] = 0;
+        }
+        __syncwarp();
+        if (lane == 0) {                                     // injections that enter at t1 keep the link marked
+            u32 ci = cb + wlen; if (ci >= c.NC) ci -= c.NC;
+            u32 any = 0;
+            for (u32 w = 0; w < mw; w++) any |= masks[ci * mw + w];
+            c.dirty[e] = any ? 1u : 0u;
+            if (any) ctl.any_merged = 1u;
+        }
+    }
+    const u32 n_back = tl - fh, n_new = tn - tl;
+    const u32 n_tot = n_back + n_new;
+    if (n_tot == 0) return;
     u64* ring = c.ring + c.ring_off[e];
     const u32 rmask = c.ring_mask[e];
-    if (lane == 0 && (tl + n_new) - c.pipe_head[e] > rmask + 1) atomicOr(&ctl.err, 1u);   // ring overflow guard
-    const u32 n_tot = n_back + n_new;
+    if (lane == 0 && tn - ld_vol(&c.pipe_head[e]) > rmask + 1) atomicOr(&ctl.err, 1u);     // ring overflow guard
     const u32 lk = c.lkind[e];
     const u32 kind = lk & 3u, param = lk >> 2;
     const u32 leff = c.leff[e];
@@ -538,59 +698,44 @@ __device__ void link_window(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32
     } else if (kind == ASTRA_LK_GENERAL) { cr = c.lstate0[e]; tc = c.lstate1[e]; }
     const u32 capq = c.ceilb[e] * 256u;
     u32 n_acc = 0, first_x = 0, last_x = 0;
-    bool saturated = (scan_limit == 0);
 
-    for (u32 base = 0; base < n_tot; base += 32) {
-        if (saturated && base + 32 <= n_back) {              // backlog that stays queued: nothing to do
-            base = (n_back & ~31u);
-            if (base >= n_tot) break;
-        }
+    for (u32 base = 0; base < scan_limit; base += 32) {
         const u32 i = base + lane;
-        const bool act = i < n_tot;
-        const bool isnew = act && i >= n_back;
-        u32 a = 0, tau = 0, q = 0;
-        if (isnew) {                                         // append cycle of the line: search the cell prefix
-            const u32 p = i - n_back;
-            u32 lo = 0, hi = wlen;                           // largest tau with pre[tau] <= p
-            while (hi - lo > 1) { const u32 mid = (lo + hi) >> 1; if (pre[mid] <= p) lo = mid; else hi = mid; }
-            tau = lo; q = p - pre[lo]; a = tau;
-        }
+        const bool act = i < scan_limit;
+        const u32 pos = (fh + i) & rmask;
+        const u64 flit = act ? ring[pos] : 0ull;
+        // append cycle relative to t0: backlog was appended before the window
+        const u32 a = (act && i >= n_back) ? ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) & 0x3ffu) : 0u;
         u32 x = 0xffffffffu;                                 // acceptance cycle relative to t0
-        if (!saturated) {
-            const bool in_scan = i < scan_limit;
-            if (kind == ASTRA_LK_INT) {
-                int val = in_scan ? (int)(param * a) - (int)i : INT_MIN;
-                int pm = warp_incl_max(val, lane);
-                pm = max(pm, run_max);
-                run_max = __shfl_sync(FULL, pm, 31);
-                if (in_scan) x = (u32)((int)i + pm) / param;
-            } else if (kind == ASTRA_LK_PERIOD) {
-                int val = in_scan ? (int)a - (int)(param * i) : INT_MIN;
-                int pm = warp_incl_max(val, lane);
-                pm = max(pm, run_max);
-                run_max = __shfl_sync(FULL, pm, 31);
-                if (in_scan) {
-                    // x_i = max(a_i, x_{i-1} + P) with x_{-1} + P = xn_rel
-                    const int xi = (int)(param * i) + max(pm, xn_rel);
-                    x = (u32)xi;
+        if (kind == ASTRA_LK_INT) {
+            int val = act ? (int)(param * a) - (int)i : INT_MIN;
+            int pm = warp_incl_max(val, lane);
+            pm = max(pm, run_max);
+            run_max = __shfl_sync(FULL, pm, 31);
+            if (act) x = (u32)((int)i + pm) / param;
+        } else if (kind == ASTRA_LK_PERIOD) {
+            int val = act ? (int)a - (int)(param * i) : INT_MIN;
+            int pm = warp_incl_max(val, lane);
+            pm = max(pm, run_max);
+            run_max = __shfl_sync(FULL, pm, 31);
+            // x_i = max(a_i, x_{i-1} + P) with x_{-1} + P = xn_rel
+            if (act) x = (u32)((int)(param * i) + max(pm, xn_rel));
+        } else {
+            // saturating credit walked in FIFO order; every lane tracks the same state
+            const u32 bw = param;
+            for (u32 j = 0; j < 32; j++) {
+                if (base + j >= scan_limit) break;
+                const u32 aj = t0 + __shfl_sync(FULL, a, j);
+                u32 tt = max(aj, tc);
+                u64 avail = min((u64)cr + (u64)(tt - tc) * bw, (u64)capq);
+                if (avail < 256) {
+                    const u32 wait = (u32)((256 - avail + bw - 1) / bw);
+                    tt += wait;
+                    avail = min(avail + (u64)wait * bw, (u64)capq);
                 }
-            } else {
-                // saturating credit walked in FIFO order; every lane tracks the same state
-                const u32 bw = param;
-                for (u32 j = 0; j < 32; j++) {
-                    if (base + j >= scan_limit) break;
-                    const u32 aj = t0 + __shfl_sync(FULL, a, j);
-                    u32 tt = max(aj, tc);
-                    u64 avail = min((u64)cr + (u64)(tt - tc) * bw, (u64)capq);
-                    if (avail < 256) {
-                        const u32 wait = (u32)((256 - avail + bw - 1) / bw);
-                        tt += wait;
-                        avail = min(avail + (u64)wait * bw, (u64)capq);
-                    }
-                    if (tt >= t1) break;                     // not in this window: state stays at the last accept
-                    cr = (u32)avail - 256u; tc = tt;
-                    if (j == lane) x = tt - t0;
-                }
+                if (tt >= t1) break;                     // not in this window: state stays at the last accept
+                cr = (u32)avail - 256u; tc = tt;
+                if (j == lane) x = tt - t0;
             }
         }
         const bool acc = act && x < wlen;
@@ -601,35 +746,12 @@ __device__ void link_window(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32
             last_x = __shfl_sync(FULL, x, 31 - __clz(accm));
             n_acc += __popc(accm);
         }
-        if (accm != actm) saturated = true;
-        const u64 stamp = acc ? ((u64)((t0 + x + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT) : 0ull;
-        if (isnew) {
-            u32 ci = cb + tau; if (ci >= c.NC) ci -= c.NC;
-            u32 slot = 0, qq = q;
-            for (u32 w = 0; w < mw; w++) {
-                const u32 word = masks[ci * mw + w];
-                const u32 pc = __popc(word);
-                if (qq < pc) { slot = w * 32 + __fns(word, 0, qq + 1); break; }
-                qq -= pc;
-            }
-            const u64 payload = stage[(size_t)ci * cap + slot];
-            ring[(tl + (i - n_back)) & rmask] = payload | stamp;
-        } else if (acc) {
-            const u32 pos = (fh + i) & rmask;
-            ring[pos] = (ring[pos] & ASTRA_FLIT_PAYLOAD_MASK) | stamp;
-        }
-    }
-    __syncwarp();
-    // consume the cells
-    if (n_new) {
-        for (u32 tau = lane; tau < wlen; tau += 32) {
-            u32 ci = cb + tau; if (ci >= c.NC) ci -= c.NC;
-            for (u32 w = 0; w < mw; w++) masks[ci * mw + w] = 0;
-        }
+        if (acc) ring[pos] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + x + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
+        if (accm != actm) break;                             // FIFO: nothing behind a waiting line is accepted
     }
     if (lane == 0) {
         c.fifo_head[e] = fh + n_acc;
-        c.ltail[e] = tl + n_new;
+        c.ltail[e] = tn;
         if (n_acc) {
             c.link_lines[e] += n_acc;
             atomicMin(&ctl.next_hint, t0 + first_x + leff);
@@ -640,89 +762,125 @@ __device__ void link_window(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32
     }
 }
 
-__device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8_t* ws, uint8_t* rs) {
+__device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8_t* ws, uint8_t* hot, uint8_t* rs, u32 rank) {
     c.G = P.G; c.V = P.V; c.E = P.E; c.S = P.S; c.C = P.C; c.Wv = P.Wv; c.K = P.K; c.H = P.H;
     c.CW = P.CW; c.nwords = P.nwords; c.slots = P.slots; c.bmwords = P.bmwords;
     c.logW = P.logW; c.W = 1u << P.logW; c.NC = P.NC; c.NW = P.NW; c.NWmask = P.NW - 1; c.kmagic = P.kdiv_magic;
     c.tmax = (u32)P.max_cycles; c.flags = P.flags;
     c.fullmask = P.K >= 64 ? ~0ull : ((1ull << P.K) - 1);
-#define CP(name) c.name = (const u32*)(cb + P.c_##name)
-    CP(in_ptr); CP(in_link); CP(head); CP(tail); CP(leff); CP(bw); CP(next_link);
-    CP(step_od); CP(lines); CP(cu_lo); CP(cu_n); CP(succ_ptr); CP(succ); CP(ndeps);
-    CP(step_q); CP(step_r); CP(first_link); CP(step_alpha); CP(cul_ptr); CP(cul); CP(rel_off); CP(init_rel); CP(init_rel_cnt); CP(ev_off);
-    CP(ring_off); CP(ring_mask); CP(lkind); CP(ceilb); CP(lstate0_init); CP(stage_off); CP(mask_off); CP(classoff);
-    CP(nd_cellcap); CP(nd_mw); CP(nd_injoff);
-#undef CP
-#define WP(name, type) c.name = (type*)(ws + P.w_##name)
-    WP(pipe_head, u32); WP(fifo_head, u32); c.ltail = (u32*)(ws + P.w_tail); WP(lstate0, u32); WP(lstate1, u32);
-    WP(link_lines, u32); WP(masks, u32); WP(ring, u64); WP(stage, u64);
-    WP(t_release, u32); WP(issued_cnt, u32); WP(t_issued, u32); WP(deliv_cnt, u32); WP(t_deliv, u32);
-    WP(ack_cnt, u32); WP(t_ack, u32); WP(ndep_left, u32); WP(rel_time, u32);
-    WP(wf_rem, u32); WP(wf_cur, u32); WP(wf_busy, u64);
-    WP(want, u32); WP(freeb, u32); WP(sel, u32); WP(plist, u32); WP(pcnt, u32); WP(ev_list, u32); WP(ev_cnt, u32); WP(ack_n, u32);
-    WP(ack_rec, u64); WP(bitmap, u32); WP(bin_cnt, u32); WP(ack_tmp, u64); WP(ack_sorted, u64);
-#undef WP
+    c.group = P.group; c.rank = rank;
+#define X(n) c.n = (const u32*)(cb + P.c_off[ASTRA_C_##n]);
+    ASTRA_CONST_TABLES(X)
+#undef X
+#define X(n, t, i) c.n = (t*)(((P.a_off[ASTRA_A_##n] & ASTRA_PLACE_SMEM) ? hot : ws) + (P.a_off[ASTRA_A_##n] & ~ASTRA_PLACE_SMEM));
+    ASTRA_WS_ARRAYS(X)
+#undef X
+    // node range of this CTA (the whole graph when the point runs on one CTA)
+    c.v_lo = c.part[rank]; c.v_hi = c.part[rank + 1];
+    c.g_lo = min(c.v_lo, c.G); c.g_hi = min(c.v_hi, c.G);
+    c.e_lo = c.row_ptr[c.v_lo]; c.e_hi = c.row_ptr[c.v_hi];
+    c.i_lo = c.in_ptr[c.v_lo]; c.i_hi = c.in_ptr[c.v_hi];
     c.r_step_ts = (u64*)(rs + P.r_step_ts);
     c.r_link_lines = (u64*)(rs + P.r_link_lines);
     c.r_summary = (DeviceSummary*)(rs + P.r_summary);
+    c.r_diag = (u64*)(rs + P.r_diag);
+}
+
+// Barrier over the CTAs of a group (all co-resident: the grid never exceeds what fits on the
+// device).  `target` = number of arrivals that completes this barrier.
+__device__ __forceinline__ void group_barrier(GroupCtl* gc, u32 target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(&gc->bar, 1u);
+        while ((int32_t)(*(volatile u32*)&gc->bar - target) < 0) { }
+        __threadfence();
+    }
+    __syncthreads();
 }
 
 extern "C" __global__ void __launch_bounds__(512, 1)
 astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
-                  u32 n_points, u64 ws_stride) {
+                  GroupCtl* groups, u32 n_points, u64 ws_stride, u32 group, u32 hot_off) {
     extern __shared__ __align__(16) uint8_t smem[];
     Ctx& c = *reinterpret_cast<Ctx*>(smem);
     Ctl& ctl = *reinterpret_cast<Ctl*>(smem + ((sizeof(Ctx) + 15) & ~size_t(15)));
     u32* scr_all = reinterpret_cast<u32*>(smem + ((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)));
+    uint8_t* hot = smem + hot_off;
     const u32 tid = threadIdx.x, nthr = blockDim.x;
     const u32 lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
     u32* scr = scr_all + warp * SCR_WORDS;
-    uint8_t* ws = ws_base + (size_t)blockIdx.x * ws_stride;
+    const u32 gid = blockIdx.x / group, rank = blockIdx.x % group;
+    uint8_t* ws = ws_base + (size_t)gid * ws_stride;
+    GroupCtl* gc = groups + gid;
+    u32 bar_target = 0;                 // arrivals that complete the next group barrier
 
     for (;;) {
         __syncthreads();
-        if (tid == 0) ctl.point = atomicAdd(queue, 1u);
-        __syncthreads();
+        if (group == 1) {
+            if (tid == 0) ctl.point = atomicAdd(queue, 1u);
+            __syncthreads();
+        } else {
+            bar_target += group; group_barrier(gc, bar_target);     // everyone is done with the previous point's control block
+            if (rank == 0 && tid == 0) {
+                gc->point = atomicAdd(queue, 1u);
+                gc->acked = 0; gc->err = 0; gc->completion = 0;
+                gc->hint[0] = gc->hint[1] = gc->hint[2] = ASTRA_T_INF;
+            }
+            bar_target += group; group_barrier(gc, bar_target);
+            if (tid == 0) ctl.point = *(volatile u32*)&gc->point;
+            __syncthreads();
+        }
         const u32 qi = ctl.point;
         if (qi >= n_points) break;
         const u32 pi = order[qi];
         const PointDesc& P = points[pi];
         if (tid == 0) {
-            resolve_ctx(c, P, cblob, ws, results);
-            ctl.acked = 0; ctl.completion = 0; ctl.err = 0; ctl.next_hint = ASTRA_T_INF;
+            resolve_ctx(c, P, cblob, ws, hot, results, rank);
+            ctl.acked = 0; ctl.completion = 0; ctl.err = 0; ctl.next_hint = ASTRA_T_INF; ctl.any_merged = 0;
+            ctl.acked_total = 0;
             ctl.busy = 0; ctl.skipped = 0;
+            for (int i = 0; i < 8; i++) ctl.clk[i] = 0;
         }
-        for (u32 i = tid; i < ASTRA_NW_MAX; i += nthr) ctl.ackwin[i] = 0;
-        // ---- workspace init ----
-        {
-            uint4 z = make_uint4(0, 0, 0, 0), f = make_uint4(~0u, ~0u, ~0u, ~0u);
-            uint4* pz = reinterpret_cast<uint4*>(ws);
-            for (u64 i = tid; i < P.ws_zero_bytes / 16; i += nthr) pz[i] = z;
-            uint4* pf = reinterpret_cast<uint4*>(ws + P.ws_ff_off);
-            for (u64 i = tid; i < P.ws_ff_bytes / 16; i += nthr) pf[i] = f;
-        }
+        long long ck0 = clock64();
         __syncthreads();
-        for (u32 e = tid; e < c.E; e += nthr) c.lstate0[e] = c.lstate0_init[e];
+        // ---- state init: shared-memory arrays by their CTA, global arrays split over the group ----
+        for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
+            const u32 kind = k_arr_init[a];
+            if (kind > 1) continue;
+            const u64 off = P.a_off[a];
+            const bool in_smem = (off & ASTRA_PLACE_SMEM) != 0;
+            uint8_t* base = (in_smem ? hot : ws) + (off & ~ASTRA_PLACE_SMEM);
+            const u32 pat = kind ? ~0u : 0u;
+            const u64 n16 = P.a_bytes[a] / 16;              // arrays are padded to 16 bytes
+            uint4* p = reinterpret_cast<uint4*>(base);
+            const uint4 v4 = make_uint4(pat, pat, pat, pat);
+            if (in_smem || group == 1) { for (u64 i = tid; i < n16; i += nthr) p[i] = v4; }
+            else { for (u64 i = (u64)rank * nthr + tid; i < n16; i += (u64)group * nthr) p[i] = v4; }
+        }
+        if (group > 1) { bar_target += group; group_barrier(gc, bar_target); } else __syncthreads();
+        for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.lstate0[e] = c.lstate0_init[e];
         for (u32 s = tid; s < c.S; s += nthr) {
+            const u32 ow = c.step_od[s] >> 16;
+            if (ow < c.g_lo || ow >= c.g_hi) continue;
             c.ndep_left[s] = c.ndeps[s];
             c.t_release[s] = c.ndeps[s] ? ASTRA_TS_NONE32 : 0u;      // steps without deps are released at t = 0 (R10)
-            c.plist[s] = c.init_rel[s];
         }
-        for (u32 i = tid; i < c.G * c.CW; i += nthr) {
-            u32 gq = i / c.CW, wf = i - gq * c.CW;
-            c.wf_cur[i] = c.cul_ptr[gq * c.C + wf / c.Wv];
+        for (u32 gq = c.g_lo; gq < c.g_hi; gq++) {
+            for (u32 j = c.rel_off[gq] + tid; j < c.rel_off[gq + 1]; j += nthr) c.plist[j] = c.init_rel[j];
+            for (u32 wf = tid; wf < c.CW; wf += nthr) c.wf_cur[(size_t)gq * c.CW + wf] = c.cul_ptr[gq * c.C + wf / c.Wv];
+            for (u32 wi = tid; wi < c.nwords; wi += nthr) {
+                const u32 nb = c.CW - wi * 32;
+                c.freeb[(size_t)gq * c.nwords + wi] = nb >= 32 ? ~0u : ((1u << nb) - 1u);
+            }
+            if (tid == 0) c.pcnt[gq] = c.init_rel_cnt[gq];
         }
-        for (u32 gq = tid; gq < c.G; gq += nthr) c.pcnt[gq] = c.init_rel_cnt[gq];
-        for (u32 i = tid; i < c.G * c.nwords; i += nthr) {
-            u32 wi = i % c.nwords;
-            u32 nb = c.CW - wi * 32;
-            c.freeb[i] = nb >= 32 ? ~0u : ((1u << nb) - 1u);
-        }
-        __syncthreads();
+        if (group > 1) { bar_target += group; group_barrier(gc, bar_target); } else __syncthreads();
+        if (tid == 0) { const long long ck = clock64(); ctl.clk[5] += (u64)(ck - ck0); ck0 = ck; }
 
         // ---- window loop ----
-        u32 k = 0;
+        u32 k = 0, seq = 0;
         int32_t status = ASTRA_STATUS_DONE;
         const u32 W = c.W;
         u64 busy = 0, skipped = 0;
@@ -734,59 +892,97 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             const u32 wlen = t1 - t0;
             const u32 cb = t0 % c.NC;
             busy += wlen;
-            // stage 1: arrivals per link, ack gather per GPU
-            for (u32 task = warp; task < c.E + c.G; task += nwarps) {
-                if (task < c.G) ack_gather(c, ctl, task, k, t0, wlen, scr, lane);
-                else arrivals_link(c, ctl, task - c.G, t0, wlen, cb, lane);
+            // stage 1: arrivals per in-link, ack gather per GPU
+            {
+                const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
+                for (u32 task = warp; task < ng + ns; task += nwarps) {
+                    if (task < ng) ack_gather(c, ctl, c.g_lo + task, k, t0, wlen, scr, lane);
+                    else arrivals_link<1>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
+                }
             }
             __syncthreads();
+            if (tid == 0) { const long long ck = clock64(); ctl.clk[1] += (u64)(ck - ck0); ck0 = ck; ctl.clk[0]++; }
             // stage 2: release + issue per GPU
-            for (u32 g = warp; g < c.G; g += nwarps) issue_window(c, ctl, g, t0, t1, cb, lane);
+            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) issue_window(c, ctl, g, t0, t1, cb, lane);
             __syncthreads();
-            // stage 3: link service per link
-            for (u32 e = warp; e < c.E; e += nwarps) link_window(c, ctl, e, t0, t1, cb, scr, lane);
-            __syncthreads();
-            // stage 4: next non-idle window
-            if (tid == 0) {
-                u32 hint = ctl.next_hint;
-                ctl.next_hint = ASTRA_T_INF;
-                for (u32 j = 1; j < c.NW; j++) {
-                    if (ctl.ackwin[(k + j) & c.NWmask]) {
-                        u64 tw = (u64)(k + j) << c.logW;
-                        hint = min(hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
-                        break;
+            if (tid == 0) { const long long ck = clock64(); ctl.clk[2] += (u64)(ck - ck0); ck0 = ck; }
+            // stage 3: merge into multi-feeder out-links (skipped when none received a line)
+            if (ctl.any_merged) {
+                for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps)
+                    if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
+                __syncthreads();
+                if (tid == 0) ctl.any_merged = 0;
+                {
+                    const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
+                    for (u32 task = warp; task < ng + ns; task += nwarps) {
+                        if (task < ng) inject_place(c, c.g_lo + task, wlen, cb, lane);
+                        else arrivals_link<3>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
                     }
                 }
+                __syncthreads();
+            }
+            if (tid == 0) { const long long ck = clock64(); ctl.clk[3] += (u64)(ck - ck0); ck0 = ck; }
+            // stage 4: link service per out-link
+            for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps) link_service(c, ctl, e, t0, t1, cb, lane);
+            __syncthreads();
+            if (tid == 0) { const long long ck = clock64(); ctl.clk[4] += (u64)(ck - ck0); ck0 = ck; }
+            // stage 5: next non-idle window
+            if (group > 1) {
+                if (tid == 0) {
+                    atomicMin(&gc->hint[seq % 3], ctl.next_hint);
+                    if (ctl.acked) { atomicAdd(&gc->acked, ctl.acked); atomicMax(&gc->completion, ctl.completion); }
+                    if (ctl.err) atomicOr(&gc->err, ctl.err);
+                    if (rank == 0) gc->hint[(seq + 1) % 3] = ASTRA_T_INF;
+                    ctl.acked = 0;
+                }
+                bar_target += group; group_barrier(gc, bar_target);
+                if (tid == 0) {
+                    ctl.next_hint = *(volatile u32*)&gc->hint[seq % 3];
+                    ctl.acked_total = *(volatile u32*)&gc->acked;
+                    ctl.err |= *(volatile u32*)&gc->err;
+                    ctl.completion = *(volatile u32*)&gc->completion;
+                }
+            } else if (tid == 0) { ctl.acked_total += ctl.acked; ctl.acked = 0; }
+            if (tid == 0) {
+                const u32 hint = ctl.next_hint;
+                ctl.next_hint = ASTRA_T_INF;
                 u32 dec = 0, nk = k + 1;
-                if (ctl.acked == c.S) dec = 1 + ASTRA_STATUS_DONE;
+                if (ctl.acked_total == c.S) dec = 1 + ASTRA_STATUS_DONE;
                 else if (ctl.err) dec = 1 + ASTRA_STATUS_INTERNAL;
                 else if (hint == ASTRA_T_INF) dec = 1 + ASTRA_STATUS_DEADLOCK;
                 else if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint >> c.logW);
                 ctl.decision = dec; ctl.next_k = nk;
             }
             __syncthreads();
+            seq++;
             const u32 dec = ctl.decision;
             if (dec) { status = (int32_t)dec - 1; break; }
             skipped += (u64)(ctl.next_k - k - 1) << c.logW;
             k = ctl.next_k;
         }
         __syncthreads();
-        // ---- A8: write-out ----
+        // ---- A8: write-out (each CTA the steps / links of its own nodes) ----
         for (u32 s = tid; s < c.S; s += nthr) {
             const u32 n = c.lines[s];
-            const u32 a = c.t_release[s];
-            c.r_step_ts[4 * (size_t)s + 0] = a == ASTRA_TS_NONE32 ? ~0ull : a;
-            c.r_step_ts[4 * (size_t)s + 1] = c.issued_cnt[s] == n ? (u64)c.t_issued[s] : ~0ull;
-            c.r_step_ts[4 * (size_t)s + 2] = c.deliv_cnt[s] == n ? (u64)c.t_deliv[s] : ~0ull;
-            c.r_step_ts[4 * (size_t)s + 3] = c.ack_cnt[s] == n ? (u64)c.t_ack[s] : ~0ull;
+            const u32 od = c.step_od[s];
+            const u32 ow = od >> 16, ds = od & 0xffffu;
+            if (ow >= c.g_lo && ow < c.g_hi) {
+                const u32 a = c.t_release[s];
+                c.r_step_ts[4 * (size_t)s + 0] = a == ASTRA_TS_NONE32 ? ~0ull : a;
+                c.r_step_ts[4 * (size_t)s + 1] = c.issued_cnt[s] == n ? (u64)c.t_issued[s] : ~0ull;
+                c.r_step_ts[4 * (size_t)s + 3] = c.ack_cnt[s] == n ? (u64)c.t_ack[s] : ~0ull;
+            }
+            if (ds >= c.g_lo && ds < c.g_hi)
+                c.r_step_ts[4 * (size_t)s + 2] = c.deliv_cnt[s] == n ? (u64)c.t_deliv[s] : ~0ull;
         }
-        for (u32 e = tid; e < c.E; e += nthr) c.r_link_lines[e] = c.link_lines[e];
-        if (tid == 0) {
+        for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.r_link_lines[e] = c.link_lines[e];
+        if (tid == 0 && rank == 0) {
             DeviceSummary sm;
             sm.status = status; sm.n_steps = c.S; sm.n_links = c.E; sm.window = W;
             sm.completion_cycle = ctl.completion; sm.total_lines = P.total_lines;
             sm.busy_cycles = busy; sm.skipped_cycles = skipped;
             *c.r_summary = sm;
+            for (int i = 0; i < 8; i++) c.r_diag[i] = ctl.clk[i];
         }
     }
 }
@@ -794,16 +990,16 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-static size_t smem_bytes(u32 warps) {
-    return ((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)) +
-           (size_t)warps * SCR_WORDS * sizeof(u32);
+u32 astra_engine_fixed_smem(u32 warps) {
+    size_t s = ((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)) + (size_t)warps * SCR_WORDS * sizeof(u32);
+    return (u32)((s + 127) & ~size_t(127));
 }
 
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32* ctas_per_sm, u32* n_sms, std::string& err) {
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err) {
     int dev = 0, sms = 0, occ = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    size_t sm = smem_bytes(warps_per_cta);
+    size_t sm = (size_t)astra_engine_fixed_smem(warps_per_cta) + hot_bytes;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, astra_step_kernel, (int)warps_per_cta * 32, sm);
     if (e != cudaSuccess) { err = std::string("occupancy query: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
@@ -812,13 +1008,16 @@ int32_t astra_engine_occupancy(u32 warps_per_cta, u32* ctas_per_sm, u32* n_sms, 
 }
 
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err) {
-    size_t sm = smem_bytes(L.warps_per_cta);
+    const u32 fixed = astra_engine_fixed_smem(L.warps_per_cta);
+    size_t sm = (size_t)fixed + L.hot_bytes;
     cudaError_t e = cudaFuncSetAttribute(astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) { err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
     e = cudaMemsetAsync(L.d_queue, 0, sizeof(u32), (cudaStream_t)stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(L.d_groups, 0, sizeof(GroupCtl) * L.n_groups, (cudaStream_t)stream);
     if (e != cudaSuccess) { err = std::string("queue reset: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
-    astra_step_kernel<<<L.grid, L.warps_per_cta * 32, sm, (cudaStream_t)stream>>>(
-        L.d_const, L.d_ws, L.d_results, L.d_points, L.d_order, L.d_queue, L.n_points, L.ws_stride);
+    astra_step_kernel<<<L.n_groups * L.group, L.warps_per_cta * 32, sm, (cudaStream_t)stream>>>(
+        L.d_const, L.d_ws, L.d_results, L.d_points, L.d_order, L.d_queue, L.d_groups, L.n_points, L.ws_stride,
+        L.group, fixed);
     e = cudaGetLastError();
     if (e != cudaSuccess) { err = std::string("kernel launch: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
     return ASTRA_OK;

@@ -12,7 +12,10 @@ typedef uint64_t u64;
 // Flit: one 128 B line in flight, 64 bits.
 //   [0,20)  step id      [20,32) wavefront id within the owner GPU (cu*W + w)
 //   [32,38) outstanding-slot index inside the wavefront (ack addressing)
-//   [38,64) arrival cycle mod 2^26 (meaningful once the link has accepted the line)
+//   [38,64) time field, 26 bits:
+//             queued in a link FIFO : cycle of the FIFO append relative to the window start
+//             accepted by the link  : arrival cycle at the link's head, mod 2^26
+//             inject record         : append cycle (10 bits) | slot index in the cell << 10
 // ---------------------------------------------------------------------------------------------
 #define ASTRA_FLIT_TIME_SHIFT 38
 #define ASTRA_FLIT_PAYLOAD_MASK ((1ull << ASTRA_FLIT_TIME_SHIFT) - 1)
@@ -20,52 +23,84 @@ typedef uint64_t u64;
 #define ASTRA_T_INF 0xffffffffu
 #define ASTRA_NOTLOADED 0xffffffffu
 #define ASTRA_TS_NONE32 0xffffffffu
-#define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles (per-warp smem scratch)
-#define ASTRA_NW_MAX 256                  // ack window bins per point (smem counters)
+#define ASTRA_NONE32 0xffffffffu
+#define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles
+#define ASTRA_NW_MAX 256                  // ack window bins per GPU
 
 // Link service kinds (R9): how the acceptance times of a FIFO are computed for a whole window.
 #define ASTRA_LK_INT     0u               // bw = B*256: B lines every cycle, no carried credit
 #define ASTRA_LK_PERIOD  1u               // 256 % bw == 0: one line every P = 256/bw cycles
 #define ASTRA_LK_GENERAL 2u               // any other bw: saturating credit walked entry by entry
 
-// Per design point descriptor.  c_* are byte offsets into the batch's constant blob, w_* byte
-// offsets into the workspace of the CTA slot running the point, r_* byte offsets into the results
-// blob.
+// Constant tables of a design point (u32 arrays in the batch's constant blob).
+#define ASTRA_CONST_TABLES(X) \
+    X(in_ptr) X(in_link) X(head) X(tail) X(leff) X(next_link) X(row_ptr) \
+    X(step_od) X(lines) X(cu_lo) X(cu_n) X(succ_ptr) X(succ) X(ndeps) \
+    X(step_q) X(step_r) X(first_link) X(step_alpha) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
+    X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(classoff) \
+    X(nd_mw) X(nd_injoff) X(inj_off) X(part)
+
+// Mutable arrays of a design point.  X(name, element type, init) with init: 0 zero, 1 0xff bytes,
+// 2 written by the kernel's own initialisation, 3 scratch (no initialisation).
+// Ordered by how often the per-window stages touch them: the loader places them in shared memory
+// in this order until the budget is spent, the rest in the CTA group's global workspace.
+#define ASTRA_WS_ARRAYS(X) \
+    X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
+    X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
+    X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
+    X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
+    X(bitmap, u32, 0) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(ring, u64, 3)
+
+enum AstraConstId {
+#define X(n) ASTRA_C_##n,
+    ASTRA_CONST_TABLES(X)
+#undef X
+    ASTRA_C_COUNT
+};
+enum AstraArrId {
+#define X(n, t, i) ASTRA_A_##n,
+    ASTRA_WS_ARRAYS(X)
+#undef X
+    ASTRA_A_COUNT
+};
+
+#define ASTRA_PLACE_SMEM (1ull << 63)     // a_off flag: offset is into the CTA's shared-memory hot region
+
+// Per design point descriptor.  c_off are byte offsets into the batch's constant blob, a_off byte
+// offsets into the hot region (flag set) or the workspace of the CTA group running the point,
+// r_* byte offsets into the results blob.
 struct PointDesc {
     u32 G, V, E, S;
     u32 C, Wv, K, H;
     u32 CW, nwords, slots, bmwords;
     u32 logW, NW, kdiv_magic, NC;              // NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
-    u32 flags, pad0;
+    u32 flags, group;                          // group: CTAs cooperating on this point
+    u32 hot_bytes, pad0;
     u64 max_cycles;
     u64 total_lines;
-    u64 ws_bytes, ws_zero_bytes, ws_ff_off, ws_ff_bytes;
-    // topology tables
-    u64 c_in_ptr, c_in_link, c_head, c_tail, c_leff, c_bw, c_next_link;
-    // collective tables
-    u64 c_step_od, c_lines, c_cu_lo, c_cu_n, c_succ_ptr, c_succ, c_ndeps;
-    // plan tables (topology x collective x gpu)
-    u64 c_step_q, c_step_r, c_first_link, c_step_alpha, c_cul_ptr, c_cul, c_rel_off, c_init_rel, c_init_rel_cnt;
-    u64 c_ev_off;
-    u64 c_ring_off, c_ring_mask, c_lkind, c_ceilb, c_lstate0_init, c_stage_off, c_mask_off, c_classoff;
-    u64 c_nd_cellcap, c_nd_mw, c_nd_injoff;
-    // workspace: zero-initialised region
-    u64 w_pipe_head, w_fifo_head, w_tail, w_lstate1, w_link_lines, w_masks;
-    u64 w_issued_cnt, w_t_issued, w_deliv_cnt, w_t_deliv, w_ack_cnt, w_t_ack, w_rel_time;
-    u64 w_wf_busy, w_want, w_bitmap, w_bin_cnt, w_ack_n, w_ev_cnt;
-    // workspace: 0xff-initialised region
-    u64 w_wf_rem;
-    // workspace: specially initialised
-    u64 w_lstate0, w_t_release, w_ndep_left, w_wf_cur, w_freeb, w_plist, w_pcnt;
-    // workspace: uninitialised
-    u64 w_ring, w_stage, w_sel, w_ack_rec, w_ack_tmp, w_ack_sorted, w_ev_list;
-    // results
-    u64 r_step_ts, r_link_lines, r_summary;
+    u64 ws_bytes;
+    u64 c_off[ASTRA_C_COUNT];
+    u64 a_off[ASTRA_A_COUNT];
+    u64 a_bytes[ASTRA_A_COUNT];
+    u64 r_step_ts, r_link_lines, r_summary, r_diag;
 };
 
 struct DeviceSummary {          // mirrors astra_summary, written by the kernel
     int32_t status; u32 n_steps, n_links, window;
     u64 completion_cycle, total_lines, busy_cycles, skipped_cycles;
+};
+
+// Control block of one CTA group in global memory (multi-CTA design points).
+struct GroupCtl {
+    u32 bar;            // monotone barrier counter
+    u32 point;          // queue index the group is running
+    u32 acked;          // steps fully acked, all CTAs
+    u32 err;
+    u32 completion;     // max t_ack
+    u32 hint[3];        // next-event time, rotated per window
+    u32 pad[8];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -97,21 +132,28 @@ struct Blob {                       // append-only byte buffer with 16-byte alig
     template <class T> u64 add(const std::vector<T>& v) { return add(v.data(), v.size() * sizeof(T)); }
 };
 
-#define ASTRA_N_TOPO_TABLES 7
-#define ASTRA_N_COLL_TABLES 7
+struct PlanOptions {
+    u64 flags = 0;
+    u64 max_cycles = 0;
+    u32 group = 1;                  // CTAs per design point
+    u32 hot_budget = 0;             // bytes of shared memory available for hot arrays
+};
 
 // loader entry points (astra_loader.cpp)
 int32_t astra_build_topo(HostTopo& t, std::string& err);
 int32_t astra_build_coll(HostColl& c, std::string& err);
-int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, u64 flags, u64 max_cycles,
+int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, const PlanOptions& opt,
                          const u64* topo_off, const u64* coll_off, Blob& blob, PointDesc& out, double& cost,
                          std::string& err);
+#define ASTRA_N_TOPO_TABLES 7
+#define ASTRA_N_COLL_TABLES 7
 
 // engine entry points (astra_engine.cu)
 struct EngineLaunch {
     const uint8_t* d_const; uint8_t* d_ws; uint8_t* d_results;
-    const PointDesc* d_points; const u32* d_order; u32* d_queue;
-    u32 n_points; u64 ws_stride; u32 grid, warps_per_cta;
+    const PointDesc* d_points; const u32* d_order; u32* d_queue; GroupCtl* d_groups;
+    u32 n_points; u64 ws_stride; u32 n_groups, group, warps_per_cta, hot_bytes;
 };
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err);
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32* ctas_per_sm, u32* n_sms, std::string& err);
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err);
+u32 astra_engine_fixed_smem(u32 warps_per_cta);

@@ -142,18 +142,20 @@ int32_t astra_build_coll(HostColl& c, std::string& err) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Plan one design point: plan tables into the blob, workspace layout into the descriptor.
+// Plan one design point: plan tables into the blob, array placement into the descriptor.
 // topo_off / coll_off are the blob offsets of the shared topology / collective tables.
 //
-// Staging cells (R7/R8).  The same-cycle append order into a link FIFO is fixed: transit lines
+// Append order (R7/R8).  The same-cycle append order into a link FIFO is fixed: transit lines
 // by ascending in-link id of the node, each in pipe order, then the node's own injections by
-// ascending wavefront id.  The engine gives every out-link of node v one cell per cycle of the
-// window with a FIXED slot layout: in-link i of v owns ceil(B_i) consecutive slots (a link
-// delivers at most ceil(B) lines per cycle), then H slots for injections (at most H issues per
-// GPU per cycle).  A line's slot is therefore known without any atomic allocation, and reading
-// a cell's occupied slots in slot order IS the FIFO order.
+// ascending wavefront id.  An out-link that only ever receives lines from ONE feeder (one in-link
+// or the node's own injections, decided here by walking every step's route) is appended to
+// directly by that feeder.  Every other out-link of node v gets one cell per cycle of the window
+// with a FIXED slot layout: in-link i of v owns ceil(B_i) consecutive slots (a link delivers at
+// most ceil(B) lines per cycle), then H slots for injections (at most H issues per GPU per
+// cycle).  A line's slot is known without any atomic allocation; one bit per slot is kept, and
+// the prefix sum of the popcounts in (cycle, slot) order IS the FIFO position.
 // ---------------------------------------------------------------------------------------------
-int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, u64 flags, u64 max_cycles,
+int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, const PlanOptions& opt,
                          const u64* topo_off, const u64* coll_off, Blob& blob, PointDesc& P, double& cost,
                          std::string& err) {
     std::memset(&P, 0, sizeof(P));
@@ -162,17 +164,19 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     if (c.max_cu_end > g.C) { err = "a step's CU range exceeds the GPU's CUs"; return ASTRA_EINVAL; }
     const u32 CW = g.C * g.Wv;
     const u32 slots = CW * g.K;
+    const u32 group = std::max<u32>(1, opt.group);
     P.G = G; P.V = V; P.E = E; P.S = S; P.C = g.C; P.Wv = g.Wv; P.K = g.K; P.H = g.H;
     P.CW = CW; P.nwords = (CW + 31) / 32; P.slots = slots; P.bmwords = (slots + 31) / 32;
     P.kdiv_magic = (u32)(((1ull << 32) + g.K - 1) / g.K);
     P.total_lines = c.total_lines;
-    P.flags = (u32)flags;
-    u64 tmax = std::min<u64>(max_cycles, 0xffffffffull - (1u << 25));
+    P.flags = (u32)opt.flags;
+    P.group = group;
+    u64 tmax = std::min<u64>(opt.max_cycles, 0xffffffffull - (1u << 25));
     P.max_cycles = tmax;
 
     // lookahead window: largest power of two <= min Leff, capped
     u32 logW = 0;
-    if (!(flags & ASTRA_FLAG_WINDOW_1)) {
+    if (!(opt.flags & ASTRA_FLAG_WINDOW_1)) {
         while ((2u << logW) <= t.min_leff && logW + 1 <= ASTRA_WMAX_LOG2) logW++;
     }
     P.logW = logW;
@@ -216,9 +220,12 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     for (u32 s = 0; s < S; s++)
         if (c.ndeps[s] == 0) { u32 o = c.owner[s]; init_rel[rel_off[o] + init_rel_cnt[o]++] = s; }
 
-    // ring capacities: lines that can sit in / fly over link e are bounded by the outstanding
-    // lines of the owners routed through it.
+    // Walk every step's route: ring capacities (lines that can sit in / fly over link e are bounded
+    // by the outstanding lines of the owners routed through it), feeders of every link, node loads.
     std::vector<u64> bound(E, 0);
+    std::vector<u32> feeder(E, ASTRA_NONE32);       // first feeder seen: in-link id, or E for injections
+    std::vector<uint8_t> multi(E, 0);
+    std::vector<double> load(V, 0.0);
     {
         std::vector<std::vector<u32>> by_owner(G);
         for (u32 s = 0; s < S; s++) by_owner[c.owner[s]].push_back(s);
@@ -226,20 +233,25 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         for (u32 o = 0; o < G; o++) {
             touched.clear();
             for (u32 s : by_owner[o]) {
-                u32 v = o, d = c.dst[s], hops = 0;
+                u32 v = o, d = c.dst[s], hops = 0, prev = E;
                 while (v != d) {
                     u32 e = t.next_link[(size_t)v * G + d];
                     if (via[e] == 0) touched.push_back(e);
                     via[e] += c.lines[s];
+                    if (feeder[e] == ASTRA_NONE32) feeder[e] = prev;
+                    else if (feeder[e] != prev) multi[e] = 1;
+                    load[v] += c.lines[s]; load[t.head[e]] += c.lines[s];
+                    prev = e;
                     v = t.head[e];
                     if (++hops > V) { err = "routing loop"; return ASTRA_EINVAL; }
                 }
+                load[o] += 2.0 * c.lines[s];
                 cost += (double)c.lines[s] * hops;
             }
             for (u32 e : touched) { bound[e] += std::min<u64>(slots, via[e]); via[e] = 0; }
         }
     }
-    // staging cells: slot layout per node, regions per link
+    // cells: slot layout per node, cell and prefix regions per multi-feeder link
     std::vector<u32> nd_cellcap(V), nd_mw(V), nd_injoff(V), classoff(E, 0);
     for (u32 v = 0; v < V; v++) {
         u32 off = 0;
@@ -253,66 +265,92 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         if (nd_cellcap[v] == 0) nd_cellcap[v] = 1;
         nd_mw[v] = (nd_cellcap[v] + 31) / 32;
     }
-    std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), credit_cap(E), lstate0(E), stage_off(E), mask_off(E);
-    u64 ring_total = 0, stage_total = 0, mask_total = 0;
+    if (g.H > 1023) { err = "hbm_lines_per_cycle above the engine limit"; return ASTRA_ELIMIT; }
+    std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), inj_off(G + 1, 0);
+    u64 ring_total = 0, mask_total = 0, pre_total = 0;
     for (u32 e = 0; e < E; e++) {
         u32 ceilb = (t.bw[e] + 255) / 256;
         ceilb_v[e] = ceilb;
-        credit_cap[e] = ceilb * 256;
         if (t.bw[e] % 256 == 0) { lkind[e] = ASTRA_LK_INT | ((t.bw[e] / 256) << 2); lstate0[e] = 0; }
         else if (256 % t.bw[e] == 0) { lkind[e] = ASTRA_LK_PERIOD | ((256 / t.bw[e]) << 2); lstate0[e] = 0; }   // next accept not before cycle 0
-        else { lkind[e] = ASTRA_LK_GENERAL | (t.bw[e] << 2); lstate0[e] = credit_cap[e]; }
-        u32 rc = std::max<u32>(32, pow2ceil(bound[e]));
+        else { lkind[e] = ASTRA_LK_GENERAL | (t.bw[e] << 2); lstate0[e] = ceilb * 256; }
+        // a group's writer checks the ring against a reader cursor that may lag one window: 2x
+        u32 rc = std::max<u32>(32, pow2ceil(bound[e] * (group > 1 ? 2 : 1)));
         if (ring_total + rc >= (1ull << 32)) { err = "ring space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
         ring_off[e] = (u32)ring_total; ring_mask[e] = rc - 1; ring_total += rc;
         u32 v = t.tail[e];
-        u64 st = (u64)NC * nd_cellcap[v], mk = (u64)NC * nd_mw[v];
-        if (stage_total + st >= (1ull << 32)) { err = "staging space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
-        stage_off[e] = (u32)stage_total; stage_total += st;
-        mask_off[e] = (u32)mask_total; mask_total += mk;
+        if (multi[e]) {
+            u64 mk = (u64)NC * nd_mw[v];
+            if (mask_total + mk >= (1ull << 31) || pre_total + NC >= (1ull << 31)) { err = "cell space exceeds 2^31 words"; return ASTRA_ELIMIT; }
+            mask_off[e] = (u32)mask_total; mask_total += mk;
+            pre_off[e] = (u32)pre_total; pre_total += NC;
+            if (v < G) inj_off[v + 1] = g.H * (W + 2);
+        } else { mask_off[e] = ASTRA_NONE32; pre_off[e] = ASTRA_NONE32; }
+    }
+    for (u32 i = 0; i < G; i++) inj_off[i + 1] += inj_off[i];
+
+    // node ranges of the CTAs of the group: contiguous, balanced by the lines each node handles
+    std::vector<u32> part(group + 1, V);
+    {
+        part[0] = 0;
+        double total = 0; for (u32 v = 0; v < V; v++) total += load[v] + 1.0;
+        double acc = 0; u32 j = 1;
+        for (u32 v = 0; v < V && j < group; v++) {
+            acc += load[v] + 1.0;
+            while (j < group && acc >= total * j / group) part[j++] = v + 1;
+        }
+        part[group] = V;
     }
 
     // constant tables
-    P.c_in_ptr = topo_off[0]; P.c_in_link = topo_off[1]; P.c_head = topo_off[2]; P.c_tail = topo_off[3];
-    P.c_leff = topo_off[4]; P.c_bw = topo_off[5]; P.c_next_link = topo_off[6];
-    P.c_step_od = coll_off[0]; P.c_lines = coll_off[1]; P.c_cu_lo = coll_off[2]; P.c_cu_n = coll_off[3];
-    P.c_succ_ptr = coll_off[4]; P.c_succ = coll_off[5]; P.c_ndeps = coll_off[6];
-    P.c_step_q = blob.add(step_q); P.c_step_r = blob.add(step_r); P.c_first_link = blob.add(first_link);
-    P.c_step_alpha = blob.add(step_alpha); P.c_cul_ptr = blob.add(cul_ptr); P.c_cul = blob.add(cul);
-    P.c_rel_off = blob.add(rel_off); P.c_init_rel = blob.add(init_rel); P.c_init_rel_cnt = blob.add(init_rel_cnt);
-    P.c_ev_off = blob.add(ev_off);
-    P.c_ring_off = blob.add(ring_off); P.c_ring_mask = blob.add(ring_mask); P.c_lkind = blob.add(lkind);
-    P.c_ceilb = blob.add(ceilb_v); P.c_lstate0_init = blob.add(lstate0);
-    P.c_stage_off = blob.add(stage_off); P.c_mask_off = blob.add(mask_off); P.c_classoff = blob.add(classoff);
-    P.c_nd_cellcap = blob.add(nd_cellcap); P.c_nd_mw = blob.add(nd_mw); P.c_nd_injoff = blob.add(nd_injoff);
+    u64* co = P.c_off;
+    co[ASTRA_C_in_ptr] = topo_off[0]; co[ASTRA_C_in_link] = topo_off[1]; co[ASTRA_C_head] = topo_off[2];
+    co[ASTRA_C_tail] = topo_off[3]; co[ASTRA_C_leff] = topo_off[4]; co[ASTRA_C_next_link] = topo_off[5];
+    co[ASTRA_C_row_ptr] = topo_off[6];
+    co[ASTRA_C_step_od] = coll_off[0]; co[ASTRA_C_lines] = coll_off[1]; co[ASTRA_C_cu_lo] = coll_off[2];
+    co[ASTRA_C_cu_n] = coll_off[3]; co[ASTRA_C_succ_ptr] = coll_off[4]; co[ASTRA_C_succ] = coll_off[5];
+    co[ASTRA_C_ndeps] = coll_off[6];
+    co[ASTRA_C_step_q] = blob.add(step_q); co[ASTRA_C_step_r] = blob.add(step_r);
+    co[ASTRA_C_first_link] = blob.add(first_link); co[ASTRA_C_step_alpha] = blob.add(step_alpha);
+    co[ASTRA_C_cul_ptr] = blob.add(cul_ptr); co[ASTRA_C_cul] = blob.add(cul);
+    co[ASTRA_C_rel_off] = blob.add(rel_off); co[ASTRA_C_init_rel] = blob.add(init_rel);
+    co[ASTRA_C_init_rel_cnt] = blob.add(init_rel_cnt); co[ASTRA_C_ev_off] = blob.add(ev_off);
+    co[ASTRA_C_ring_off] = blob.add(ring_off); co[ASTRA_C_ring_mask] = blob.add(ring_mask);
+    co[ASTRA_C_lkind] = blob.add(lkind); co[ASTRA_C_ceilb] = blob.add(ceilb_v);
+    co[ASTRA_C_lstate0_init] = blob.add(lstate0);
+    co[ASTRA_C_mask_off] = blob.add(mask_off); co[ASTRA_C_pre_off] = blob.add(pre_off);
+    co[ASTRA_C_classoff] = blob.add(classoff); co[ASTRA_C_nd_mw] = blob.add(nd_mw);
+    co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
+    co[ASTRA_C_part] = blob.add(part);
 
-    // workspace layout
-    u64 off = 0;
-    auto take = [&](u64 bytes) { u64 o = off; off = (off + bytes + 15) & ~15ull; return o; };
+    // mutable arrays: sizes, then placement (shared memory in declaration order while it fits)
     const u64 GW = (u64)G * CW;
-    const u32 nw = P.NW;
-    // zero region
-    P.w_pipe_head = take(4ull * E); P.w_fifo_head = take(4ull * E); P.w_tail = take(4ull * E);
-    P.w_lstate1 = take(4ull * E); P.w_link_lines = take(4ull * E); P.w_masks = take(4ull * mask_total);
-    P.w_issued_cnt = take(4ull * S); P.w_t_issued = take(4ull * S); P.w_deliv_cnt = take(4ull * S);
-    P.w_t_deliv = take(4ull * S); P.w_ack_cnt = take(4ull * S); P.w_t_ack = take(4ull * S); P.w_rel_time = take(4ull * S);
-    P.w_wf_busy = take(8ull * GW); P.w_want = take(4ull * G * P.nwords);
-    P.w_bitmap = take(4ull * G * nw * P.bmwords); P.w_bin_cnt = take(4ull * G * nw);
-    P.w_ack_n = take(4ull * G); P.w_ev_cnt = take(4ull * G);
-    P.ws_zero_bytes = off;
-    // 0xff region
-    P.ws_ff_off = off;
-    P.w_wf_rem = take(4ull * GW);
-    P.ws_ff_bytes = off - P.ws_ff_off;
-    // specially initialised
-    P.w_lstate0 = take(4ull * E); P.w_t_release = take(4ull * S); P.w_ndep_left = take(4ull * S);
-    P.w_wf_cur = take(4ull * GW); P.w_freeb = take(4ull * G * P.nwords);
-    P.w_plist = take(4ull * (S ? S : 1)); P.w_pcnt = take(4ull * G);
-    // uninitialised
-    P.w_ring = take(8ull * ring_total); P.w_stage = take(8ull * stage_total);
-    P.w_sel = take(4ull * G * g.H);
-    P.w_ack_rec = take(8ull * G * slots); P.w_ack_tmp = take(8ull * G * slots); P.w_ack_sorted = take(8ull * G * slots);
-    P.w_ev_list = take(4ull * (ev_off[G] ? ev_off[G] : 1));
-    P.ws_bytes = off;
+    u64* ab = P.a_bytes;
+    for (u32 a : {ASTRA_A_pipe_head, ASTRA_A_fifo_head, ASTRA_A_ltail, ASTRA_A_run, ASTRA_A_lstate0, ASTRA_A_lstate1,
+                  ASTRA_A_link_lines, ASTRA_A_dirty, ASTRA_A_ndue}) ab[a] = 4ull * E;
+    for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
+    ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = 4ull * G * P.nwords;
+    ab[ASTRA_A_sel] = 4ull * G * g.H;
+    ab[ASTRA_A_masks] = 4ull * mask_total; ab[ASTRA_A_pre] = 4ull * pre_total;
+    for (u32 a : {ASTRA_A_t_release, ASTRA_A_issued_cnt, ASTRA_A_t_issued, ASTRA_A_deliv_cnt, ASTRA_A_t_deliv,
+                  ASTRA_A_ack_cnt, ASTRA_A_t_ack, ASTRA_A_ndep_left, ASTRA_A_rel_time, ASTRA_A_plist}) ab[a] = 4ull * S;
+    ab[ASTRA_A_ev_list] = 4ull * ev_off[G];
+    ab[ASTRA_A_bin_cnt] = 4ull * G * P.NW;
+    ab[ASTRA_A_wf_busy] = 8ull * GW; ab[ASTRA_A_wf_rem] = 4ull * GW; ab[ASTRA_A_wf_cur] = 4ull * GW;
+    ab[ASTRA_A_bitmap] = 4ull * G * P.NW * P.bmwords;
+    ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
+    ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
+    ab[ASTRA_A_ring] = 8ull * ring_total;
+    u64 hot = 0, ws = 0;
+    for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
+        ab[a] = (std::max<u64>(ab[a], 16) + 15) & ~15ull;
+        // streamed arrays and, for a CTA group, everything another CTA may touch stay in global memory
+        bool global_only = a == ASTRA_A_bitmap || a == ASTRA_A_ack_rec || a == ASTRA_A_ack_tmp ||
+                           a == ASTRA_A_ack_sorted || a == ASTRA_A_ring || group > 1;
+        if (!global_only && hot + ab[a] <= opt.hot_budget) { P.a_off[a] = hot | ASTRA_PLACE_SMEM; hot += ab[a]; }
+        else { P.a_off[a] = ws; ws += ab[a]; }
+    }
+    P.hot_bytes = (u32)hot;
+    P.ws_bytes = ws;
     return ASTRA_OK;
 }

@@ -61,6 +61,17 @@ def test_i8_skip_equivalence(flags):
     check_workload(configs.config1(), flags=flags)
 
 
+@pytest.mark.parametrize("group", [2, 3, 8])
+def test_cta_groups(group):
+    """A design point spread over a group of CTAs (one node range each, one group barrier per
+    window) gives the same bits as on one CTA."""
+    from paper_2606_10440_b200.binding import FLAG_GROUP
+    check_workload(configs.config1(), flags=FLAG_GROUP(group))
+    check_workload(configs.random_workload(5, n_points=6, max_gpus=6, max_steps=24, max_lines=200), flags=FLAG_GROUP(group))
+    check_workload(configs.config2(range(6, 9)), flags=FLAG_GROUP(group), processes=6)
+    check_workload(configs.config5(n_nodes=4), flags=FLAG_GROUP(group), oracle_flags=oracle.FLAG_PRUNED_SCAN)
+
+
 def test_named_families_small():
     gpu = GpuCfg(8, 2, 4, 6)
     cases = [
