@@ -65,6 +65,7 @@ extern "C" {
 #define ASTRA_FLAG_NONE           0ull
 #define ASTRA_FLAG_NO_WINDOW_SKIP 1ull   /* step through every lookahead window (testing I8)   */
 #define ASTRA_FLAG_WINDOW_1       2ull   /* force a 1-cycle lookahead window (testing I8)      */
+#define ASTRA_FLAG_SERIAL_ISSUE   4ull   /* always take the cycle-serial issue path (testing)  */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g
                                             CTAs (1..16), one node range each; 0 = engine's choice */
 
@@ -154,11 +155,12 @@ int32_t astra_sync(astra_ctx* ctx);
 int32_t astra_read_results(astra_ctx* ctx, uint32_t point, astra_summary* out,
                            uint64_t* step_ts, uint64_t* link_lines);
 
-/* Diagnostics of design point `point` of the last batch, out8[8]: [0] lookahead windows stepped,
+/* Diagnostics of design point `point` of the last batch, out16[16]: [0] lookahead windows stepped,
  * [1..4] SM clocks the point's first CTA spent in the stages of a window (arrivals + ack gather,
  * release + issue, multi-feeder merge, link service + next-non-idle decision), [5] SM clocks of
- * state initialisation, [6..7] reserved.  Same errors as astra_read_results. */
-int32_t astra_read_diag(astra_ctx* ctx, uint32_t point, uint64_t* out8);
+ * state initialisation, [6] GPU-windows that took the cycle-serial issue path, [8..12] SM clocks of
+ * the parts of stage 2 (prepare, count, check, commit, place).  Same errors as astra_read_results. */
+int32_t astra_read_diag(astra_ctx* ctx, uint32_t point, uint64_t* out16);
 
 /* Diagnostics: device milliseconds (CUDA events on the ctx's stream) of the last batch and the
  * number of kernels it launched; bytes of device memory held by the prepared batch. */

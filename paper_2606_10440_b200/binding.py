@@ -194,7 +194,7 @@ class Engine:
                 link_lines[:s.n_links] if want_links else None)
 
     def read_diag(self, point: int) -> np.ndarray:
-        out = np.zeros(8, dtype=np.uint64)
+        out = np.zeros(16, dtype=np.uint64)
         self._check(self._lib.astra_read_diag(self._ctx, point, _ptr(out)))
         return out
 

@@ -158,11 +158,18 @@ extern "C" int32_t astra_set_gpu(astra_ctx* c, uint32_t cus, uint32_t wpc, uint3
 // CTAs per design point and warps per CTA for a batch of n points (A0 scheduling policy).
 // Few points: spread each over a group of CTAs (one node range each) so the device is used;
 // many points: one CTA per point, the queue balances.  ASTRA_FLAG_GROUP(g) overrides.
-static void choose_shape(const astra_ctx* c, u32 n, u32 max_nodes, u32 sms, u32* group, u32* warps) {
+static void choose_shape(const astra_ctx* c, u32 n, const astra_point* pts, u32 max_nodes, u32 sms, u32* group, u32* warps) {
     u32 g = (u32)((c->flags >> 8) & 0xff);
-    if (g == 0) g = 1;
-    (void)n; (void)sms;
-    *group = std::max<u32>(1, std::min<u32>(g, std::max<u32>(1, max_nodes)));
+    if (g == 0) {
+        // heavy points = those within 4x of the most expensive one (lines issued is the proxy);
+        // give each of them as many CTAs as there are nodes, as long as they all stay co-resident
+        u64 mx = 1;
+        for (u32 i = 0; i < n; i++) mx = std::max<u64>(mx, c->colls[pts[i].coll_id].total_lines);
+        u32 heavy = 0;
+        for (u32 i = 0; i < n; i++) if (c->colls[pts[i].coll_id].total_lines * 4 >= mx) heavy++;
+        g = std::max<u32>(1, std::min<u32>(16, sms / std::max<u32>(1, heavy)));
+    }
+    *group = std::max<u32>(1, std::min<u32>(std::min<u32>(g, 16), std::max<u32>(1, max_nodes)));
     *warps = 16;
 }
 
@@ -184,7 +191,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     CUDA_TRY(c, cudaGetDevice(&dev), "cudaGetDevice");
     CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "device attribute");
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "device attribute");
-    choose_shape(c, n, max_nodes, (u32)sms, &c->group, &c->warps);
+    choose_shape(c, n, pts, max_nodes, (u32)sms, &c->group, &c->warps);
     PlanOptions opt;
     opt.flags = c->flags & 0xff; opt.max_cycles = max_cycles; opt.group = c->group;
     const u32 fixed = astra_engine_fixed_smem(c->warps);
@@ -216,7 +223,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         P.r_step_ts = roff; roff += 32ull * P.S;
         P.r_link_lines = roff; roff += 8ull * P.E;
         P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
-        P.r_diag = roff; roff += 64;
+        P.r_diag = roff; roff += 128;
         ws_max = std::max(ws_max, P.ws_bytes);
         hot_max = std::max(hot_max, P.hot_bytes);
     }
@@ -332,12 +339,12 @@ extern "C" int32_t astra_read_results(astra_ctx* c, uint32_t point, astra_summar
     return ASTRA_OK;
 }
 
-extern "C" int32_t astra_read_diag(astra_ctx* c, uint32_t point, uint64_t* out8) {
+extern "C" int32_t astra_read_diag(astra_ctx* c, uint32_t point, uint64_t* out16) {
     if (!c) return ASTRA_EINVAL;
-    if (!out8) return fail(c, ASTRA_EINVAL, "null argument");
+    if (!out16) return fail(c, ASTRA_EINVAL, "null argument");
     int32_t rc = astra_read_results(c, point, nullptr, nullptr, nullptr);
     if (rc) return rc;
-    std::memcpy(out8, c->h_results.data() + c->descs[point].r_diag, 64);
+    std::memcpy(out16, c->h_results.data() + c->descs[point].r_diag, 128);
     return ASTRA_OK;
 }
 

@@ -61,7 +61,7 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 any_merged;     // some multi-feeder out-link received lines this window
     u32 acked_total, pad;
     u64 busy, skipped;
-    u64 clk[8];         // diagnostics: [0] windows, [1..4] SM clocks in stage groups, [5] init
+    u64 clk[16];        // diagnostics: [0] windows, [1..4] SM clocks in stage groups, [5] init, [6] serial GPU-windows, [8..15] stage-2 parts
 };
 
 __device__ const unsigned char k_arr_init[ASTRA_A_COUNT] = {
@@ -73,6 +73,15 @@ __device__ const unsigned char k_arr_init[ASTRA_A_COUNT] = {
 // Arrays that the loader may place in shared OR global memory and that another CTA of a group may
 // have written: a volatile generic load (never served from a stale L1 line, legal on both spaces).
 __device__ __forceinline__ u32 ld_vol(const u32* p) { return *(const volatile u32*)p; }
+
+// SM clock read that cannot issue before the preceding __syncthreads() has completed (the barrier is
+// non-blocking at issue; a shared-memory load after it is not).
+__device__ __forceinline__ long long clock_after_barrier(const volatile u32* smem_word) {
+    const u32 dep = *smem_word;
+    long long ck;
+    asm volatile("mov.u64 %0, %%clock64;\n\t// %1" : "=l"(ck) : "r"(dep) : "memory");
+    return ck;
+}
 
 __device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
@@ -221,9 +230,12 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 t0, u32 wlen, u32 cb,
 }
 
 // ---------------------------------------------------------------------------------------------
-// stage 1b: this window's acks of GPU g, counting-sorted by cycle; per-step ack counts (R6, A3)
+// stage 1b: this window's acks of GPU g (R6, A3): per-step ack counts, t_ack, ACKED events, and the
+// wavefronts that get a slot back this window (amask).  The bitmap of the window's bin holds one
+// bit per (wavefront, slot); ack_rec the (step, cycle) of each.  Nothing is consumed here: the
+// wavefront simulation (wf_sim) or, on the cycle-serial path, ack_sort reads the same bits again.
 // ---------------------------------------------------------------------------------------------
-__device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
+__device__ void ack_discover(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 lane) {
     const u32 bin = k & c.NWmask;
     // earliest later window with acks pending for this GPU (A7)
     {
@@ -239,13 +251,62 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
     const u32 n = ld_vol(&c.bin_cnt[g * c.NW + bin]);
     if (lane == 0) c.ack_n[g] = n;
     if (n == 0) return;
+    const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
+    const u64* rec = c.ack_rec + (size_t)g * c.slots;
+    u32* am = c.amask + (size_t)g * c.nwords;
+    u32 total = 0, acked_steps = 0, completion = 0;
+    for (u32 wb = 0; wb < c.bmwords; wb += 32) {
+        const u32 wi = wb + lane;
+        u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
+        while (__any_sync(FULL, w != 0)) {
+            const bool act = w != 0;
+            const u32 amk = __ballot_sync(FULL, act);
+            bool completed = false;
+            if (act) {
+                const u32 b = __ffs(w) - 1; w &= w - 1;
+                const u32 idx = wi * 32 + b;
+                const u64 rc = __ldcg(&rec[idx]);
+                const u32 step = (u32)(rc >> 32), ta = (u32)rc;
+                const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K
+                atomicOr(&am[wf >> 5], 1u << (wf & 31));
+                const u32 m = __match_any_sync(amk, step);
+                const u32 cmax = __reduce_max_sync(m, ta);
+                if ((m & lanemask_lt()) == 0) {
+                    const u32 ac = c.ack_cnt[step] + __popc(m);
+                    const u32 tm = max(c.t_ack[step], cmax);
+                    c.ack_cnt[step] = ac; c.t_ack[step] = tm;
+                    if (ac == c.lines[step]) {
+                        completed = true;
+                        const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
+                        c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
+                        completion = max(completion, tm);
+                    }
+                }
+            }
+            total += __popc(amk);
+            acked_steps += __popc(__ballot_sync(FULL, completed));
+        }
+    }
+    completion = __reduce_max_sync(FULL, completion);
+    if (lane == 0) {
+        if (total != n) atomicOr(&ctl.err, 2u);
+        if (acked_steps) { atomicAdd(&ctl.acked, acked_steps); atomicMax(&ctl.completion, completion); }
+    }
+    __syncwarp();
+}
+
+// Cycle-serial path only: consume the window's ack bits of GPU g into ack_sorted, counting-sorted
+// by cycle (low word: cycle << 18 | wavefront << 6 | slot).
+__device__ void ack_sort(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
+    const u32 bin = k & c.NWmask;
+    const u32 n = c.ack_n[g];
+    if (n == 0) return;
     for (u32 i = lane; i <= wlen; i += 32) scnt[i] = 0;
     __syncwarp();
     u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
     const u64* rec = c.ack_rec + (size_t)g * c.slots;
     u64* tmp = c.ack_tmp + (size_t)g * c.slots;
     u64* srt = c.ack_sorted + (size_t)g * c.slots;
-    // pass 1: discover, histogram by cycle, compact into tmp
     u32 total = 0;
     for (u32 wb = 0; wb < c.bmwords; wb += 32) {
         const u32 wi = wb + lane;
@@ -260,14 +321,13 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
             const u32 idx = wi * 32 + b;
             const u64 rc = __ldcg(&rec[idx]);
             const u32 cyc = (u32)rc - t0;
-            const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K (magic overflows for K == 1)
+            const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);
             const u32 slot = idx - wf * c.K;
             atomicAdd(&scnt[cyc], 1u);
             tmp[pos++] = (rc & 0xffffffff00000000ull) | (cyc << 18) | (wf << 6) | slot;
         }
     }
     __syncwarp();
-    // exclusive scan of the histogram
     u32 carry = 0;
     for (u32 b = 0; b < wlen; b += 32) {
         const u32 i = b + lane;
@@ -277,40 +337,17 @@ __device__ void ack_gather(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32
         carry += __shfl_sync(FULL, incl, 31);
     }
     __syncwarp();
-    // pass 2: scatter into cycle order; count acks per step, stamp t_ack (R3, R14)
-    u32 acked_steps = 0, completion = 0;
     for (u32 b = 0; b < total; b += 32) {
         const u32 i = b + lane;
-        const bool act = i < total;
-        const u64 ent = act ? tmp[i] : 0ull;
-        const u32 amask = __ballot_sync(FULL, act);
-        bool completed = false;
-        if (act) {
-            const u32 cyc = (u32)ent >> 18;
-            const u32 pos = atomicAdd(&scnt[cyc], 1u);
+        if (i < total) {
+            const u64 ent = tmp[i];
+            const u32 pos = atomicAdd(&scnt[(u32)ent >> 18], 1u);
             srt[pos] = ent;
-            const u32 step = (u32)(ent >> 32);
-            const u32 m = __match_any_sync(amask, step);
-            const u32 cmax = __reduce_max_sync(m, cyc);
-            if ((m & lanemask_lt()) == 0) {
-                const u32 ac = c.ack_cnt[step] + __popc(m);
-                const u32 tm = max(c.t_ack[step], t0 + cmax);
-                c.ack_cnt[step] = ac; c.t_ack[step] = tm;
-                if (ac == c.lines[step]) {
-                    completed = true;
-                    const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
-                    c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
-                    completion = max(completion, tm);
-                }
-            }
         }
-        acked_steps += __popc(__ballot_sync(FULL, completed));
     }
-    completion = __reduce_max_sync(FULL, completion);
     if (lane == 0) {
         c.bin_cnt[g * c.NW + bin] = 0;
         if (total != n) atomicOr(&ctl.err, 2u);
-        if (acked_steps) { atomicAdd(&ctl.acked, acked_steps); atomicMax(&ctl.completion, completion); }
     }
     __syncwarp();
 }
@@ -366,18 +403,6 @@ __device__ __forceinline__ bool wf_advance(Ctx& c, u32 g, u32 wf, u32& cur, u32&
 // stage 2: release + issue of GPU g over [t0, t1)   (R10 - R13, slot return of R7 A3)
 // ---------------------------------------------------------------------------------------------
 __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
-    // dependency events of this window (DELIVERED from stage 1a, ACKED from stage 1b)
-    {
-        const u32 nev = c.ev_cnt[g];
-        for (u32 j = 0; j < nev; j++) {
-            const u32 ek = c.ev_list[c.ev_off[g] + j];
-            const u32 p = ek & 0xfffffu, kind = ek >> 30;
-            const u32 time = kind == ASTRA_DEP_DELIVERED ? c.t_deliv[p] : c.t_ack[p];
-            on_event(c, g, p, kind, time, lane);
-        }
-        __syncwarp();
-        if (lane == 0 && nev) c.ev_cnt[g] = 0;
-    }
     const u32 ack_n = c.ack_n[g];
     const u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32* plist = c.plist + c.rel_off[g];
@@ -598,6 +623,271 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
     if (lane == 0) {
         c.inj_n[g] = n_inj;
         if (t != ASTRA_T_INF) atomicMin(&ctl.next_hint, t);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage 2, wavefront-parallel path.  Inside a window every input of a wavefront's issue decisions
+// is known up front -- its acks (stage 1b), the release times of its steps (events of stage 1) --
+// EXCEPT the HBM budget H shared by the GPU's wavefronts (R12).  So every wavefront that can change
+// state this window is simulated on its own thread as if the budget never bound, the issues are
+// counted per (first-hop link, cycle), and the GPU's warp checks that no cycle exceeded H.  If none
+// did, the unconstrained run IS the fixed-priority run (no wavefront was ever denied), and its
+// issues are ranked (cycle, wavefront id) by counting into per-cycle buckets: that rank is the
+// FIFO position (direct out-link) or the cell slot (multi-feeder out-link) R7 A2 prescribes.
+// A GPU-window where the budget binds, or whose steps have ISSUED-kind successors (their release
+// times depend on this window's issues), takes the cycle-serial path (issue_window) instead.
+// ---------------------------------------------------------------------------------------------
+
+// stage 2a: dependency events -> release times (R10); the set of wavefronts to look at; the mode.
+__device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
+    {
+        const u32 nev = c.ev_cnt[g];
+        for (u32 j = 0; j < nev; j++) {
+            const u32 ek = c.ev_list[c.ev_off[g] + j];
+            const u32 p = ek & 0xfffffu, kind = ek >> 30;
+            const u32 time = kind == ASTRA_DEP_DELIVERED ? c.t_deliv[p] : c.t_ack[p];
+            on_event(c, g, p, kind, time, lane);
+        }
+        __syncwarp();
+        if (lane == 0 && nev) c.ev_cnt[g] = 0;
+    }
+    u32* am = c.amask + (size_t)g * c.nwords;
+    const u32* want = c.want + (size_t)g * c.nwords;
+    const u32* freeb = c.freeb + (size_t)g * c.nwords;
+    // wavefronts of the CU range of every step released inside this window
+    const u32 np = c.pcnt[g];
+    const u32* plist = c.plist + c.rel_off[g];
+    for (u32 i = 0; i < np; i++) {
+        const u32 s = plist[i];
+        if (c.t_release[s] >= t1) continue;
+        const u32 lo = c.cu_lo[s] * c.Wv, hi = lo + c.cu_n[s] * c.Wv;
+        for (u32 wi = (lo >> 5) + lane; wi <= ((hi - 1) >> 5); wi += 32) {
+            const u32 b0 = wi * 32;
+            u32 m = ~0u;
+            if (lo > b0) m &= ~0u << (lo - b0);
+            if (hi < b0 + 32) m &= (1u << (hi - b0)) - 1u;
+            am[wi] |= m;
+        }
+        __syncwarp();
+    }
+    u32 any = 0;
+    for (u32 wi = lane; wi < c.nwords; wi += 32) {
+        const u32 a = am[wi] | (want[wi] & freeb[wi]);
+        am[wi] = a; any |= a;
+    }
+    const bool active = __ballot_sync(FULL, any != 0) != 0;
+    u32 mode = 0;
+    if (active) mode = ((c.gflag[g] & ASTRA_GF_ISSUED_DEPS) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE)) ? 2u : 1u;
+    if (mode == 1) {
+        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+        u32* h = c.hist + (size_t)e0 * c.W;
+        for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0;
+    }
+    if (lane == 0) c.gmode[g] = mode;
+}
+
+// stage 2b / 2d: the 32 wavefronts of word wi of GPU g.  PASS 0 counts the issues per (link, cycle);
+// PASS 1 (after the budget check) stores them in their buckets and commits the wavefront state.
+template <int PASS>
+__device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+    u32* amp = c.amask + (size_t)g * c.nwords + wi;
+    const u32 am = *amp;
+    if (am == 0) return;
+    const bool active = (am >> lane) & 1u;
+    const u32 wf = wi * 32 + lane;
+    const u32 e0 = c.row_ptr[g];
+    u32* h = c.hist + (size_t)e0 * c.W;
+    bool wantb = false, freebit = false, hint = false;
+    if (active) {
+        const size_t gw = (size_t)g * c.CW + wf;
+        u32 cur = c.wf_cur[gw], rem = c.wf_rem[gw];
+        u64 busy = c.wf_busy[gw];
+        // this wavefront's ack bits of the window's bin: bits [wf*K, wf*K + K) of the GPU's bitmap
+        u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
+        const u32 b0 = wf * c.K, w0 = b0 >> 5, sh = b0 & 31;
+        u64 rb = 0;
+        if (c.ack_n[g]) {
+            const u32 x0 = __ldcg(&bm[w0]);
+            const u32 x1 = (w0 + 1 < c.bmwords) ? __ldcg(&bm[w0 + 1]) : 0u;
+            const u32 x2 = (sh && w0 + 2 < c.bmwords) ? __ldcg(&bm[w0 + 2]) : 0u;
+            rb = ((((u64)x1 << 32) | x0) >> sh);
+            if (sh) rb |= (u64)x2 << (64 - sh);
+            rb &= c.fullmask;
+        }
+        const u64 rb_all = rb;
+        const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
+        // the wavefront's acks of the window, sorted by cycle: (cycle - t0) << 6 | slot
+        u32 aq[64];
+        u32 na = 0, ai = 0;
+        {
+            u64 x = rb;
+            while (x) {                                         // four loads in flight at a time
+                u32 b[4]; u32 v[4]; int m = 0;
+#pragma unroll
+                for (int q = 0; q < 4; q++) { b[q] = 0; if (x) { b[q] = __ffsll((long long)x) - 1; x &= x - 1; m = q + 1; } }
+#pragma unroll
+                for (int q = 0; q < 4; q++) v[q] = (q < m) ? (u32)__ldcg(&rec[b[q]]) : 0u;
+#pragma unroll
+                for (int q = 0; q < 4; q++) if (q < m) aq[na++] = ((v[q] - t0) << 6) | b[q];
+            }
+            for (u32 i = 1; i < na; i++) {
+                const u32 xv = aq[i]; u32 j = i;
+                while (j > 0 && aq[j - 1] > xv) { aq[j] = aq[j - 1]; j--; }
+                aq[j] = xv;
+            }
+        }
+        u32 na_t = na ? t0 + (aq[0] >> 6) : ASTRA_T_INF;        // earliest ack not applied yet
+        const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
+        u32 t = t0, s = 0, o = 0, scnt = 0, slast = 0, last_issue = ASTRA_T_INF;
+        bool have_s = false;
+        for (;;) {
+            if (rem == ASTRA_NOTLOADED) {
+                bool got = false;
+                while (cur < end) {
+                    const u32 s2 = c.cul[cur];
+                    const u32 tr = c.t_release[s2];
+                    if (tr >= t1) break;                        // not released by the end of the window
+                    if (tr > t) t = tr;
+                    const u32 q = c.step_q[s2] + (((wf - c.cu_lo[s2] * c.Wv) < c.step_r[s2]) ? 1u : 0u);   // R11
+                    if (q) { rem = q; got = true; break; }
+                    cur++;
+                }
+                if (!got) break;
+                have_s = false;
+            }
+            if (!have_s) { s = c.cul[cur]; o = c.first_link[s]; have_s = true; }
+            while (na_t <= t) {                                 // slots returned by cycle t (A3 before D)
+                busy &= ~(1ull << (aq[ai] & 63u)); ai++;
+                na_t = ai < na ? t0 + (aq[ai] >> 6) : ASTRA_T_INF;
+            }
+            if (t >= t1) break;
+            if (busy == c.fullmask) {                           // all K slots in flight: wait for the next ack
+                if (na_t >= t1) break;
+                t = na_t; continue;
+            }
+            const u32 slot = __ffsll((long long)~busy) - 1;
+            busy |= 1ull << slot;
+            const u32 key = (o - e0) * c.W + (t - t0);
+            if (PASS == 0) atomicAdd(&h[key], 1u);
+            else {
+                const u32 pos = atomicAdd(&h[key], 1u);
+                c.evb[(size_t)g * c.H * c.W + pos] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(t + 1 - t0) << ASTRA_FLIT_TIME_SHIFT);
+                scnt++; slast = t;
+            }
+            last_issue = t;
+            rem--; t++;
+            if (rem == 0) {
+                if (PASS == 1) { atomicAdd(&c.issued_cnt[s], scnt); atomicMax(&c.t_issued[s], slast); scnt = 0; }
+                cur++; rem = ASTRA_NOTLOADED;
+            }
+        }
+        if (PASS == 1) {
+            if (scnt) { atomicAdd(&c.issued_cnt[s], scnt); atomicMax(&c.t_issued[s], slast); }
+            for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));   // acks later in the window than the last look
+            c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
+            if (rb_all) {                                       // consume the ack bits
+                const u32 m0 = (u32)(rb_all << sh);
+                if (m0) atomicAnd(&bm[w0], ~m0);
+                const u32 m1 = (u32)((sh ? (rb_all >> (32 - sh)) : (rb_all >> 32)));
+                if (m1) atomicAnd(&bm[w0 + 1], ~m1);
+                const u32 m2 = sh ? (u32)(rb_all >> (64 - sh)) : 0u;
+                if (m2) atomicAnd(&bm[w0 + 2], ~m2);
+            }
+            wantb = rem != ASTRA_NOTLOADED;
+            freebit = busy != c.fullmask;
+            hint = (wantb && freebit) || last_issue == t1 - 1;
+        }
+    }
+    if (PASS == 1) {
+        const u32 wm = __ballot_sync(FULL, wantb), fm = __ballot_sync(FULL, freebit);
+        const bool anyh = __any_sync(FULL, hint);
+        if (lane == 0) {
+            u32* want = c.want + (size_t)g * c.nwords + wi;
+            u32* freeb = c.freeb + (size_t)g * c.nwords + wi;
+            *want = (*want & ~am) | wm;
+            *freeb = (*freeb & ~am) | fm;
+            *amp = 0;
+            if (anyh) atomicMin(&ctl.next_hint, t1);
+        }
+    }
+}
+
+// stage 2c: did the HBM budget bind in any cycle (R12)?  If not: exclusive prefix over the
+// (link, cycle) counts = bucket bases; direct out-links get their new tails.
+__device__ void gpu_check(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    u32* h = c.hist + (size_t)e0 * c.W;
+    bool bind = false;
+    if (c.H < c.CW) {
+        for (u32 tt = lane; tt < wlen; tt += 32) {
+            u32 tot = 0;
+            for (u32 x = 0; x < deg; x++) tot += h[x * c.W + tt];
+            if (tot > c.H) bind = true;
+        }
+    }
+    if (__any_sync(FULL, bind)) {
+        if (lane == 0) c.gmode[g] = 2u;
+        return;
+    }
+    const u32 nkeys = deg * c.W;
+    u32 carry = 0;
+    for (u32 b = 0; b < nkeys; b += 32) {
+        const u32 i = b + lane;
+        const u32 v = (i < nkeys) ? h[i] : 0;
+        const u32 incl = warp_incl_scan(v, lane);
+        if (i < nkeys) h[i] = carry + incl - v;
+        carry += __shfl_sync(FULL, incl, 31);
+    }
+    __syncwarp();
+    for (u32 x = lane; x < deg; x += 32) {                      // direct out-links: new FIFO tails
+        const u32 o = e0 + x;
+        if (c.mask_off[o] != ASTRA_NONE32) continue;
+        const u32 st = h[x * c.W], en = (x + 1 < deg) ? h[(x + 1) * c.W] : carry;
+        if (en != st) c.run[o] += en - st;
+    }
+    if (lane == 0) {
+        c.sel[(size_t)g * c.H] = carry;                         // events of the GPU this window (sel is free on this path)
+        c.pcnt[g] = 0;                                          // the released steps are consumed by the wavefronts
+        c.bin_cnt[g * c.NW + (k & c.NWmask)] = 0;
+    }
+    __syncwarp();
+}
+
+// stage 2e: rank the issues of GPU g inside their cycle (ascending wavefront id, R7 A2 / R12) and
+// put each line where that rank says: FIFO position on a direct out-link, cell slot + injection
+// record on a multi-feeder one.  After PASS 1, h[key] is the END of bucket key.
+__device__ void ev_place(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 cb, u32 lane) {
+    const u32 nev = c.sel[(size_t)g * c.H];
+    const u32 i = chunk * 32 + lane;
+    if (i >= nev) return;
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    const u32* h = c.hist + (size_t)e0 * c.W;
+    const u64* ev = c.evb + (size_t)g * c.H * c.W;
+    const u64 rec = ev[i];
+    const u32 s = (u32)rec & 0xfffffu, wf = ((u32)rec >> 20) & 0xfffu;
+    const u32 d = (u32)(rec >> ASTRA_FLIT_TIME_SHIFT);
+    const u32 o = c.first_link[s], ox = o - e0, tt = d - 1;
+    const u32 key = ox * c.W + tt;
+    const u32 st = key ? h[key - 1] : 0u, en = h[key];
+    u32 jo = 0;
+    for (u32 x = st; x < en; x++) jo += ((((u32)ev[x]) >> 20) & 0xfffu) < wf;
+    if (c.mask_off[o] == ASTRA_NONE32) {
+        const u32 en_o = h[ox * c.W + c.W - 1];
+        const u32 pos = c.run[o] - (en_o - (st + jo));
+        c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+    } else {
+        u32 j = jo;
+        for (u32 x2 = 0; x2 < deg; x2++) {
+            if (x2 == ox) continue;
+            const u32 k2 = x2 * c.W + tt;
+            const u32 st2 = k2 ? h[k2 - 1] : 0u, en2 = h[k2];
+            for (u32 x = st2; x < en2; x++) j += ((((u32)ev[x]) >> 20) & 0xfffu) < wf;
+        }
+        cell_set(c, ctl, o, g, cb, d, c.nd_injoff[g] + j);
+        const u32 p = atomicAdd(&c.inj_n[g], 1u);
+        if (p < c.inj_off[g + 1] - c.inj_off[g]) c.inj_list[c.inj_off[g] + p] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
+        else atomicOr(&ctl.err, 4u);
     }
 }
 
@@ -841,7 +1131,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0; ctl.next_hint = ASTRA_T_INF; ctl.any_merged = 0;
             ctl.acked_total = 0;
             ctl.busy = 0; ctl.skipped = 0;
-            for (int i = 0; i < 8; i++) ctl.clk[i] = 0;
+            for (int i = 0; i < 16; i++) ctl.clk[i] = 0;
         }
         long long ck0 = clock64();
         __syncthreads();
@@ -877,7 +1167,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             if (tid == 0) c.pcnt[gq] = c.init_rel_cnt[gq];
         }
         if (group > 1) { bar_target += group; group_barrier(gc, bar_target); } else __syncthreads();
-        if (tid == 0) { const long long ck = clock64(); ctl.clk[5] += (u64)(ck - ck0); ck0 = ck; }
+        if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[5] += (u64)(ck - ck0); ck0 = ck; }
 
         // ---- window loop ----
         u32 k = 0, seq = 0;
@@ -892,20 +1182,52 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             const u32 wlen = t1 - t0;
             const u32 cb = t0 % c.NC;
             busy += wlen;
-            // stage 1: arrivals per in-link, ack gather per GPU
+            // stage 1: arrivals per in-link, ack discovery per GPU
             {
                 const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
                 for (u32 task = warp; task < ng + ns; task += nwarps) {
-                    if (task < ng) ack_gather(c, ctl, c.g_lo + task, k, t0, wlen, scr, lane);
+                    if (task < ng) ack_discover(c, ctl, c.g_lo + task, k, t0, lane);
                     else arrivals_link<1>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
                 }
             }
             __syncthreads();
-            if (tid == 0) { const long long ck = clock64(); ctl.clk[1] += (u64)(ck - ck0); ck0 = ck; ctl.clk[0]++; }
-            // stage 2: release + issue per GPU
-            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) issue_window(c, ctl, g, t0, t1, cb, lane);
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[1] += (u64)(ck - ck0); ck0 = ck; ctl.clk[0]++; }
+            // stage 2: release + issue.  2a events/releases/mode per GPU; 2b unconstrained wavefront runs,
+            // counted; 2c budget check + bucket bases; 2d commit (or the cycle-serial path); 2e placement.
+            long long ck1 = ck0;
+            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) gpu_prepare(c, ctl, g, t0, t1, lane);
             __syncthreads();
-            if (tid == 0) { const long long ck = clock64(); ctl.clk[2] += (u64)(ck - ck0); ck0 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[8] += (u64)(ck - ck1); ck1 = ck; }
+            for (u32 g = c.g_lo; g < c.g_hi; g++) {
+                if (c.gmode[g] != 1u) continue;
+                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim<0>(c, ctl, g, wi, k, t0, t1, lane);
+            }
+            __syncthreads();
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[9] += (u64)(ck - ck1); ck1 = ck; }
+            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) if (c.gmode[g] == 1u) gpu_check(c, ctl, g, k, wlen, lane);
+            __syncthreads();
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[10] += (u64)(ck - ck1); ck1 = ck; }
+            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) {
+                if (c.gmode[g] != 2u) continue;
+                if (lane == 0) atomicAdd((unsigned long long*)&ctl.clk[6], 1ull);
+                ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
+                issue_window(c, ctl, g, t0, t1, cb, lane);
+                for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
+            }
+            for (u32 g = c.g_lo; g < c.g_hi; g++) {
+                if (c.gmode[g] != 1u) continue;
+                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim<1>(c, ctl, g, wi, k, t0, t1, lane);
+            }
+            __syncthreads();
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[11] += (u64)(ck - ck1); ck1 = ck; }
+            for (u32 g = c.g_lo; g < c.g_hi; g++) {
+                if (c.gmode[g] != 1u) continue;
+                const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
+                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ev_place(c, ctl, g, ch, cb, lane);
+            }
+            __syncthreads();
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[12] += (u64)(ck - ck1); ck1 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[2] += (u64)(ck - ck0); ck0 = ck; }
             // stage 3: merge into multi-feeder out-links (skipped when none received a line)
             if (ctl.any_merged) {
                 for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps)
@@ -921,11 +1243,11 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                 }
                 __syncthreads();
             }
-            if (tid == 0) { const long long ck = clock64(); ctl.clk[3] += (u64)(ck - ck0); ck0 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[3] += (u64)(ck - ck0); ck0 = ck; }
             // stage 4: link service per out-link
             for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps) link_service(c, ctl, e, t0, t1, cb, lane);
             __syncthreads();
-            if (tid == 0) { const long long ck = clock64(); ctl.clk[4] += (u64)(ck - ck0); ck0 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[4] += (u64)(ck - ck0); ck0 = ck; }
             // stage 5: next non-idle window
             if (group > 1) {
                 if (tid == 0) {
@@ -982,7 +1304,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             sm.completion_cycle = ctl.completion; sm.total_lines = P.total_lines;
             sm.busy_cycles = busy; sm.skipped_cycles = skipped;
             *c.r_summary = sm;
-            for (int i = 0; i < 8; i++) c.r_diag[i] = ctl.clk[i];
+            for (int i = 0; i < 16; i++) c.r_diag[i] = ctl.clk[i];
         }
     }
 }

@@ -302,6 +302,12 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         part[group] = V;
     }
 
+    // per-GPU flags: a GPU whose steps have ISSUED-kind successors always takes the cycle-serial issue path
+    std::vector<u32> gflag(G, 0);
+    for (u32 s = 0; s < S; s++)
+        for (u32 i = c.succ_ptr[s]; i < c.succ_ptr[s + 1]; i++)
+            if ((c.succ[i] >> 30) == ASTRA_DEP_ISSUED) gflag[c.owner[s]] |= ASTRA_GF_ISSUED_DEPS;
+
     // constant tables
     u64* co = P.c_off;
     co[ASTRA_C_in_ptr] = topo_off[0]; co[ASTRA_C_in_link] = topo_off[1]; co[ASTRA_C_head] = topo_off[2];
@@ -322,6 +328,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_classoff] = blob.add(classoff); co[ASTRA_C_nd_mw] = blob.add(nd_mw);
     co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
     co[ASTRA_C_part] = blob.add(part);
+    co[ASTRA_C_gflag] = blob.add(gflag);
 
     // mutable arrays: sizes, then placement (shared memory in declaration order while it fits)
     const u64 GW = (u64)G * CW;
@@ -329,7 +336,10 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     for (u32 a : {ASTRA_A_pipe_head, ASTRA_A_fifo_head, ASTRA_A_ltail, ASTRA_A_run, ASTRA_A_lstate0, ASTRA_A_lstate1,
                   ASTRA_A_link_lines, ASTRA_A_dirty, ASTRA_A_ndue}) ab[a] = 4ull * E;
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
-    ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = 4ull * G * P.nwords;
+    ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
+    ab[ASTRA_A_gmode] = 4ull * G;
+    ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
+    ab[ASTRA_A_evb] = 8ull * G * g.H * W;
     ab[ASTRA_A_sel] = 4ull * G * g.H;
     ab[ASTRA_A_masks] = 4ull * mask_total; ab[ASTRA_A_pre] = 4ull * pre_total;
     for (u32 a : {ASTRA_A_t_release, ASTRA_A_issued_cnt, ASTRA_A_t_issued, ASTRA_A_deliv_cnt, ASTRA_A_t_deliv,
@@ -344,9 +354,13 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     u64 hot = 0, ws = 0;
     for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
         ab[a] = (std::max<u64>(ab[a], 16) + 15) & ~15ull;
-        // streamed arrays and, for a CTA group, everything another CTA may touch stay in global memory
+        // streamed arrays stay in global memory; so does, for a CTA group, what another CTA of the group
+        // reads or writes: link cursors seen from both ends, ack records / bitmap / bin counts (written
+        // at the destination, read at the owner).  Every other array is only ever touched by the CTA
+        // that owns the node, so each CTA keeps its own shared-memory copy and uses its nodes' part.
         bool global_only = a == ASTRA_A_bitmap || a == ASTRA_A_ack_rec || a == ASTRA_A_ack_tmp ||
-                           a == ASTRA_A_ack_sorted || a == ASTRA_A_ring || group > 1;
+                           a == ASTRA_A_ack_sorted || a == ASTRA_A_ring || a == ASTRA_A_evb ||
+                           (group > 1 && (a == ASTRA_A_pipe_head || a == ASTRA_A_fifo_head || a == ASTRA_A_bin_cnt));
         if (!global_only && hot + ab[a] <= opt.hot_budget) { P.a_off[a] = hot | ASTRA_PLACE_SMEM; hot += ab[a]; }
         else { P.a_off[a] = ws; ws += ab[a]; }
     }
