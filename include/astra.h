@@ -66,6 +66,7 @@ extern "C" {
 #define ASTRA_FLAG_NO_WINDOW_SKIP 1ull   /* step through every lookahead window (testing I8)   */
 #define ASTRA_FLAG_WINDOW_1       2ull   /* force a 1-cycle lookahead window (testing I8)      */
 #define ASTRA_FLAG_SERIAL_ISSUE   4ull   /* always take the cycle-serial issue path (testing)  */
+#define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g
                                             CTAs (1..16), one node range each; 0 = engine's choice */
 

@@ -59,7 +59,8 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 decision;       // 0 = run window `next_k`, else 1 + status
     u32 next_k;
     u32 any_merged;     // some multi-feeder out-link received lines this window
-    u32 acked_total, pad;
+    u32 ntasks;         // link tasks of stage 1 this window
+    u32 acked_total;
     u64 busy, skipped;
     u64 clk[16];        // diagnostics: [0] windows, [1..4] SM clocks in stage groups, [5] init, [6] serial GPU-windows, [8..15] stage-2 parts
 };
@@ -230,71 +231,6 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 t0, u32 wlen, u32 cb,
 }
 
 // ---------------------------------------------------------------------------------------------
-// stage 1b: this window's acks of GPU g (R6, A3): per-step ack counts, t_ack, ACKED events, and the
-// wavefronts that get a slot back this window (amask).  The bitmap of the window's bin holds one
-// bit per (wavefront, slot); ack_rec the (step, cycle) of each.  Nothing is consumed here: the
-// wavefront simulation (wf_sim) or, on the cycle-serial path, ack_sort reads the same bits again.
-// ---------------------------------------------------------------------------------------------
-__device__ void ack_discover(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 lane) {
-    const u32 bin = k & c.NWmask;
-    // earliest later window with acks pending for this GPU (A7)
-    {
-        u32 best = ASTRA_T_INF;
-        for (u32 j = 1 + lane; j < c.NW; j += 32)
-            if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
-        best = __reduce_min_sync(FULL, best);
-        if (lane == 0 && best != ASTRA_T_INF) {
-            const u64 tw = (u64)(k + best) << c.logW;
-            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
-        }
-    }
-    const u32 n = ld_vol(&c.bin_cnt[g * c.NW + bin]);
-    if (lane == 0) c.ack_n[g] = n;
-    if (n == 0) return;
-    const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
-    const u64* rec = c.ack_rec + (size_t)g * c.slots;
-    u32* am = c.amask + (size_t)g * c.nwords;
-    u32 total = 0, acked_steps = 0, completion = 0;
-    for (u32 wb = 0; wb < c.bmwords; wb += 32) {
-        const u32 wi = wb + lane;
-        u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
-        while (__any_sync(FULL, w != 0)) {
-            const bool act = w != 0;
-            const u32 amk = __ballot_sync(FULL, act);
-            bool completed = false;
-            if (act) {
-                const u32 b = __ffs(w) - 1; w &= w - 1;
-                const u32 idx = wi * 32 + b;
-                const u64 rc = __ldcg(&rec[idx]);
-                const u32 step = (u32)(rc >> 32), ta = (u32)rc;
-                const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K
-                atomicOr(&am[wf >> 5], 1u << (wf & 31));
-                const u32 m = __match_any_sync(amk, step);
-                const u32 cmax = __reduce_max_sync(m, ta);
-                if ((m & lanemask_lt()) == 0) {
-                    const u32 ac = c.ack_cnt[step] + __popc(m);
-                    const u32 tm = max(c.t_ack[step], cmax);
-                    c.ack_cnt[step] = ac; c.t_ack[step] = tm;
-                    if (ac == c.lines[step]) {
-                        completed = true;
-                        const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
-                        c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
-                        completion = max(completion, tm);
-                    }
-                }
-            }
-            total += __popc(amk);
-            acked_steps += __popc(__ballot_sync(FULL, completed));
-        }
-    }
-    completion = __reduce_max_sync(FULL, completion);
-    if (lane == 0) {
-        if (total != n) atomicOr(&ctl.err, 2u);
-        if (acked_steps) { atomicAdd(&ctl.acked, acked_steps); atomicMax(&ctl.completion, completion); }
-    }
-    __syncwarp();
-}
-
 // Cycle-serial path only: consume the window's ack bits of GPU g into ack_sorted, counting-sorted
 // by cycle (low word: cycle << 18 | wavefront << 6 | slot).
 __device__ void ack_sort(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
@@ -350,6 +286,163 @@ __device__ void ack_sort(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* 
         if (total != n) atomicOr(&ctl.err, 2u);
     }
     __syncwarp();
+}
+
+// ---------------------------------------------------------------------------------------------
+// stage 1 as a flat task list.  The number of lines due on every in-link this window is known
+// (link_service counted them per arrival window), so a link whose lines all terminate at its head,
+// or all go on to one single-feeder link, is cut into independent chunks of 32 pipe entries; any
+// other link stays one task (arrivals_link).  Ack discovery is cut into chunks of 32 bitmap words.
+// ---------------------------------------------------------------------------------------------
+__device__ void stage1_setup_gpu(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 lane) {
+    u32 best = ASTRA_T_INF;                                     // earliest later window with acks pending (A7)
+    for (u32 j = 1 + lane; j < c.NW; j += 32)
+        if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
+    best = __reduce_min_sync(FULL, best);
+    if (lane == 0) {
+        if (best != ASTRA_T_INF) {
+            const u64 tw = (u64)(k + best) << c.logW;
+            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
+        }
+        c.ack_n[g] = ld_vol(&c.bin_cnt[g * c.NW + (k & c.NWmask)]);
+    }
+}
+
+__device__ void stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
+    const u32 e = c.in_link[i];
+    u32* dc = &c.due_cnt[(size_t)e * c.NW + (k & c.NWmask)];
+    const u32 n = ld_vol(dc);
+    if (n) *dc = 0;
+    const u32 lo = c.pipe_head[e], hi = ld_vol(&c.fifo_head[e]);
+    const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
+    u32 nch = 0;
+    if (fl) {
+        if (n) {
+            nch = (n + 31) / 32;
+            c.tl_lo[e] = lo; c.tl_n[e] = n; c.pipe_head[e] = lo + n;
+            if (fl == ASTRA_LF_FORWARD_ONLY) { const u32 o = c.lfwd[e]; c.tl_base[e] = c.run[o]; c.run[o] += n; }
+        }
+        if (hi != lo + n) {                                     // in flight beyond this window: next arrival (A7)
+            const u64 flit = __ldcg(&c.ring[c.ring_off[e] + ((lo + n) & c.ring_mask[e])]);
+            atomicMin(&ctl.next_hint, t0 + (((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26));
+        }
+        if (hi - lo > c.ring_mask[e] + 1) atomicOr(&ctl.err, 1u);
+    } else if (hi != lo) nch = 1;
+    c.tbase[i] = nch;
+}
+
+// exclusive prefix of the per-link task counts (one warp); tbase[i_hi] = total
+__device__ void stage1_prefix(Ctx& c, Ctl& ctl, u32 lane) {
+    u32 carry = 0;
+    for (u32 b = c.i_lo; b < c.i_hi; b += 32) {
+        const u32 i = b + lane;
+        const u32 v = (i < c.i_hi) ? c.tbase[i] : 0;
+        const u32 incl = warp_incl_scan(v, lane);
+        if (i < c.i_hi) c.tbase[i] = carry + incl - v;
+        carry += __shfl_sync(FULL, incl, 31);
+    }
+    if (lane == 0) { c.tbase[c.i_hi] = carry; ctl.ntasks = carry; }
+}
+
+// 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3)
+__device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32 lane) {
+    const u32 bin = k & c.NWmask;
+    const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
+    const u64* rec = c.ack_rec + (size_t)g * c.slots;
+    u32* am = c.amask + (size_t)g * c.nwords;
+    const u32 wi = chunk * 32 + lane;
+    u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
+    u32 acked_steps = 0, tmax = 0;
+    while (__any_sync(FULL, w != 0)) {
+        const bool act = w != 0;
+        const u32 amk = __ballot_sync(FULL, act);
+        bool completed = false;
+        if (act) {
+            const u32 b = __ffs(w) - 1; w &= w - 1;
+            const u32 idx = wi * 32 + b;
+            const u64 rc = __ldcg(&rec[idx]);
+            const u32 ta = (u32)rc;
+            const u32 step = ta < t1 ? (u32)(rc >> 32) : 0xffffffffu;     // beyond the watchdog cut: not processed
+            const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K
+            atomicOr(&am[wf >> 5], 1u << (wf & 31));
+            const u32 m = __match_any_sync(amk, step);
+            const u32 cmax = __reduce_max_sync(m, ta);
+            if (step != 0xffffffffu) tmax = max(tmax, ta);
+            if ((m & lanemask_lt()) == 0 && step != 0xffffffffu) {
+                atomicMax(&c.t_ack[step], cmax);
+                const u32 cntm = __popc(m);
+                const u32 old = atomicAdd(&c.ack_cnt[step], cntm);
+                if (old + cntm == c.lines[step]) {
+                    completed = true;
+                    const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
+                    c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
+                }
+            }
+        }
+        acked_steps += __popc(__ballot_sync(FULL, completed));
+    }
+    tmax = __reduce_max_sync(FULL, tmax);
+    if (lane == 0) {
+        if (acked_steps) atomicAdd(&ctl.acked, acked_steps);
+        if (tmax) atomicMax(&ctl.completion, tmax);
+    }
+}
+
+// 32 pipe entries of a link whose lines all terminate at its head GPU (R7 A1, deliveries)
+__device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
+    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+    const u32 ii = lo + chunk * 32 + lane;
+    bool valid = (int32_t)(lo + n - ii) > 0;
+    u64 flit0 = 0;
+    if (valid) {
+        flit0 = __ldcg(&c.ring[c.ring_off[e] + (ii & c.ring_mask[e])]);
+        valid = (((u32)(flit0 >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) < wlen;   // watchdog cut inside the window
+    }
+    const u32 amk = __ballot_sync(FULL, valid);
+    u32 hint = ASTRA_T_INF;
+    if (valid) {
+        const u32 v = c.head[e];
+        const u64 flit = flit0;
+        const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
+        const u32 step = (u32)flit & 0xfffffu;
+        const u32 owner = c.step_od[step] >> 16;
+        const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
+        const u32 ta = t0 + d + c.step_alpha[step];                       // R6
+        const u32 bit = wf * c.K + slot;
+        c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
+        const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+        atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
+        const u32 mb = __match_any_sync(amk, bin);
+        if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+        hint = ta;
+        const u32 m = __match_any_sync(amk, step);
+        const u32 dmax = __reduce_max_sync(m, d);
+        if ((m & lanemask_lt()) == 0) {
+            atomicMax(&c.t_deliv[step], t0 + dmax);
+            const u32 cntm = __popc(m);
+            const u32 old = atomicAdd(&c.deliv_cnt[step], cntm);
+            if (old + cntm == c.lines[step]) {                  // DELIVERED event at GPU v (dst of the step)
+                const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
+                c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
+            }
+        }
+        hint = __reduce_min_sync(amk, hint);
+        if ((amk & lanemask_lt()) == 0) atomicMin(&ctl.next_hint, hint);
+    }
+}
+
+// 32 pipe entries of a link whose lines all go on to the single-feeder link lfwd[e] (R7 A1, transit):
+// stream order is FIFO order, so the position is the base plus the index in the stream
+__device__ void forward_chunk(Ctx& c, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
+    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+    const u32 ii = lo + chunk * 32 + lane;
+    if ((int32_t)(lo + n - ii) <= 0) return;
+    const u64 flit = __ldcg(&c.ring[c.ring_off[e] + (ii & c.ring_mask[e])]);
+    const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
+    if (d >= wlen) return;                                      // watchdog cut inside the window
+    const u32 o = c.lfwd[e];
+    const u32 pos = c.tl_base[e] + (ii - lo);
+    c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -681,46 +774,58 @@ __device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
     if (active) mode = ((c.gflag[g] & ASTRA_GF_ISSUED_DEPS) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE)) ? 2u : 1u;
     if (mode == 1) {
         const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-        u32* h = c.hist + (size_t)e0 * c.W;
-        for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0;
+        u32* cnt = c.cnt + (size_t)g * c.W;
+        for (u32 i = lane; i < c.W; i += 32) cnt[i] = 0;
+        if (deg > 1) {
+            u32* h = c.hist + (size_t)e0 * c.W;
+            for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0;
+        }
     }
     if (lane == 0) c.gmode[g] = mode;
 }
 
-// stage 2b / 2d: the 32 wavefronts of word wi of GPU g.  PASS 0 counts the issues per (link, cycle);
-// PASS 1 (after the budget check) stores them in their buckets and commits the wavefront state.
-template <int PASS>
+// stage 2b: the 32 wavefronts of word wi of GPU g, each on its own thread, run through the window as
+// if the HBM budget never bound.  Issues go to the bucket of their cycle (first H of a cycle are
+// kept: more than H means the budget binds and the GPU-window is redone cycle-serially).  The new
+// wavefront state is written in place, the old one kept in the undo arrays for that case.
 __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
-    u32* amp = c.amask + (size_t)g * c.nwords + wi;
-    const u32 am = *amp;
+    const u32 nwords = c.nwords;
+    const u32 am = c.amask[(size_t)g * nwords + wi];
     if (am == 0) return;
     const bool active = (am >> lane) & 1u;
     const u32 wf = wi * 32 + lane;
-    const u32 e0 = c.row_ptr[g];
-    u32* h = c.hist + (size_t)e0 * c.W;
+    const u32 W = c.W, H = c.H, K = c.K;
+    const u64 fullmask = c.fullmask;
     bool wantb = false, freebit = false, hint = false;
     if (active) {
+        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+        u32* const cnt = c.cnt + (size_t)g * W;
+        u32* const h = c.hist + (size_t)e0 * W;
+        u64* const evb = c.evb + (size_t)g * H * W;
+        const u32* const t_release = c.t_release;
+        const u32* const cul = c.cul;
         const size_t gw = (size_t)g * c.CW + wf;
         u32 cur = c.wf_cur[gw], rem = c.wf_rem[gw];
         u64 busy = c.wf_busy[gw];
+        c.undo_cur[gw] = cur; c.undo_rem[gw] = rem; c.undo_busy[gw] = busy;
         // this wavefront's ack bits of the window's bin: bits [wf*K, wf*K + K) of the GPU's bitmap
-        u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
-        const u32 b0 = wf * c.K, w0 = b0 >> 5, sh = b0 & 31;
+        const u32 b0 = wf * K, w0 = b0 >> 5, sh = b0 & 31;
         u64 rb = 0;
         if (c.ack_n[g]) {
+            const u32 bmwords = c.bmwords;
+            const u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * bmwords;
             const u32 x0 = __ldcg(&bm[w0]);
-            const u32 x1 = (w0 + 1 < c.bmwords) ? __ldcg(&bm[w0 + 1]) : 0u;
-            const u32 x2 = (sh && w0 + 2 < c.bmwords) ? __ldcg(&bm[w0 + 2]) : 0u;
+            const u32 x1 = (w0 + 1 < bmwords) ? __ldcg(&bm[w0 + 1]) : 0u;
+            const u32 x2 = (sh && w0 + 2 < bmwords) ? __ldcg(&bm[w0 + 2]) : 0u;
             rb = ((((u64)x1 << 32) | x0) >> sh);
             if (sh) rb |= (u64)x2 << (64 - sh);
-            rb &= c.fullmask;
+            rb &= fullmask;
         }
-        const u64 rb_all = rb;
-        const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
         // the wavefront's acks of the window, sorted by cycle: (cycle - t0) << 6 | slot
         u32 aq[64];
         u32 na = 0, ai = 0;
-        {
+        if (rb) {
+            const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
             u64 x = rb;
             while (x) {                                         // four loads in flight at a time
                 u32 b[4]; u32 v[4]; int m = 0;
@@ -737,18 +842,19 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
                 aq[j] = xv;
             }
         }
-        u32 na_t = na ? t0 + (aq[0] >> 6) : ASTRA_T_INF;        // earliest ack not applied yet
+        u32 nq = na ? aq[0] : 0xffffffffu;                       // earliest ack not applied yet (packed)
         const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
-        u32 t = t0, s = 0, o = 0, scnt = 0, slast = 0, last_issue = ASTRA_T_INF;
+        const u32 wlen = t1 - t0;
+        u32 tt = 0, s = 0, ox = 0, last_issue = 0xffffffffu;    // tt: candidate cycle relative to t0
         bool have_s = false;
         for (;;) {
             if (rem == ASTRA_NOTLOADED) {
                 bool got = false;
                 while (cur < end) {
-                    const u32 s2 = c.cul[cur];
-                    const u32 tr = c.t_release[s2];
+                    const u32 s2 = cul[cur];
+                    const u32 tr = t_release[s2];
                     if (tr >= t1) break;                        // not released by the end of the window
-                    if (tr > t) t = tr;
+                    if (tr > t0 + tt) tt = tr - t0;
                     const u32 q = c.step_q[s2] + (((wf - c.cu_lo[s2] * c.Wv) < c.step_r[s2]) ? 1u : 0u);   // R11
                     if (q) { rem = q; got = true; break; }
                     cur++;
@@ -756,99 +862,111 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
                 if (!got) break;
                 have_s = false;
             }
-            if (!have_s) { s = c.cul[cur]; o = c.first_link[s]; have_s = true; }
-            while (na_t <= t) {                                 // slots returned by cycle t (A3 before D)
-                busy &= ~(1ull << (aq[ai] & 63u)); ai++;
-                na_t = ai < na ? t0 + (aq[ai] >> 6) : ASTRA_T_INF;
+            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; have_s = true; }
+            if (busy == fullmask) {                             // all K slots in flight: wait for the next ack
+                if (ai >= na) break;
+                tt = max(tt, nq >> 6);
             }
-            if (t >= t1) break;
-            if (busy == c.fullmask) {                           // all K slots in flight: wait for the next ack
-                if (na_t >= t1) break;
-                t = na_t; continue;
+            while ((nq >> 6) <= tt) {                           // slots returned by this cycle (A3 before D)
+                busy &= ~(1ull << (nq & 63u)); ai++;
+                nq = ai < na ? aq[ai] : 0xffffffffu;
             }
+            if (tt >= wlen) break;
             const u32 slot = __ffsll((long long)~busy) - 1;
             busy |= 1ull << slot;
-            const u32 key = (o - e0) * c.W + (t - t0);
-            if (PASS == 0) atomicAdd(&h[key], 1u);
-            else {
-                const u32 pos = atomicAdd(&h[key], 1u);
-                c.evb[(size_t)g * c.H * c.W + pos] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(t + 1 - t0) << ASTRA_FLIT_TIME_SHIFT);
-                scnt++; slast = t;
-            }
-            last_issue = t;
-            rem--; t++;
-            if (rem == 0) {
-                if (PASS == 1) { atomicAdd(&c.issued_cnt[s], scnt); atomicMax(&c.t_issued[s], slast); scnt = 0; }
-                cur++; rem = ASTRA_NOTLOADED;
-            }
+            const u32 p = atomicAdd(&cnt[tt], 1u);
+            if (p < H) evb[(size_t)tt * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(tt + 1) << ASTRA_FLIT_TIME_SHIFT);
+            if (deg > 1) atomicAdd(&h[ox * W + tt], 1u);
+            last_issue = tt;
+            rem--; tt++;
+            if (rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
         }
-        if (PASS == 1) {
-            if (scnt) { atomicAdd(&c.issued_cnt[s], scnt); atomicMax(&c.t_issued[s], slast); }
-            for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));   // acks later in the window than the last look
-            c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
-            if (rb_all) {                                       // consume the ack bits
-                const u32 m0 = (u32)(rb_all << sh);
-                if (m0) atomicAnd(&bm[w0], ~m0);
-                const u32 m1 = (u32)((sh ? (rb_all >> (32 - sh)) : (rb_all >> 32)));
-                if (m1) atomicAnd(&bm[w0 + 1], ~m1);
-                const u32 m2 = sh ? (u32)(rb_all >> (64 - sh)) : 0u;
-                if (m2) atomicAnd(&bm[w0 + 2], ~m2);
-            }
-            wantb = rem != ASTRA_NOTLOADED;
-            freebit = busy != c.fullmask;
-            hint = (wantb && freebit) || last_issue == t1 - 1;
-        }
+        for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));   // acks later in the window than the last look
+        c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
+        wantb = rem != ASTRA_NOTLOADED;
+        freebit = busy != fullmask;
+        hint = (wantb && freebit) || last_issue == wlen - 1;
     }
-    if (PASS == 1) {
-        const u32 wm = __ballot_sync(FULL, wantb), fm = __ballot_sync(FULL, freebit);
-        const bool anyh = __any_sync(FULL, hint);
-        if (lane == 0) {
-            u32* want = c.want + (size_t)g * c.nwords + wi;
-            u32* freeb = c.freeb + (size_t)g * c.nwords + wi;
-            *want = (*want & ~am) | wm;
-            *freeb = (*freeb & ~am) | fm;
-            *amp = 0;
-            if (anyh) atomicMin(&ctl.next_hint, t1);
-        }
+    __syncwarp();
+    const u32 wm = __ballot_sync(FULL, wantb), fm = __ballot_sync(FULL, freebit);
+    const bool anyh = __any_sync(FULL, hint);
+    if (lane == 0) {
+        u32* want = c.want + (size_t)g * nwords + wi;
+        u32* freeb = c.freeb + (size_t)g * nwords + wi;
+        const u32 ow = *want, of = *freeb;
+        c.undo_want[(size_t)g * nwords + wi] = ow; c.undo_freeb[(size_t)g * nwords + wi] = of;
+        *want = (ow & ~am) | wm;
+        *freeb = (of & ~am) | fm;
+        if (anyh) atomicMin(&ctl.next_hint, t1);
     }
 }
 
-// stage 2c: did the HBM budget bind in any cycle (R12)?  If not: exclusive prefix over the
-// (link, cycle) counts = bucket bases; direct out-links get their new tails.
-__device__ void gpu_check(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
-    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-    u32* h = c.hist + (size_t)e0 * c.W;
-    bool bind = false;
-    if (c.H < c.CW) {
-        for (u32 tt = lane; tt < wlen; tt += 32) {
-            u32 tot = 0;
-            for (u32 x = 0; x < deg; x++) tot += h[x * c.W + tt];
-            if (tot > c.H) bind = true;
+// The budget bound: put the wavefronts of GPU g back to their state at the window start.
+__device__ void wf_restore(Ctx& c, u32 g, u32 lane) {
+    for (u32 wi = 0; wi < c.nwords; wi++) {
+        const u32 am = c.amask[(size_t)g * c.nwords + wi];
+        if (am == 0) continue;
+        if ((am >> lane) & 1u) {
+            const size_t gw = (size_t)g * c.CW + wi * 32 + lane;
+            c.wf_cur[gw] = c.undo_cur[gw]; c.wf_rem[gw] = c.undo_rem[gw]; c.wf_busy[gw] = c.undo_busy[gw];
+        }
+        if (lane == 0) {
+            c.want[(size_t)g * c.nwords + wi] = c.undo_want[(size_t)g * c.nwords + wi];
+            c.freeb[(size_t)g * c.nwords + wi] = c.undo_freeb[(size_t)g * c.nwords + wi];
         }
     }
+    __syncwarp();
+}
+
+// stage 2c: did the HBM budget bind in any cycle (R12)?  If not, the run stands: exclusive prefix of
+// the per-cycle counts (item enumeration), FIFO positions of every (direct out-link, cycle), new
+// tails, and the window's ack bits / released steps are consumed.
+__device__ void gpu_check(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
+    const u32 W = c.W;
+    u32* cnt = c.cnt + (size_t)g * W;
+    bool bind = false;
+    for (u32 tt = lane; tt < wlen; tt += 32) if (cnt[tt] > c.H) bind = true;
     if (__any_sync(FULL, bind)) {
         if (lane == 0) c.gmode[g] = 2u;
         return;
     }
-    const u32 nkeys = deg * c.W;
     u32 carry = 0;
-    for (u32 b = 0; b < nkeys; b += 32) {
+    for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
-        const u32 v = (i < nkeys) ? h[i] : 0;
+        const u32 v = (i < wlen) ? cnt[i] : 0;
         const u32 incl = warp_incl_scan(v, lane);
-        if (i < nkeys) h[i] = carry + incl - v;
+        if (i < W) cnt[i] = carry + incl - v;
         carry += __shfl_sync(FULL, incl, 31);
     }
-    __syncwarp();
-    for (u32 x = lane; x < deg; x += 32) {                      // direct out-links: new FIFO tails
-        const u32 o = e0 + x;
-        if (c.mask_off[o] != ASTRA_NONE32) continue;
-        const u32 st = h[x * c.W], en = (x + 1 < deg) ? h[(x + 1) * c.W] : carry;
-        if (en != st) c.run[o] += en - st;
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    if (deg == 1) {
+        if (lane == 0 && carry && c.mask_off[e0] == ASTRA_NONE32) c.run[e0] += carry;
+    } else if (carry) {
+        for (u32 x = 0; x < deg; x++) {                         // per out-link: absolute FIFO position of each cycle's first line
+            u32* h = c.hist + (size_t)(e0 + x) * W;
+            const bool direct = c.mask_off[e0 + x] == ASTRA_NONE32;
+            u32 acc = direct ? c.run[e0 + x] : 0u;
+            const u32 acc0 = acc;
+            for (u32 b = 0; b < W; b += 32) {
+                const u32 i = b + lane;
+                const u32 v = (i < wlen) ? h[i] : 0;
+                const u32 incl = warp_incl_scan(v, lane);
+                if (i < W) h[i] = acc + incl - v;
+                acc += __shfl_sync(FULL, incl, 31);
+            }
+            __syncwarp();
+            if (lane == 0 && direct && acc != acc0) c.run[e0 + x] = acc;
+        }
     }
+    // consume the acks of the window's bin and the releases
+    if (c.ack_n[g]) {
+        u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
+        for (u32 i = lane; i < c.bmwords; i += 32) bm[i] = 0;
+    }
+    for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
     if (lane == 0) {
-        c.sel[(size_t)g * c.H] = carry;                         // events of the GPU this window (sel is free on this path)
-        c.pcnt[g] = 0;                                          // the released steps are consumed by the wavefronts
+        c.sel[(size_t)g * c.H] = carry;                         // issues of the GPU this window (sel is free on this path)
+        c.pcnt[g] = 0;
         c.bin_cnt[g * c.NW + (k & c.NWmask)] = 0;
     }
     __syncwarp();
@@ -856,39 +974,47 @@ __device__ void gpu_check(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
 
 // stage 2e: rank the issues of GPU g inside their cycle (ascending wavefront id, R7 A2 / R12) and
 // put each line where that rank says: FIFO position on a direct out-link, cell slot + injection
-// record on a multi-feeder one.  After PASS 1, h[key] is the END of bucket key.
-__device__ void ev_place(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 cb, u32 lane) {
+// record on a multi-feeder one.  Item i of the window is entry i - cnt[tt] of the bucket of the
+// last cycle tt with cnt[tt] <= i (cnt = exclusive prefix of the per-cycle issue counts).
+__device__ void ev_place(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 t0, u32 cb, u32 lane) {
     const u32 nev = c.sel[(size_t)g * c.H];
     const u32 i = chunk * 32 + lane;
-    if (i >= nev) return;
-    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-    const u32* h = c.hist + (size_t)e0 * c.W;
-    const u64* ev = c.evb + (size_t)g * c.H * c.W;
-    const u64 rec = ev[i];
+    const bool act = i < nev;
+    const u32 amk = __ballot_sync(FULL, act);
+    if (!act) return;
+    const u32 W = c.W, H = c.H;
+    const u32* cnt = c.cnt + (size_t)g * W;
+    u32 lo = 0, hi = W;                                         // first index with cnt > i
+    while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (cnt[mid] > i) hi = mid; else lo = mid + 1; }
+    const u32 tt = lo - 1;
+    const u32 st = cnt[tt], n = (tt + 1 < W ? cnt[tt + 1] : nev) - st;
+    const u64* bucket = c.evb + ((size_t)g * W + tt) * H;
+    const u64 rec = bucket[i - st];
     const u32 s = (u32)rec & 0xfffffu, wf = ((u32)rec >> 20) & 0xfffu;
-    const u32 d = (u32)(rec >> ASTRA_FLIT_TIME_SHIFT);
-    const u32 o = c.first_link[s], ox = o - e0, tt = d - 1;
-    const u32 key = ox * c.W + tt;
-    const u32 st = key ? h[key - 1] : 0u, en = h[key];
-    u32 jo = 0;
-    for (u32 x = st; x < en; x++) jo += ((((u32)ev[x]) >> 20) & 0xfffu) < wf;
+    const u32 d = tt + 1;
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    const u32 o = c.first_link[s];
+    u32 j = 0, jo = 0;
+    for (u32 x = 0; x < n; x++) {
+        const u32 r2 = (u32)bucket[x];
+        const bool lower = ((r2 >> 20) & 0xfffu) < wf;
+        j += lower;
+        if (deg > 1) jo += lower && c.first_link[r2 & 0xfffffu] == o;
+    }
+    if (deg == 1) jo = j;
     if (c.mask_off[o] == ASTRA_NONE32) {
-        const u32 en_o = h[ox * c.W + c.W - 1];
-        const u32 pos = c.run[o] - (en_o - (st + jo));
+        const u32 pos = (deg == 1 ? c.run[o] - nev + st : c.hist[(size_t)o * W + tt]) + jo;
         c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
     } else {
-        u32 j = jo;
-        for (u32 x2 = 0; x2 < deg; x2++) {
-            if (x2 == ox) continue;
-            const u32 k2 = x2 * c.W + tt;
-            const u32 st2 = k2 ? h[k2 - 1] : 0u, en2 = h[k2];
-            for (u32 x = st2; x < en2; x++) j += ((((u32)ev[x]) >> 20) & 0xfffu) < wf;
-        }
         cell_set(c, ctl, o, g, cb, d, c.nd_injoff[g] + j);
         const u32 p = atomicAdd(&c.inj_n[g], 1u);
         if (p < c.inj_off[g + 1] - c.inj_off[g]) c.inj_list[c.inj_off[g] + p] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
         else atomicOr(&ctl.err, 4u);
     }
+    // issued counts and the cycle of each step's last issue (R3)
+    const u32 ms = __match_any_sync(amk, s);
+    const u32 tmax = __reduce_max_sync(ms, t0 + tt);
+    if ((ms & lanemask_lt()) == 0) { atomicAdd(&c.issued_cnt[s], (u32)__popc(ms)); atomicMax(&c.t_issued[s], tmax); }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1036,7 +1162,13 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
             last_x = __shfl_sync(FULL, x, 31 - __clz(accm));
             n_acc += __popc(accm);
         }
-        if (acc) ring[pos] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + x + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
+        if (acc) {
+            ring[pos] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + x + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
+            // lines due at the head per lookahead window: stage 1 of that window reads the count
+            const u32 wa = (t0 + x + leff) >> c.logW;
+            const u32 mb = __match_any_sync(accm, wa);
+            if ((mb & lanemask_lt()) == 0) atomicAdd(&c.due_cnt[(size_t)e * c.NW + (wa & c.NWmask)], (u32)__popc(mb));
+        }
         if (accm != actm) break;                             // FIFO: nothing behind a waiting line is accepted
     }
     if (lane == 0) {
@@ -1182,12 +1314,28 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             const u32 wlen = t1 - t0;
             const u32 cb = t0 % c.NC;
             busy += wlen;
-            // stage 1: arrivals per in-link, ack discovery per GPU
+            // stage 1: arrivals and ack discovery, as a flat list of chunk tasks
+            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) stage1_setup_gpu(c, ctl, g, k, lane);
+            for (u32 i = c.i_lo + tid; i < c.i_hi; i += nthr) stage1_setup_link(c, ctl, i, k, t0);
+            __syncthreads();
+            if (warp == 0) stage1_prefix(c, ctl, lane);
+            __syncthreads();
+            for (u32 g = c.g_lo; g < c.g_hi; g++) {
+                if (c.ack_n[g] == 0) continue;
+                const u32 nch = (c.bmwords + 31) / 32;
+                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ack_chunk(c, ctl, g, ch, k, t1, lane);
+            }
             {
-                const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
-                for (u32 task = warp; task < ng + ns; task += nwarps) {
-                    if (task < ng) ack_discover(c, ctl, c.g_lo + task, k, t0, lane);
-                    else arrivals_link<1>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
+                const u32 ntl = ctl.ntasks;
+                for (u32 task = nwarps - 1 - warp; task < ntl; task += nwarps) {
+                    u32 lo = c.i_lo, hi = c.i_hi;               // first in-link with tbase > task
+                    while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (c.tbase[mid] > task) hi = mid; else lo = mid + 1; }
+                    const u32 i = lo - 1, ch = task - c.tbase[i];
+                    const u32 e = c.in_link[i];
+                    const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
+                    if (fl == ASTRA_LF_DELIVER_ONLY) deliver_chunk(c, ctl, e, ch, t0, wlen, lane);
+                    else if (fl == ASTRA_LF_FORWARD_ONLY) forward_chunk(c, e, ch, t0, wlen, lane);
+                    else arrivals_link<1>(c, ctl, i, t0, wlen, cb, lane);
                 }
             }
             __syncthreads();
@@ -1200,33 +1348,28 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[8] += (u64)(ck - ck1); ck1 = ck; }
             for (u32 g = c.g_lo; g < c.g_hi; g++) {
                 if (c.gmode[g] != 1u) continue;
-                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim<0>(c, ctl, g, wi, k, t0, t1, lane);
+                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim(c, ctl, g, wi, k, t0, t1, lane);
             }
             __syncthreads();
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[9] += (u64)(ck - ck1); ck1 = ck; }
-            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) if (c.gmode[g] == 1u) gpu_check(c, ctl, g, k, wlen, lane);
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[10] += (u64)(ck - ck1); ck1 = ck; }
             for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) {
-                if (c.gmode[g] != 2u) continue;
+                if (c.gmode[g] == 1u) gpu_check(c, ctl, g, k, wlen, lane);
+                if (c.gmode[g] != 2u) continue;                  // cycle-serial path
                 if (lane == 0) atomicAdd((unsigned long long*)&ctl.clk[6], 1ull);
+                if (!((c.gflag[g] & ASTRA_GF_ISSUED_DEPS) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE))) wf_restore(c, g, lane);
                 ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
                 issue_window(c, ctl, g, t0, t1, cb, lane);
                 for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
             }
-            for (u32 g = c.g_lo; g < c.g_hi; g++) {
-                if (c.gmode[g] != 1u) continue;
-                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim<1>(c, ctl, g, wi, k, t0, t1, lane);
-            }
             __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[11] += (u64)(ck - ck1); ck1 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[10] += (u64)(ck - ck1); ck1 = ck; }
             for (u32 g = c.g_lo; g < c.g_hi; g++) {
                 if (c.gmode[g] != 1u) continue;
                 const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
-                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ev_place(c, ctl, g, ch, cb, lane);
+                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ev_place(c, ctl, g, ch, t0, cb, lane);
             }
             __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[12] += (u64)(ck - ck1); ck1 = ck; }
+            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[11] += (u64)(ck - ck1); ck1 = ck; }
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[2] += (u64)(ck - ck0); ck0 = ck; }
             // stage 3: merge into multi-feeder out-links (skipped when none received a line)
             if (ctl.any_merged) {

@@ -225,6 +225,8 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     std::vector<u64> bound(E, 0);
     std::vector<u32> feeder(E, ASTRA_NONE32);       // first feeder seen: in-link id, or E for injections
     std::vector<uint8_t> multi(E, 0);
+    std::vector<uint8_t> delivers(E, 0), transits(E, 0), multi_fwd(E, 0);
+    std::vector<u32> fwd(E, ASTRA_NONE32);       // the one link that lines arriving over e are forwarded to
     std::vector<double> load(V, 0.0);
     {
         std::vector<std::vector<u32>> by_owner(G);
@@ -241,6 +243,12 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
                     if (feeder[e] == ASTRA_NONE32) feeder[e] = prev;
                     else if (feeder[e] != prev) multi[e] = 1;
                     load[v] += c.lines[s]; load[t.head[e]] += c.lines[s];
+                    if (t.head[e] == d) delivers[e] = 1;
+                    else {
+                        transits[e] = 1;
+                        u32 e2 = t.next_link[(size_t)t.head[e] * G + d];
+                        if (fwd[e] == ASTRA_NONE32) fwd[e] = e2; else if (fwd[e] != e2) multi_fwd[e] = 1;
+                    }
                     prev = e;
                     v = t.head[e];
                     if (++hops > V) { err = "routing loop"; return ASTRA_EINVAL; }
@@ -302,6 +310,13 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         part[group] = V;
     }
 
+    // per-link flags for the chunk-parallel arrival paths: every line over e terminates at head(e), or
+    // every line over e is forwarded to the same single-feeder out-link
+    std::vector<u32> lflag(E, 0), lfwd(E, 0);
+    for (u32 e = 0; e < E; e++) {
+        if (delivers[e] && !transits[e]) lflag[e] = ASTRA_LF_DELIVER_ONLY;
+        else if (transits[e] && !delivers[e] && !multi_fwd[e] && !multi[fwd[e]]) { lflag[e] = ASTRA_LF_FORWARD_ONLY; lfwd[e] = fwd[e]; }
+    }
     // per-GPU flags: a GPU whose steps have ISSUED-kind successors always takes the cycle-serial issue path
     std::vector<u32> gflag(G, 0);
     for (u32 s = 0; s < S; s++)
@@ -329,15 +344,20 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
     co[ASTRA_C_part] = blob.add(part);
     co[ASTRA_C_gflag] = blob.add(gflag);
+    co[ASTRA_C_lflag] = blob.add(lflag); co[ASTRA_C_lfwd] = blob.add(lfwd);
 
     // mutable arrays: sizes, then placement (shared memory in declaration order while it fits)
     const u64 GW = (u64)G * CW;
     u64* ab = P.a_bytes;
     for (u32 a : {ASTRA_A_pipe_head, ASTRA_A_fifo_head, ASTRA_A_ltail, ASTRA_A_run, ASTRA_A_lstate0, ASTRA_A_lstate1,
-                  ASTRA_A_link_lines, ASTRA_A_dirty, ASTRA_A_ndue}) ab[a] = 4ull * E;
+                  ASTRA_A_link_lines, ASTRA_A_dirty, ASTRA_A_ndue, ASTRA_A_tl_lo, ASTRA_A_tl_n, ASTRA_A_tl_base}) ab[a] = 4ull * E;
+    ab[ASTRA_A_due_cnt] = 4ull * E * P.NW;
+    ab[ASTRA_A_tbase] = 4ull * (E + 1);
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
     ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
     ab[ASTRA_A_gmode] = 4ull * G;
+    ab[ASTRA_A_cnt] = 4ull * G * W;
+    ab[ASTRA_A_undo_want] = ab[ASTRA_A_undo_freeb] = 4ull * G * P.nwords;
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
     ab[ASTRA_A_evb] = 8ull * G * g.H * W;
     ab[ASTRA_A_sel] = 4ull * G * g.H;
@@ -346,7 +366,8 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
                   ASTRA_A_ack_cnt, ASTRA_A_t_ack, ASTRA_A_ndep_left, ASTRA_A_rel_time, ASTRA_A_plist}) ab[a] = 4ull * S;
     ab[ASTRA_A_ev_list] = 4ull * ev_off[G];
     ab[ASTRA_A_bin_cnt] = 4ull * G * P.NW;
-    ab[ASTRA_A_wf_busy] = 8ull * GW; ab[ASTRA_A_wf_rem] = 4ull * GW; ab[ASTRA_A_wf_cur] = 4ull * GW;
+    ab[ASTRA_A_wf_busy] = ab[ASTRA_A_undo_busy] = 8ull * GW;
+    ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = 4ull * GW;
     ab[ASTRA_A_bitmap] = 4ull * G * P.NW * P.bmwords;
     ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
     ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
@@ -360,7 +381,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         // that owns the node, so each CTA keeps its own shared-memory copy and uses its nodes' part.
         bool global_only = a == ASTRA_A_bitmap || a == ASTRA_A_ack_rec || a == ASTRA_A_ack_tmp ||
                            a == ASTRA_A_ack_sorted || a == ASTRA_A_ring || a == ASTRA_A_evb ||
-                           (group > 1 && (a == ASTRA_A_pipe_head || a == ASTRA_A_fifo_head || a == ASTRA_A_bin_cnt));
+                           (group > 1 && (a == ASTRA_A_pipe_head || a == ASTRA_A_fifo_head || a == ASTRA_A_bin_cnt || a == ASTRA_A_due_cnt));
         if (!global_only && hot + ab[a] <= opt.hot_budget) { P.a_off[a] = hot | ASTRA_PLACE_SMEM; hot += ab[a]; }
         else { P.a_off[a] = ws; ws += ab[a]; }
     }

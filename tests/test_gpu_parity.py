@@ -11,7 +11,7 @@ from tests.parity import check_workload, compare_point
 
 pytestmark = pytest.mark.gpu
 
-FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1 = 1, 2
+FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS = 1, 2, 4, 8
 
 
 def _single(topo, coll, gpu, name="case", max_cycles=1 << 22):
@@ -61,7 +61,17 @@ def test_i8_skip_equivalence(flags):
     check_workload(configs.config1(), flags=flags)
 
 
-@pytest.mark.parametrize("group", [2, 3, 8])
+@pytest.mark.parametrize("flags", [FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_SERIAL_ISSUE | FLAG_SERIAL_ARRIVALS | 0x100])
+def test_engine_paths_agree(flags):
+    """The wavefront-parallel issue stage and the chunked arrival stage (defaults) and the cycle-serial /
+    one-task-per-link paths they fall back to give the same bits; 0x100 = one CTA per point."""
+    check_workload(configs.random_workload(91, n_points=6, max_gpus=6, max_steps=24, max_lines=200), flags=flags)
+    check_workload(configs.config1(), flags=flags)
+    check_workload(configs.config2(range(6, 8)), flags=flags, processes=4)
+    check_workload(configs.config4(12), flags=flags, oracle_flags=oracle.FLAG_PRUNED_SCAN, processes=6)
+
+
+@pytest.mark.parametrize("group", [1, 2, 3, 8])
 def test_cta_groups(group):
     """A design point spread over a group of CTAs (one node range each, one group barrier per
     window) gives the same bits as on one CTA."""
