@@ -344,42 +344,69 @@ __device__ void stage1_prefix(Ctx& c, Ctl& ctl, u32 lane) {
     if (lane == 0) { c.tbase[c.i_hi] = carry; ctl.ntasks = carry; }
 }
 
-// 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3)
-__device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32 lane) {
+// 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3).
+// The set bits are first compacted into the warp's scratch so that every lane handles the same
+// number of acks whatever their spread over the words, four record loads in flight per lane.
+__device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32* scr, u32 lane) {
+    const u32 CAP = 512;
     const u32 bin = k & c.NWmask;
     const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
     const u64* rec = c.ack_rec + (size_t)g * c.slots;
     u32* am = c.amask + (size_t)g * c.nwords;
     const u32 wi = chunk * 32 + lane;
-    u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
+    const u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
+    const u32 cntw = __popc(w);
+    const u32 incl = warp_incl_scan(cntw, lane);
+    const u32 excl = incl - cntw, total = __shfl_sync(FULL, incl, 31);
+    if (total == 0) return;
+    const u32 K = c.K, kmagic = c.kmagic;
+    const u32* lines = c.lines;
     u32 acked_steps = 0, tmax = 0;
-    while (__any_sync(FULL, w != 0)) {
-        const bool act = w != 0;
-        const u32 amk = __ballot_sync(FULL, act);
-        bool completed = false;
-        if (act) {
-            const u32 b = __ffs(w) - 1; w &= w - 1;
-            const u32 idx = wi * 32 + b;
-            const u64 rc = __ldcg(&rec[idx]);
-            const u32 ta = (u32)rc;
-            const u32 step = ta < t1 ? (u32)(rc >> 32) : 0xffffffffu;     // beyond the watchdog cut: not processed
-            const u32 wf = c.K == 1 ? idx : (u32)(((u64)idx * c.kmagic) >> 32);   // idx / K
-            atomicOr(&am[wf >> 5], 1u << (wf & 31));
-            const u32 m = __match_any_sync(amk, step);
-            const u32 cmax = __reduce_max_sync(m, ta);
-            if (step != 0xffffffffu) tmax = max(tmax, ta);
-            if ((m & lanemask_lt()) == 0 && step != 0xffffffffu) {
-                atomicMax(&c.t_ack[step], cmax);
-                const u32 cntm = __popc(m);
-                const u32 old = atomicAdd(&c.ack_cnt[step], cntm);
-                if (old + cntm == c.lines[step]) {
-                    completed = true;
-                    const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
-                    c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
-                }
+    for (u32 base = 0; base < total; base += CAP) {
+        {
+            u32 pos = excl, ww = w;
+            while (ww) {
+                const u32 b = __ffs(ww) - 1; ww &= ww - 1;
+                if (pos >= base && pos < base + CAP) scr[pos - base] = (lane << 5) | b;
+                pos++;
             }
         }
-        acked_steps += __popc(__ballot_sync(FULL, completed));
+        __syncwarp();
+        const u32 nn = min(CAP, total - base);
+        for (u32 j0 = 0; j0 < nn; j0 += 128) {
+            u32 idx[4]; u64 rc[4];
+#pragma unroll
+            for (int q = 0; q < 4; q++) { const u32 j = j0 + q * 32 + lane; idx[q] = j < nn ? chunk * 1024 + scr[j] : 0xffffffffu; }
+#pragma unroll
+            for (int q = 0; q < 4; q++) rc[q] = idx[q] != 0xffffffffu ? __ldcg(&rec[idx[q]]) : 0ull;
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const bool act = idx[q] != 0xffffffffu;
+                const u32 amk = __ballot_sync(FULL, act);
+                bool completed = false;
+                if (act) {
+                    const u32 ta = (u32)rc[q];
+                    const u32 step = ta < t1 ? (u32)(rc[q] >> 32) : 0xffffffffu;   // beyond the watchdog cut: not processed
+                    const u32 wf = K == 1 ? idx[q] : (u32)(((u64)idx[q] * kmagic) >> 32);   // idx / K
+                    atomicOr(&am[wf >> 5], 1u << (wf & 31));
+                    const u32 m = __match_any_sync(amk, step);
+                    const u32 cmax = __reduce_max_sync(m, ta);
+                    if (step != 0xffffffffu) tmax = max(tmax, ta);
+                    if ((m & lanemask_lt()) == 0 && step != 0xffffffffu) {
+                        atomicMax(&c.t_ack[step], cmax);
+                        const u32 cntm = __popc(m);
+                        const u32 old = atomicAdd(&c.ack_cnt[step], cntm);
+                        if (old + cntm == lines[step]) {
+                            completed = true;
+                            const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
+                            c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
+                        }
+                    }
+                }
+                acked_steps += __popc(__ballot_sync(FULL, completed));
+            }
+        }
+        __syncwarp();
     }
     tmax = __reduce_max_sync(FULL, tmax);
     if (lane == 0) {
@@ -846,6 +873,7 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
         const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
         const u32 wlen = t1 - t0;
         u32 tt = 0, s = 0, ox = 0, last_issue = 0xffffffffu;    // tt: candidate cycle relative to t0
+        u32 eq0 = 0, eq1 = 0, eq2 = 0, eq3 = 0, nb = 0;             // buffered issues: cycle << 6 | slot
         bool have_s = false;
         for (;;) {
             if (rem == ASTRA_NOTLOADED) {
@@ -874,12 +902,34 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
             if (tt >= wlen) break;
             const u32 slot = __ffsll((long long)~busy) - 1;
             busy |= 1ull << slot;
-            const u32 p = atomicAdd(&cnt[tt], 1u);
-            if (p < H) evb[(size_t)tt * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(tt + 1) << ASTRA_FLIT_TIME_SHIFT);
-            if (deg > 1) atomicAdd(&h[ox * W + tt], 1u);
+            // issues are buffered four at a time so that their bucket-slot atomics overlap
+            eq3 = eq2; eq2 = eq1; eq1 = eq0; eq0 = (tt << 6) | slot; nb++;
             last_issue = tt;
             rem--; tt++;
+            if (nb == 4 || rem == 0) {
+                u32 pp[4]; const u32 bb[4] = {eq0, eq1, eq2, eq3};
+#pragma unroll
+                for (int q = 0; q < 4; q++) pp[q] = (u32)q < nb ? atomicAdd(&cnt[bb[q] >> 6], 1u) : 0u;
+#pragma unroll
+                for (int q = 0; q < 4; q++) if ((u32)q < nb) {
+                    const u32 t2 = bb[q] >> 6;
+                    if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT);
+                    if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
+                }
+                nb = 0;
+            }
             if (rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
+        }
+        if (nb) {
+            u32 pp[4]; const u32 bb[4] = {eq0, eq1, eq2, eq3};
+#pragma unroll
+            for (int q = 0; q < 4; q++) pp[q] = (u32)q < nb ? atomicAdd(&cnt[bb[q] >> 6], 1u) : 0u;
+#pragma unroll
+            for (int q = 0; q < 4; q++) if ((u32)q < nb) {
+                const u32 t2 = bb[q] >> 6;
+                if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT);
+                if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
+            }
         }
         for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));   // acks later in the window than the last look
         c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
@@ -1115,11 +1165,16 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
     const u32 capq = c.ceilb[e] * 256u;
     u32 n_acc = 0, first_x = 0, last_x = 0;
 
+    // ring loads run two chunks ahead of the scan
+    u64 fq0 = lane < scan_limit ? ring[(fh + lane) & rmask] : 0ull;
+    u64 fq1 = 32 + lane < scan_limit ? ring[(fh + 32 + lane) & rmask] : 0ull;
     for (u32 base = 0; base < scan_limit; base += 32) {
         const u32 i = base + lane;
         const bool act = i < scan_limit;
         const u32 pos = (fh + i) & rmask;
-        const u64 flit = act ? ring[pos] : 0ull;
+        const u64 flit = fq0;
+        fq0 = fq1;
+        fq1 = i + 64 < scan_limit ? ring[(fh + i + 64) & rmask] : 0ull;
         // append cycle relative to t0: backlog was appended before the window
         const u32 a = (act && i >= n_back) ? ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) & 0x3ffu) : 0u;
         u32 x = 0xffffffffu;                                 // acceptance cycle relative to t0
@@ -1165,9 +1220,15 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
         if (acc) {
             ring[pos] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + x + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
             // lines due at the head per lookahead window: stage 1 of that window reads the count
+        }
+        if (accm) {                                          // arrivals of a chunk fall in at most two windows
             const u32 wa = (t0 + x + leff) >> c.logW;
-            const u32 mb = __match_any_sync(accm, wa);
-            if ((mb & lanemask_lt()) == 0) atomicAdd(&c.due_cnt[(size_t)e * c.NW + (wa & c.NWmask)], (u32)__popc(mb));
+            const u32 w_first = __shfl_sync(FULL, wa, __ffs(accm) - 1);
+            const u32 m0 = __ballot_sync(FULL, acc && wa == w_first);
+            if (lane == 0) {
+                atomicAdd(&c.due_cnt[(size_t)e * c.NW + (w_first & c.NWmask)], (u32)__popc(m0));
+                if (accm != m0) atomicAdd(&c.due_cnt[(size_t)e * c.NW + ((w_first + 1) & c.NWmask)], (u32)__popc(accm & ~m0));
+            }
         }
         if (accm != actm) break;                             // FIFO: nothing behind a waiting line is accepted
     }
@@ -1323,7 +1384,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             for (u32 g = c.g_lo; g < c.g_hi; g++) {
                 if (c.ack_n[g] == 0) continue;
                 const u32 nch = (c.bmwords + 31) / 32;
-                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ack_chunk(c, ctl, g, ch, k, t1, lane);
+                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ack_chunk(c, ctl, g, ch, k, t1, scr, lane);
             }
             {
                 const u32 ntl = ctl.ntasks;
