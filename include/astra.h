@@ -66,7 +66,9 @@ extern "C" {
 #define ASTRA_FLAG_NO_WINDOW_SKIP 1ull   /* step through every lookahead window (testing I8)   */
 #define ASTRA_FLAG_WINDOW_1       2ull   /* force a 1-cycle lookahead window (testing I8)      */
 #define ASTRA_FLAG_SERIAL_ISSUE   4ull   /* always take the cycle-serial issue path (testing)  */
+#define ASTRA_FLAG_NO_HEAVY        16ull  /* no warp-per-wavefront issue path (testing)         */
 #define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
+#define ASTRA_FLAG_DIAG_RANK(r) (((uint64_t)(r) & 0xfull) << 16) /* which CTA of a group reports astra_read_diag */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g
                                             CTAs (1..16), one node range each; 0 = engine's choice */
 
@@ -160,7 +162,8 @@ int32_t astra_read_results(astra_ctx* ctx, uint32_t point, astra_summary* out,
  * [1..4] SM clocks the point's first CTA spent in the stages of a window (arrivals + ack gather,
  * release + issue, multi-feeder merge, link service + next-non-idle decision), [5] SM clocks of
  * state initialisation, [6] GPU-windows that took the cycle-serial issue path, [8..12] SM clocks of
- * the parts of stage 2 (prepare, count, check, commit, place).  Same errors as astra_read_results. */
+ * the parts of stage 2 (prepare, wavefront runs, check + cycle-serial path, placement), [13] SM clocks
+ * waiting at the group barrier.  Same errors as astra_read_results. */
 int32_t astra_read_diag(astra_ctx* ctx, uint32_t point, uint64_t* out16);
 
 /* Diagnostics: device milliseconds (CUDA events on the ctx's stream) of the last batch and the

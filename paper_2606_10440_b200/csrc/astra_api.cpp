@@ -193,7 +193,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "device attribute");
     choose_shape(c, n, pts, max_nodes, (u32)sms, &c->group, &c->warps);
     PlanOptions opt;
-    opt.flags = c->flags & 0xff; opt.max_cycles = max_cycles; opt.group = c->group;
+    opt.flags = c->flags & 0xf00ffull; opt.max_cycles = max_cycles; opt.group = c->group;
     const u32 fixed = astra_engine_fixed_smem(c->warps);
     opt.hot_budget = (u32)smem_max > fixed + 1024 ? (u32)smem_max - fixed - 1024 : 0;
     u32 hot_max = 0;

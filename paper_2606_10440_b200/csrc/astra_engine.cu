@@ -803,6 +803,7 @@ __device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
         const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
         u32* cnt = c.cnt + (size_t)g * c.W;
         for (u32 i = lane; i < c.W; i += 32) cnt[i] = 0;
+        if (lane == 0) c.nheavy[g] = 0;
         if (deg > 1) {
             u32* h = c.hist + (size_t)e0 * c.W;
             for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0;
@@ -817,27 +818,20 @@ __device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
 // wavefront state is written in place, the old one kept in the undo arrays for that case.
 __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
     const u32 nwords = c.nwords;
-    const u32 am = c.amask[(size_t)g * nwords + wi];
-    if (am == 0) return;
-    const bool active = (am >> lane) & 1u;
+    const u32 am0 = c.amask[(size_t)g * nwords + wi];
+    if (am0 == 0) return;
+    const bool active = (am0 >> lane) & 1u;
     const u32 wf = wi * 32 + lane;
     const u32 W = c.W, H = c.H, K = c.K;
     const u64 fullmask = c.fullmask;
-    bool wantb = false, freebit = false, hint = false;
+    bool wantb = false, freebit = false, hint = false, heavy = false;
+    const size_t gw = (size_t)g * c.CW + wf;
+    const u32 b0 = wf * K, w0 = b0 >> 5, sh = b0 & 31;
+    u32 cur = 0, rem = 0;
+    u64 busy = 0, rb = 0;
     if (active) {
-        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-        u32* const cnt = c.cnt + (size_t)g * W;
-        u32* const h = c.hist + (size_t)e0 * W;
-        u64* const evb = c.evb + (size_t)g * H * W;
-        const u32* const t_release = c.t_release;
-        const u32* const cul = c.cul;
-        const size_t gw = (size_t)g * c.CW + wf;
-        u32 cur = c.wf_cur[gw], rem = c.wf_rem[gw];
-        u64 busy = c.wf_busy[gw];
-        c.undo_cur[gw] = cur; c.undo_rem[gw] = rem; c.undo_busy[gw] = busy;
+        cur = c.wf_cur[gw]; rem = c.wf_rem[gw]; busy = c.wf_busy[gw];
         // this wavefront's ack bits of the window's bin: bits [wf*K, wf*K + K) of the GPU's bitmap
-        const u32 b0 = wf * K, w0 = b0 >> 5, sh = b0 & 31;
-        u64 rb = 0;
         if (c.ack_n[g]) {
             const u32 bmwords = c.bmwords;
             const u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * bmwords;
@@ -848,6 +842,25 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
             if (sh) rb |= (u64)x2 << (64 - sh);
             rb &= fullmask;
         }
+        // a wavefront that may issue many lines this window, in a word where few do, gets a warp of
+        // its own (wf_heavy); when most of the word does, the lanes run the same long loop together
+        heavy = min(K - (u32)__popcll(busy) + (u32)__popcll(rb), t1 - t0) >= ASTRA_HEAVY_MIN && !(c.flags & (u32)ASTRA_FLAG_NO_HEAVY);
+    }
+    __syncwarp();
+    if (__popc(__ballot_sync(FULL, heavy)) > ASTRA_HEAVY_MAX_PER_WORD) heavy = false;
+    if (heavy) {
+        const u32 hp = atomicAdd(&c.nheavy[g], 1u);
+        c.hlist[(size_t)g * c.CW + hp] = wf;
+    }
+    if (active) {
+        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+        u32* const cnt = c.cnt + (size_t)g * W;
+        u32* const h = c.hist + (size_t)e0 * W;
+        u64* const evb = c.evb + (size_t)g * H * W;
+        const u32* const t_release = c.t_release;
+        const u32* const cul = c.cul;
+      if (!heavy) {
+        c.undo_cur[gw] = cur; c.undo_rem[gw] = rem; c.undo_busy[gw] = busy;
         // the wavefront's acks of the window, sorted by cycle: (cycle - t0) << 6 | slot
         u32 aq[64];
         u32 na = 0, ai = 0;
@@ -936,10 +949,12 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
         wantb = rem != ASTRA_NOTLOADED;
         freebit = busy != fullmask;
         hint = (wantb && freebit) || last_issue == wlen - 1;
+      }
     }
     __syncwarp();
     const u32 wm = __ballot_sync(FULL, wantb), fm = __ballot_sync(FULL, freebit);
     const bool anyh = __any_sync(FULL, hint);
+    const u32 am = am0 & ~__ballot_sync(FULL, heavy);         // heavy wavefronts update their own bits later
     if (lane == 0) {
         u32* want = c.want + (size_t)g * nwords + wi;
         u32* freeb = c.freeb + (size_t)g * nwords + wi;
@@ -949,6 +964,129 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
         *freeb = (of & ~am) | fm;
         if (anyh) atomicMin(&ctl.next_hint, t1);
     }
+}
+
+// One wavefront with many issues in the window, on a whole warp: lane = issue index.  The i-th
+// issue of the window needs a slot -- one of the F0 slots free at the window start, else the
+// (i - F0)-th ack in cycle order -- and its step released, and comes at least one cycle after the
+// (i-1)-th: x_i = max(x_{i-1} + 1, c_i), a prefix maximum of c_j - j.  Same result as wf_sim.
+__device__ void wf_heavy(Ctx& c, Ctl& ctl, u32 g, u32 wf, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+    const u32 W = c.W, H = c.H, K = c.K, nwords = c.nwords;
+    const u64 fullmask = c.fullmask;
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    u32* const cnt = c.cnt + (size_t)g * W;
+    u32* const h = c.hist + (size_t)e0 * W;
+    u64* const evb = c.evb + (size_t)g * H * W;
+    const u32* const t_release = c.t_release;
+    const u32* const cul = c.cul;
+    const size_t gw = (size_t)g * c.CW + wf;
+    u32 cur = c.wf_cur[gw], rem = c.wf_rem[gw];
+    const u64 busy = c.wf_busy[gw];
+    if (lane == 0) { c.undo_cur[gw] = cur; c.undo_rem[gw] = rem; c.undo_busy[gw] = busy; }
+    const u32 b0 = wf * K, w0 = b0 >> 5, sh = b0 & 31;
+    u64 rb = 0;
+    if (c.ack_n[g]) {
+        const u32 bmwords = c.bmwords;
+        const u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * bmwords;
+        const u32 x0 = __ldcg(&bm[w0]);
+        const u32 x1 = (w0 + 1 < bmwords) ? __ldcg(&bm[w0 + 1]) : 0u;
+        const u32 x2 = (sh && w0 + 2 < bmwords) ? __ldcg(&bm[w0 + 2]) : 0u;
+        rb = ((((u64)x1 << 32) | x0) >> sh);
+        if (sh) rb |= (u64)x2 << (64 - sh);
+        rb &= fullmask;
+    }
+    const u32 na = __popcll(rb);
+    const u64 fb = ~busy & fullmask;
+    const u32 F0 = __popcll(fb);
+    // scr[64 ..): positions of the set bits of rb (acked slots); scr[128 ..): of fb (free slots)
+    {
+        const u32 rlo = (u32)rb, rhi = (u32)(rb >> 32), flo = (u32)fb, fhi = (u32)(fb >> 32), lt = lanemask_lt();
+        if ((rlo >> lane) & 1u) scr[64 + __popc(rlo & lt)] = lane;
+        if ((rhi >> lane) & 1u) scr[64 + __popc(rlo) + __popc(rhi & lt)] = 32 + lane;
+        if ((flo >> lane) & 1u) scr[128 + __popc(flo & lt)] = lane;
+        if ((fhi >> lane) & 1u) scr[128 + __popc(flo) + __popc(fhi & lt)] = 32 + lane;
+        __syncwarp();
+    }
+    // acks sorted by (cycle, slot) into scr[0 .. na): rank = number of smaller keys
+    {
+        const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
+        u32 key0 = 0xffffffffu, key1 = 0xffffffffu;
+        if (lane < na) { const u32 b = scr[64 + lane]; key0 = (((u32)__ldcg(&rec[b]) - t0) << 6) | b; }
+        if (lane + 32 < na) { const u32 b = scr[96 + lane]; key1 = (((u32)__ldcg(&rec[b]) - t0) << 6) | b; }
+        u32 r0 = 0, r1 = 0;
+        if (na > 32) {
+#pragma unroll
+            for (u32 j = 0; j < 32; j++) {
+                const u32 k0 = __shfl_sync(FULL, key0, j), k1 = __shfl_sync(FULL, key1, j);
+                r0 += (k0 < key0) + (k1 < key0); r1 += (k0 < key1) + (k1 < key1);
+            }
+        } else if (na > 1) {
+#pragma unroll
+            for (u32 j = 0; j < 32; j++) r0 += __shfl_sync(FULL, key0, j) < key0;
+        }
+        if (lane < na) scr[r0] = key0;
+        if (lane + 32 < na) scr[r1] = key1;
+        __syncwarp();
+    }
+    const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
+    const u32 wlen = t1 - t0;
+    u32 idx = 0, xp = 0, last_issue = 0xffffffffu;              // xp: earliest cycle (relative to t0) of the next issue
+    u32 im_lo = 0, im_hi = 0;                                   // slots taken by this lane's issues
+    bool stop = false;
+    while (!stop) {
+        if (rem == ASTRA_NOTLOADED) {
+            bool got = false;
+            while (cur < end) {
+                const u32 s2 = cul[cur];
+                const u32 tr = t_release[s2];
+                if (tr >= t1) break;
+                if (tr > t0 + xp) xp = tr - t0;
+                const u32 q = c.step_q[s2] + (((wf - c.cu_lo[s2] * c.Wv) < c.step_r[s2]) ? 1u : 0u);   // R11
+                if (q) { rem = q; got = true; break; }
+                cur++;
+            }
+            if (!got) break;
+        }
+        const u32 s = cul[cur];
+        const u32 ox = c.first_link[s] - e0;
+        while (rem > 0) {
+            const u32 i = idx + lane;
+            const u32 want_n = min(32u, rem);
+            const bool cand = lane < want_n && i < F0 + na;
+            const u32 key = (cand && i >= F0) ? scr[i - F0] : 0u;
+            const int val = cand ? (int)(key >> 6) - (int)lane : INT_MIN;
+            const int y = max(warp_incl_max(val, lane), (int)xp);
+            const u32 x = lane + (u32)y;
+            const bool valid = cand && x < wlen;
+            const u32 nv = __popc(__ballot_sync(FULL, valid));
+            if (valid) {
+                const u32 slot = i < F0 ? scr[128 + i] : (key & 63u);
+                if (slot < 32) im_lo |= 1u << slot; else im_hi |= 1u << (slot - 32);
+                const u32 p = atomicAdd(&cnt[x], 1u);
+                if (p < H) evb[(size_t)x * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(x + 1) << ASTRA_FLIT_TIME_SHIFT);
+                if (deg > 1) atomicAdd(&h[ox * W + x], 1u);
+            }
+            if (nv) {
+                last_issue = __shfl_sync(FULL, x, nv - 1);
+                xp = last_issue + 1; idx += nv; rem -= nv;
+            }
+            if (nv < want_n) { stop = true; break; }            // out of slots or out of window
+        }
+        if (!stop && rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
+    }
+    im_lo = __reduce_or_sync(FULL, im_lo); im_hi = __reduce_or_sync(FULL, im_hi);
+    if (lane == 0) {
+        const u64 nbusy = (busy & ~rb) | (((u64)im_hi << 32) | im_lo);
+        c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = nbusy;
+        const bool wantb = rem != ASTRA_NOTLOADED, freebit = nbusy != fullmask;
+        u32* want = c.want + (size_t)g * nwords + (wf >> 5);
+        u32* freeb = c.freeb + (size_t)g * nwords + (wf >> 5);
+        const u32 bit = 1u << (wf & 31);
+        if (wantb) atomicOr(want, bit); else atomicAnd(want, ~bit);
+        if (freebit) atomicOr(freeb, bit); else atomicAnd(freeb, ~bit);
+        if ((wantb && freebit) || last_issue == wlen - 1) atomicMin(&ctl.next_hint, t1);
+    }
+    __syncwarp();
 }
 
 // The budget bound: put the wavefronts of GPU g back to their state at the window start.
@@ -1412,6 +1550,12 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                 for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim(c, ctl, g, wi, k, t0, t1, lane);
             }
             __syncthreads();
+            for (u32 g = c.g_lo; g < c.g_hi; g++) {
+                if (c.gmode[g] != 1u) continue;
+                const u32 nh = c.nheavy[g];
+                for (u32 j = (warp + nwarps - g % nwarps) % nwarps; j < nh; j += nwarps) wf_heavy(c, ctl, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
+            }
+            __syncthreads();
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[9] += (u64)(ck - ck1); ck1 = ck; }
             for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) {
                 if (c.gmode[g] == 1u) gpu_check(c, ctl, g, k, wlen, lane);
@@ -1462,6 +1606,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                     ctl.acked = 0;
                 }
                 bar_target += group; group_barrier(gc, bar_target);
+                if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[13] += (u64)(ck - ck0); ck0 = ck; }
                 if (tid == 0) {
                     ctl.next_hint = *(volatile u32*)&gc->hint[seq % 3];
                     ctl.acked_total = *(volatile u32*)&gc->acked;
@@ -1508,6 +1653,8 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             sm.completion_cycle = ctl.completion; sm.total_lines = P.total_lines;
             sm.busy_cycles = busy; sm.skipped_cycles = skipped;
             *c.r_summary = sm;
+        }
+        if (tid == 0 && rank == min(group - 1, (c.flags >> 16) & 0xfu)) {     // diagnostics of one CTA of the group
             for (int i = 0; i < 16; i++) c.r_diag[i] = ctl.clk[i];
         }
     }

@@ -26,6 +26,8 @@ typedef uint64_t u64;
 #define ASTRA_NONE32 0xffffffffu
 #define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles
 #define ASTRA_NW_MAX 256                  // ack window bins per GPU
+#define ASTRA_HEAVY_MIN 8u                // possible issues in a window from which a wavefront gets a warp of its own
+#define ASTRA_HEAVY_MAX_PER_WORD 16        // more such wavefronts among 32 consecutive ones: they stay on their threads
 #define ASTRA_LF_DELIVER_ONLY 1u           // lflag: every line over the link terminates at its head
 #define ASTRA_LF_FORWARD_ONLY 2u           // lflag: every line over the link goes on to the single-feeder link lfwd[e]
 #define ASTRA_GF_ISSUED_DEPS 1u            // gflag: some step of the GPU has an ISSUED-kind successor
@@ -50,11 +52,11 @@ typedef uint64_t u64;
 #define ASTRA_WS_ARRAYS(X) \
     X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
     X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(due_cnt, u32, 0) X(tl_lo, u32, 3) X(tl_n, u32, 3) X(tl_base, u32, 3) X(tbase, u32, 3) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
-    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
-    X(undo_busy, u64, 3) X(undo_rem, u32, 3) X(undo_cur, u32, 3) X(undo_want, u32, 3) X(undo_freeb, u32, 3) \
+    X(hlist, u32, 3) X(undo_busy, u64, 3) X(undo_rem, u32, 3) X(undo_cur, u32, 3) X(undo_want, u32, 3) X(undo_freeb, u32, 3) \
     X(bitmap, u32, 0) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
 
 enum AstraConstId {

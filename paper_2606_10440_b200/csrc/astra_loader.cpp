@@ -299,14 +299,26 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
 
     // node ranges of the CTAs of the group: contiguous, balanced by the lines each node handles
     std::vector<u32> part(group + 1, V);
-    {
-        part[0] = 0;
-        double total = 0; for (u32 v = 0; v < V; v++) total += load[v] + 1.0;
-        double acc = 0; u32 j = 1;
-        for (u32 v = 0; v < V && j < group; v++) {
-            acc += load[v] + 1.0;
-            while (j < group && acc >= total * j / group) part[j++] = v + 1;
-        }
+    if (group >= V) {
+        for (u32 j = 0; j <= group; j++) part[j] = std::min(j, V);     // one node per CTA
+    } else {
+        // contiguous ranges; the smallest bottleneck load is found by bisection over a greedy fill
+        std::vector<double> w(V);
+        double total = 0, wmax = 0;
+        for (u32 v = 0; v < V; v++) { w[v] = load[v] + 1.0; total += w[v]; wmax = std::max(wmax, w[v]); }
+        double lo = std::max(wmax, total / group), hi = total;
+        auto fill = [&](double cap, std::vector<u32>* out) {
+            u32 j = 1; double acc = 0;
+            if (out) (*out)[0] = 0;
+            for (u32 v = 0; v < V; v++) {
+                if (acc + w[v] > cap && acc > 0) { if (j >= group) return false; if (out) (*out)[j] = v; j++; acc = 0; }
+                acc += w[v];
+            }
+            if (out) for (; j <= group; j++) (*out)[j] = V;
+            return true;
+        };
+        for (int it = 0; it < 50; it++) { double mid = 0.5 * (lo + hi); if (fill(mid, nullptr)) hi = mid; else lo = mid; }
+        fill(hi, &part);
         part[group] = V;
     }
 
@@ -355,7 +367,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_tbase] = 4ull * (E + 1);
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
     ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
-    ab[ASTRA_A_gmode] = 4ull * G;
+    ab[ASTRA_A_gmode] = ab[ASTRA_A_nheavy] = 4ull * G;
     ab[ASTRA_A_cnt] = 4ull * G * W;
     ab[ASTRA_A_undo_want] = ab[ASTRA_A_undo_freeb] = 4ull * G * P.nwords;
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
@@ -367,7 +379,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_ev_list] = 4ull * ev_off[G];
     ab[ASTRA_A_bin_cnt] = 4ull * G * P.NW;
     ab[ASTRA_A_wf_busy] = ab[ASTRA_A_undo_busy] = 8ull * GW;
-    ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = 4ull * GW;
+    ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = ab[ASTRA_A_hlist] = 4ull * GW;
     ab[ASTRA_A_bitmap] = 4ull * G * P.NW * P.bmwords;
     ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
     ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
