@@ -1303,6 +1303,62 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
     const u32 capq = c.ceilb[e] * 256u;
     u32 n_acc = 0, first_x = 0, last_x = 0;
 
+    if (kind != ASTRA_LK_GENERAL) {
+        // 128 entries per step, four consecutive ones per lane: local running max, then one warp scan
+        const int P = (int)param;
+        for (u32 base = 0; base < scan_limit; base += 128) {
+            const u32 j0 = base + 4 * lane;
+            u64 fl[4]; int val[4]; u32 xx[4]; bool act[4];
+#pragma unroll
+            for (int q = 0; q < 4; q++) { act[q] = j0 + q < scan_limit; fl[q] = act[q] ? ring[(fh + j0 + q) & rmask] : 0ull; }
+            int m = INT_MIN;
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const u32 j = j0 + q;
+                const int a = (act[q] && j >= n_back) ? (int)((u32)(fl[q] >> ASTRA_FLIT_TIME_SHIFT) & 0x3ffu) : 0;
+                const int v = kind == ASTRA_LK_INT ? P * a - (int)j : a - P * (int)j;
+                m = act[q] ? max(m, v) : m;
+                val[q] = m;                                  // running max inside the lane
+            }
+            // exclusive prefix max of the lane totals, seeded with the carried maximum
+            int incl = warp_incl_max(m, lane);
+            int excl = __shfl_up_sync(FULL, incl, 1);
+            if (lane == 0) excl = INT_MIN;
+            excl = max(excl, run_max);
+            run_max = max(run_max, __shfl_sync(FULL, incl, 31));
+            u32 cnt_acc = 0, cnt_act = 0, xmax = 0;
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const u32 j = j0 + q;
+                const int pm = max(excl, val[q]);
+                xx[q] = kind == ASTRA_LK_INT ? (u32)((int)j + pm) / param : (u32)(P * (int)j + max(pm, xn_rel));
+                const bool acc = act[q] && xx[q] < wlen;
+                cnt_act += act[q]; cnt_acc += acc;
+                if (acc) {
+                    xmax = xx[q];
+                    ring[(fh + j) & rmask] = (fl[q] & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + xx[q] + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
+                } else xx[q] = 0xffffffffu;
+            }
+            const u32 tot_acc = __reduce_add_sync(FULL, cnt_acc), tot_act = __reduce_add_sync(FULL, cnt_act);
+            if (tot_acc) {
+                const u32 x_first = __shfl_sync(FULL, xx[0], 0);   // acceptance is a prefix: entry `base` is the first
+                if (n_acc == 0) first_x = x_first;
+                last_x = __reduce_max_sync(FULL, xmax);
+                n_acc += tot_acc;
+                // arrivals of one step fall in at most two lookahead windows
+                const u32 w_first = (t0 + x_first + leff) >> c.logW;
+                u32 c0 = 0;
+#pragma unroll
+                for (int q = 0; q < 4; q++) c0 += (xx[q] != 0xffffffffu) && ((t0 + xx[q] + leff) >> c.logW) == w_first;
+                c0 = __reduce_add_sync(FULL, c0);
+                if (lane == 0) {
+                    atomicAdd(&c.due_cnt[(size_t)e * c.NW + (w_first & c.NWmask)], c0);
+                    if (tot_acc != c0) atomicAdd(&c.due_cnt[(size_t)e * c.NW + ((w_first + 1) & c.NWmask)], tot_acc - c0);
+                }
+            }
+            if (tot_acc != tot_act) break;                   // FIFO: nothing behind a waiting line is accepted
+        }
+    } else {
     // ring loads run two chunks ahead of the scan
     u64 fq0 = lane < scan_limit ? ring[(fh + lane) & rmask] : 0ull;
     u64 fq1 = 32 + lane < scan_limit ? ring[(fh + 32 + lane) & rmask] : 0ull;
@@ -1369,6 +1425,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
             }
         }
         if (accm != actm) break;                             // FIFO: nothing behind a waiting line is accepted
+    }
     }
     if (lane == 0) {
         c.fifo_head[e] = fh + n_acc;
