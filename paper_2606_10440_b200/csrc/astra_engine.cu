@@ -321,11 +321,13 @@ __device__ void stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
             nch = (n + 31) / 32;
             c.tl_lo[e] = lo; c.tl_n[e] = n; c.pipe_head[e] = lo + n;
             if (fl == ASTRA_LF_FORWARD_ONLY) { const u32 o = c.lfwd[e]; c.tl_base[e] = c.run[o]; c.run[o] += n; }
+            else if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;          // set by a chunk that marks a cell: pass 3 needed
         }
         if (hi != lo + n) {                                     // in flight beyond this window: next arrival (A7)
             const u64 flit = __ldcg(&c.ring[c.ring_off[e] + ((lo + n) & c.ring_mask[e])]);
             atomicMin(&ctl.next_hint, t0 + (((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26));
         }
+        else if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;
         if (hi - lo > c.ring_mask[e] + 1) atomicOr(&ctl.err, 1u);
     } else if (hi != lo) nch = 1;
     c.tbase[i] = nch;
@@ -361,7 +363,9 @@ __device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32
     if (total == 0) return;
     const u32 K = c.K, kmagic = c.kmagic;
     const u32* lines = c.lines;
-    u32 acked_steps = 0, tmax = 0;
+    u32 tmax = 0;
+    // per-lane caches: consecutive acks of a lane mostly belong to one step and one amask word
+    u32 cs = 0xffffffffu, cc = 0, cm = 0, aw = 0xffffffffu, ab = 0;
     for (u32 base = 0; base < total; base += CAP) {
         {
             u32 pos = excl, ww = w;
@@ -381,38 +385,45 @@ __device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32
             for (int q = 0; q < 4; q++) rc[q] = idx[q] != 0xffffffffu ? __ldcg(&rec[idx[q]]) : 0ull;
 #pragma unroll
             for (int q = 0; q < 4; q++) {
-                const bool act = idx[q] != 0xffffffffu;
-                const u32 amk = __ballot_sync(FULL, act);
-                bool completed = false;
-                if (act) {
-                    const u32 ta = (u32)rc[q];
-                    const u32 step = ta < t1 ? (u32)(rc[q] >> 32) : 0xffffffffu;   // beyond the watchdog cut: not processed
-                    const u32 wf = K == 1 ? idx[q] : (u32)(((u64)idx[q] * kmagic) >> 32);   // idx / K
-                    atomicOr(&am[wf >> 5], 1u << (wf & 31));
-                    const u32 m = __match_any_sync(amk, step);
-                    const u32 cmax = __reduce_max_sync(m, ta);
-                    if (step != 0xffffffffu) tmax = max(tmax, ta);
-                    if ((m & lanemask_lt()) == 0 && step != 0xffffffffu) {
-                        atomicMax(&c.t_ack[step], cmax);
-                        const u32 cntm = __popc(m);
-                        const u32 old = atomicAdd(&c.ack_cnt[step], cntm);
-                        if (old + cntm == lines[step]) {
-                            completed = true;
-                            const u32 pos2 = atomicAdd(&c.ev_cnt[g], 1u);
-                            c.ev_list[c.ev_off[g] + pos2] = step | ((u32)ASTRA_DEP_ACKED << 30);
+                if (idx[q] == 0xffffffffu) continue;
+                const u32 ta = (u32)rc[q];
+                const u32 wf = K == 1 ? idx[q] : (u32)(((u64)idx[q] * kmagic) >> 32);   // idx / K
+                if ((wf >> 5) != aw) { if (ab) atomicOr(&am[aw], ab); aw = wf >> 5; ab = 0; }
+                ab |= 1u << (wf & 31);
+                if (ta >= t1) continue;                          // beyond the watchdog cut: not processed
+                const u32 step = (u32)(rc[q] >> 32);
+                tmax = max(tmax, ta);
+                if (step != cs) {
+                    if (cc) {                                    // flush the cached step
+                        atomicMax(&c.t_ack[cs], cm);
+                        if (atomicAdd(&c.ack_cnt[cs], cc) + cc == lines[cs]) {
+                            c.ev_list[c.ev_off[g] + atomicAdd(&c.ev_cnt[g], 1u)] = cs | ((u32)ASTRA_DEP_ACKED << 30);
+                            atomicAdd(&ctl.acked, 1u);
                         }
                     }
+                    cs = step; cc = 0; cm = 0;
                 }
-                acked_steps += __popc(__ballot_sync(FULL, completed));
+                cc++; cm = max(cm, ta);
             }
         }
         __syncwarp();
     }
-    tmax = __reduce_max_sync(FULL, tmax);
-    if (lane == 0) {
-        if (acked_steps) atomicAdd(&ctl.acked, acked_steps);
-        if (tmax) atomicMax(&ctl.completion, tmax);
+    if (ab) atomicOr(&am[aw], ab);
+    // final flush, aggregated over the lanes that hold the same step
+    {
+        const u32 key = cc ? cs : 0xffffffffu;
+        const u32 m = __match_any_sync(FULL, key);
+        const u32 csum = __reduce_add_sync(m, cc), cmax = __reduce_max_sync(m, cm);
+        if (cc && (m & lanemask_lt()) == 0) {
+            atomicMax(&c.t_ack[cs], cmax);
+            if (atomicAdd(&c.ack_cnt[cs], csum) + csum == lines[cs]) {
+                c.ev_list[c.ev_off[g] + atomicAdd(&c.ev_cnt[g], 1u)] = cs | ((u32)ASTRA_DEP_ACKED << 30);
+                atomicAdd(&ctl.acked, 1u);
+            }
+        }
     }
+    tmax = __reduce_max_sync(FULL, tmax);
+    if (lane == 0 && tmax) atomicMax(&ctl.completion, tmax);
 }
 
 // 32 pipe entries of a link whose lines all terminate at its head GPU (R7 A1, deliveries)
@@ -455,6 +466,82 @@ __device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wl
         }
         hint = __reduce_min_sync(amk, hint);
         if ((amk & lanemask_lt()) == 0) atomicMin(&ctl.next_hint, hint);
+    }
+}
+
+// 32 pipe entries of a link whose lines terminate at its head or go on to multi-feeder links (R7 A1).
+// A line's cell slot is (in-link's slot base + its rank among the lines this link delivers in the
+// same cycle); lines of one cycle are consecutive in the stream, so the rank is a look at the
+// neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
+// PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
+template <int PASS>
+__device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wlen, u32 cb, u32 lane) {
+    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+    const u32 i0 = lo + chunk * 32, ii = i0 + lane;
+    const u64* ring = c.ring + c.ring_off[e];
+    const u32 rmask = c.ring_mask[e];
+    bool valid = (int32_t)(lo + n - ii) > 0;
+    u64 flit = 0; u32 d = 0xffffffffu;
+    if (valid) {
+        flit = __ldcg(&ring[ii & rmask]);
+        d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
+        valid = d < wlen;                                     // watchdog cut inside the window
+    }
+    // rank among the same-cycle lines of this link
+    const u32 d0 = __shfl_sync(FULL, d, 0);
+    u32 back = 0;
+    {
+        const u32 nb = c.ceilb[e] - 1;                        // at most ceil(B) lines per cycle
+        bool same = false;
+        if (lane < nb && (int32_t)(i0 - 1 - lane - lo) >= 0) {
+            const u64 f2 = __ldcg(&ring[(i0 - 1 - lane) & rmask]);
+            same = (((u32)(f2 >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) == d0;
+        }
+        back = __popc(__ballot_sync(FULL, same));
+    }
+    const u32 vmask = __ballot_sync(FULL, valid);
+    if (!valid) return;
+    const u32 grp = __match_any_sync(vmask, d);
+    const u32 r = __popc(grp & lanemask_lt()) + (d == d0 ? back : 0u);
+    const u32 v = c.head[e];
+    const u32 step = (u32)flit & 0xfffffu;
+    const u32 od = c.step_od[step];
+    const u32 dstg = od & 0xffffu;
+    const bool deliver = dstg == v;
+    if (!deliver) {
+        const u32 o = c.next_link[(size_t)v * c.G + dstg];
+        if (PASS == 1) { cell_set(c, ctl, o, v, cb, d, c.classoff[e] + r); c.tl_base[e] = 1u; }
+        else {
+            const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, c.classoff[e] + r);
+            c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+        }
+    }
+    if (PASS == 1) {
+        const u32 dmask = __ballot_sync(vmask, deliver);
+        if (deliver) {
+            const u32 owner = od >> 16;
+            const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
+            const u32 ta = t0 + d + c.step_alpha[step];                       // R6
+            const u32 bit = wf * c.K + slot;
+            c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
+            const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+            atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
+            const u32 mb = __match_any_sync(dmask, bin);
+            if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+            const u32 m = __match_any_sync(dmask, step);
+            const u32 dmax = __reduce_max_sync(m, d);
+            if ((m & lanemask_lt()) == 0) {
+                atomicMax(&c.t_deliv[step], t0 + dmax);
+                const u32 cntm = __popc(m);
+                const u32 old = atomicAdd(&c.deliv_cnt[step], cntm);
+                if (old + cntm == c.lines[step]) {
+                    const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
+                    c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
+                }
+            }
+            const u32 hint = __reduce_min_sync(dmask, ta);
+            if ((dmask & lanemask_lt()) == 0) atomicMin(&ctl.next_hint, hint);
+        }
     }
 }
 
@@ -1591,6 +1678,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                     const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
                     if (fl == ASTRA_LF_DELIVER_ONLY) deliver_chunk(c, ctl, e, ch, t0, wlen, lane);
                     else if (fl == ASTRA_LF_FORWARD_ONLY) forward_chunk(c, e, ch, t0, wlen, lane);
+                    else if (fl == ASTRA_LF_CELLS) cells_chunk<1>(c, ctl, e, ch, t0, wlen, cb, lane);
                     else arrivals_link<1>(c, ctl, i, t0, wlen, cb, lane);
                 }
             }
@@ -1644,6 +1732,15 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                     for (u32 task = warp; task < ng + ns; task += nwarps) {
                         if (task < ng) inject_place(c, c.g_lo + task, wlen, cb, lane);
                         else arrivals_link<3>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
+                    }
+                    // chunked links that marked cells: same chunks again, now with the FIFO positions known
+                    const u32 ntl = ctl.ntasks;
+                    for (u32 task = nwarps - 1 - warp; task < ntl; task += nwarps) {
+                        u32 lo = c.i_lo, hi = c.i_hi;
+                        while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (c.tbase[mid] > task) hi = mid; else lo = mid + 1; }
+                        const u32 i = lo - 1, e = c.in_link[i];
+                        if (c.lflag[e] == ASTRA_LF_CELLS && !(c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) && c.tl_base[e])
+                            cells_chunk<3>(c, ctl, e, task - c.tbase[i], t0, wlen, cb, lane);
                     }
                 }
                 __syncthreads();

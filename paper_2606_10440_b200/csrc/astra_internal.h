@@ -30,6 +30,7 @@ typedef uint64_t u64;
 #define ASTRA_HEAVY_MAX_PER_WORD 16        // more such wavefronts among 32 consecutive ones: they stay on their threads
 #define ASTRA_LF_DELIVER_ONLY 1u           // lflag: every line over the link terminates at its head
 #define ASTRA_LF_FORWARD_ONLY 2u           // lflag: every line over the link goes on to the single-feeder link lfwd[e]
+#define ASTRA_LF_CELLS 3u                  // lflag: lines terminate at the head or go on to multi-feeder links only (cells)
 #define ASTRA_GF_ISSUED_DEPS 1u            // gflag: some step of the GPU has an ISSUED-kind successor
 
 // Link service kinds (R9): how the acceptance times of a FIFO are computed for a whole window.

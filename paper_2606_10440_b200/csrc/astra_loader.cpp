@@ -322,12 +322,24 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         part[group] = V;
     }
 
+    // all_merged[e]: every link that lines arriving over e are forwarded to has several feeders
+    std::vector<uint8_t> all_merged(E, 1);
+    for (u32 s = 0; s < S; s++) {
+        u32 v = c.owner[s], d = c.dst[s];
+        while (v != d) {
+            u32 e = t.next_link[(size_t)v * G + d];
+            u32 h = t.head[e];
+            if (h != d && !multi[t.next_link[(size_t)h * G + d]]) all_merged[e] = 0;
+            v = h;
+        }
+    }
     // per-link flags for the chunk-parallel arrival paths: every line over e terminates at head(e), or
     // every line over e is forwarded to the same single-feeder out-link
     std::vector<u32> lflag(E, 0), lfwd(E, 0);
     for (u32 e = 0; e < E; e++) {
         if (delivers[e] && !transits[e]) lflag[e] = ASTRA_LF_DELIVER_ONLY;
         else if (transits[e] && !delivers[e] && !multi_fwd[e] && !multi[fwd[e]]) { lflag[e] = ASTRA_LF_FORWARD_ONLY; lfwd[e] = fwd[e]; }
+        else if (transits[e] && all_merged[e]) lflag[e] = ASTRA_LF_CELLS;
     }
     // per-GPU flags: a GPU whose steps have ISSUED-kind successors always takes the cycle-serial issue path
     std::vector<u32> gflag(G, 0);
