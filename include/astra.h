@@ -67,6 +67,7 @@ extern "C" {
 #define ASTRA_FLAG_WINDOW_1       2ull   /* force a 1-cycle lookahead window (testing I8)      */
 #define ASTRA_FLAG_SERIAL_ISSUE   4ull   /* always take the cycle-serial issue path (testing)  */
 #define ASTRA_FLAG_NO_HEAVY        16ull  /* no warp-per-wavefront issue path (testing)         */
+#define ASTRA_FLAG_NO_PRIORITY_SWEEP 32ull /* budget-bound windows take the cycle-serial path (testing) */
 #define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
 #define ASTRA_FLAG_DIAG_RANK(r) (((uint64_t)(r) & 0xfull) << 16) /* which CTA of a group reports astra_read_diag */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g

@@ -1193,18 +1193,152 @@ __device__ void wf_restore(Ctx& c, u32 g, u32 lane) {
     __syncwarp();
 }
 
+// The budget binds in this GPU-window: exact fixed-priority grants (R12), word by word in ascending
+// wavefront id.  A wavefront is granted at cycle t iff it is ready and fewer than H wavefronts with a
+// lower id are granted at t; occ[t] (the cnt array) holds the grants of all lower words, so the 32
+// wavefronts of a word step together through the cycles where one of them is ready and occ[t] < H,
+// a ballot giving the rank inside the word.  That rank is the bucket position of the issue.
+__device__ void wf_priority_word(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+    const u32 nwords = c.nwords;
+    const u32 am = c.amask[(size_t)g * nwords + wi];
+    if (am == 0) return;
+    const bool active = (am >> lane) & 1u;
+    const u32 wf = wi * 32 + lane;
+    const u32 W = c.W, H = c.H, K = c.K, wlen = t1 - t0;
+    const u64 fullmask = c.fullmask;
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    u32* const occ = c.cnt + (size_t)g * W;
+    u32* const h = c.hist + (size_t)e0 * W;
+    u64* const evb = c.evb + (size_t)g * H * W;
+    const u32* const t_release = c.t_release;
+    const u32* const cul = c.cul;
+    const size_t gw = (size_t)g * c.CW + wf;
+    u32 cur = 0, rem = ASTRA_NOTLOADED, end = 0;
+    u64 busy = fullmask;
+    u32 aq[64];
+    u32 na = 0, ai = 0;
+    if (active) {
+        cur = c.wf_cur[gw]; rem = c.wf_rem[gw]; busy = c.wf_busy[gw];
+        end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
+        const u32 b0 = wf * K, w0 = b0 >> 5, sh = b0 & 31;
+        u64 rb = 0;
+        if (c.ack_n[g]) {
+            const u32 bmwords = c.bmwords;
+            const u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * bmwords;
+            const u32 x0 = __ldcg(&bm[w0]);
+            const u32 x1 = (w0 + 1 < bmwords) ? __ldcg(&bm[w0 + 1]) : 0u;
+            const u32 x2 = (sh && w0 + 2 < bmwords) ? __ldcg(&bm[w0 + 2]) : 0u;
+            rb = ((((u64)x1 << 32) | x0) >> sh);
+            if (sh) rb |= (u64)x2 << (64 - sh);
+            rb &= fullmask;
+        }
+        const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
+        while (rb) { const u32 b = __ffsll((long long)rb) - 1; rb &= rb - 1; aq[na++] = (((u32)__ldcg(&rec[b]) - t0) << 6) | b; }
+        for (u32 i = 1; i < na; i++) {
+            const u32 xv = aq[i]; u32 j = i;
+            while (j > 0 && aq[j - 1] > xv) { aq[j] = aq[j - 1]; j--; }
+            aq[j] = xv;
+        }
+    }
+    u32 nq = na ? aq[0] : 0xffffffffu;
+    u32 s = 0, ox = 0, last_issue = 0xffffffffu;
+    bool have_s = false;
+    u32 T = 0;
+    for (;;) {
+        // bring the lane to cycle T: slots returned by T, step loaded if released by T
+        u32 np = 0xffffffffu;                                   // earliest cycle this lane can be ready
+        if (active) {
+            while ((nq >> 6) <= T) { busy &= ~(1ull << (nq & 63u)); ai++; nq = ai < na ? aq[ai] : 0xffffffffu; }
+            if (rem == ASTRA_NOTLOADED) {
+                while (cur < end) {
+                    const u32 s2 = cul[cur];
+                    const u32 tr = t_release[s2];
+                    if (tr >= t1) break;
+                    if (tr > t0 + T) { np = tr - t0; break; }
+                    const u32 q = c.step_q[s2] + (((wf - c.cu_lo[s2] * c.Wv) < c.step_r[s2]) ? 1u : 0u);   // R11
+                    if (q) { rem = q; have_s = false; break; }
+                    cur++;
+                }
+            }
+            if (rem != ASTRA_NOTLOADED) np = busy != fullmask ? T : (ai < na ? (nq >> 6) : 0xffffffffu);
+        }
+        const u32 tmin = __reduce_min_sync(FULL, np);
+        if (tmin >= wlen) break;
+        if (tmin > T) { T = tmin; continue; }
+        const u32 o = occ[T];
+        if (o >= H) {                                           // cycle taken by lower ids: next cycle with room
+            u32 t2 = T + 1;
+            for (;;) {
+                const bool room = t2 + lane < wlen && occ[t2 + lane] < H;
+                const u32 rm2 = __ballot_sync(FULL, room);
+                if (rm2) { t2 += __ffs(rm2) - 1; break; }
+                t2 += 32;
+                if (t2 >= wlen) break;
+            }
+            if (t2 >= wlen) break;
+            T = t2; continue;
+        }
+        const bool ready = active && rem != ASTRA_NOTLOADED && busy != fullmask;
+        const u32 rm = __ballot_sync(FULL, ready);
+        const u32 rank = o + __popc(rm & lanemask_lt());
+        const bool granted = ready && rank < H;
+        if (granted) {
+            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; have_s = true; }
+            const u32 slot = __ffsll((long long)~busy) - 1;
+            busy |= 1ull << slot;
+            evb[(size_t)T * H + rank] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(T + 1) << ASTRA_FLIT_TIME_SHIFT);
+            if (deg > 1) atomicAdd(&h[ox * W + T], 1u);
+            last_issue = T;
+            if (--rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
+        }
+        __syncwarp();
+        if (lane == 0) occ[T] = min(H, o + (u32)__popc(rm));
+        __syncwarp();
+        T++;
+        if (T >= wlen) break;
+    }
+    bool wantb = false, freebit = false, hint = false;
+    if (active) {
+        for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));
+        if (rem == ASTRA_NOTLOADED) {                           // a step released by the end of the window is loaded (as in wf_sim)
+            while (cur < end) {
+                const u32 s2 = cul[cur];
+                if (t_release[s2] >= t1) break;
+                const u32 q = c.step_q[s2] + (((wf - c.cu_lo[s2] * c.Wv) < c.step_r[s2]) ? 1u : 0u);
+                if (q) { rem = q; break; }
+                cur++;
+            }
+        }
+        c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
+        wantb = rem != ASTRA_NOTLOADED; freebit = busy != fullmask;
+        hint = (wantb && freebit) || last_issue == wlen - 1;
+    }
+    __syncwarp();
+    const u32 wm = __ballot_sync(FULL, wantb), fm = __ballot_sync(FULL, freebit);
+    const bool anyh = __any_sync(FULL, hint);
+    if (lane == 0) {
+        u32* want = c.want + (size_t)g * nwords + wi;
+        u32* freeb = c.freeb + (size_t)g * nwords + wi;
+        *want = (*want & ~am) | wm;
+        *freeb = (*freeb & ~am) | fm;
+        if (anyh) atomicMin(&ctl.next_hint, t1);
+    }
+    __syncwarp();
+}
+
 // stage 2c: did the HBM budget bind in any cycle (R12)?  If not, the run stands: exclusive prefix of
 // the per-cycle counts (item enumeration), FIFO positions of every (direct out-link, cycle), new
 // tails, and the window's ack bits / released steps are consumed.
-__device__ void gpu_check(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
-    const u32 W = c.W;
-    u32* cnt = c.cnt + (size_t)g * W;
+__device__ bool gpu_binds(Ctx& c, u32 g, u32 wlen, u32 lane) {
+    const u32* cnt = c.cnt + (size_t)g * c.W;
     bool bind = false;
     for (u32 tt = lane; tt < wlen; tt += 32) if (cnt[tt] > c.H) bind = true;
-    if (__any_sync(FULL, bind)) {
-        if (lane == 0) c.gmode[g] = 2u;
-        return;
-    }
+    return __any_sync(FULL, bind);
+}
+
+__device__ void gpu_finalize(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
+    const u32 W = c.W;
+    u32* cnt = c.cnt + (size_t)g * W;
     u32 carry = 0;
     for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
@@ -1703,10 +1837,23 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             __syncthreads();
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[9] += (u64)(ck - ck1); ck1 = ck; }
             for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) {
-                if (c.gmode[g] == 1u) gpu_check(c, ctl, g, k, wlen, lane);
+                if (c.gmode[g] == 1u) {
+                    if (!gpu_binds(c, g, wlen, lane)) { gpu_finalize(c, ctl, g, k, wlen, lane); continue; }
+                    // the budget binds: back to the window start, then exact grants
+                    if (lane == 0) atomicAdd((unsigned long long*)&ctl.clk[6], 1ull);
+                    wf_restore(c, g, lane);
+                    if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
+                    else {
+                        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+                        for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
+                        if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e0 * c.W + i] = 0;
+                        __syncwarp();
+                        for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, g, wi, k, t0, t1, lane);
+                        gpu_finalize(c, ctl, g, k, wlen, lane);
+                        continue;
+                    }
+                }
                 if (c.gmode[g] != 2u) continue;                  // cycle-serial path
-                if (lane == 0) atomicAdd((unsigned long long*)&ctl.clk[6], 1ull);
-                if (!((c.gflag[g] & ASTRA_GF_ISSUED_DEPS) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE))) wf_restore(c, g, lane);
                 ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
                 issue_window(c, ctl, g, t0, t1, cb, lane);
                 for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
