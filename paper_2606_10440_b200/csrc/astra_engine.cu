@@ -38,7 +38,7 @@
 #define SCR_WORDS ((1u << ASTRA_WMAX_LOG2) + 64)   // per-warp scratch words
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
-    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, logW, W, NC, NWmask, NW, kmagic, tmax, flags;
+    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, W, NC, NWmask, NW, kmagic, tmax, flags;
     u32 group, rank, v_lo, v_hi, g_lo, g_hi, e_lo, e_hi, i_lo, i_hi;
     u64 fullmask;
 #define X(n) const u32* n;
@@ -121,7 +121,7 @@ __device__ __forceinline__ u32 cell_pos(Ctx& c, u32 o, u32 v, u32 cb, u32 d, u32
 // sums) writes the lines that go to multi-feeder out-links at their FIFO positions.
 // ---------------------------------------------------------------------------------------------
 template <int PASS>
-__device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 t0, u32 wlen, u32 cb, u32 lane) {
+__device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 e = c.in_link[i];
     const u32 lo = c.pipe_head[e];
     u32 hi;
@@ -188,7 +188,7 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 t0, u32 wlen, u32 cb,
                         const u32 ta = t0 + d + c.step_alpha[step];                       // R6
                         const u32 bit = wf * c.K + slot;
                         c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
-                        const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+                        const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
                         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
                         const u32 mb = __match_any_sync(dmask, bin);
                         if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
@@ -301,7 +301,7 @@ __device__ void stage1_setup_gpu(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 lane) {
     best = __reduce_min_sync(FULL, best);
     if (lane == 0) {
         if (best != ASTRA_T_INF) {
-            const u64 tw = (u64)(k + best) << c.logW;
+            const u64 tw = (u64)(k + best) * c.W;
             atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
         }
         c.ack_n[g] = ld_vol(&c.bin_cnt[g * c.NW + (k & c.NWmask)]);
@@ -427,7 +427,7 @@ __device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32
 }
 
 // 32 pipe entries of a link whose lines all terminate at its head GPU (R7 A1, deliveries)
-__device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
+__device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
     const u32 ii = lo + chunk * 32 + lane;
     bool valid = (int32_t)(lo + n - ii) > 0;
@@ -448,7 +448,7 @@ __device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wl
         const u32 ta = t0 + d + c.step_alpha[step];                       // R6
         const u32 bit = wf * c.K + slot;
         c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
-        const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+        const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
         const u32 mb = __match_any_sync(amk, bin);
         if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
@@ -475,7 +475,7 @@ __device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wl
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
 // PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
 template <int PASS>
-__device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wlen, u32 cb, u32 lane) {
+__device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
     const u32 i0 = lo + chunk * 32, ii = i0 + lane;
     const u64* ring = c.ring + c.ring_off[e];
@@ -524,7 +524,7 @@ __device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 t0, u32 wlen
             const u32 ta = t0 + d + c.step_alpha[step];                       // R6
             const u32 bit = wf * c.K + slot;
             c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
-            const u32 bin = owner * c.NW + ((ta >> c.logW) & c.NWmask);
+            const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
             atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
             const u32 mb = __match_any_sync(dmask, bin);
             if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
@@ -1483,7 +1483,7 @@ __device__ void inject_place(Ctx& c, u32 g, u32 wlen, u32 cb, u32 lane) {
 // ---------------------------------------------------------------------------------------------
 // stage 4: link e over [t0, t1): acceptance times of the whole FIFO (R9), arrival stamps.
 // ---------------------------------------------------------------------------------------------
-__device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 wlen = t1 - t0;
     const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
     if (c.dirty[e]) {                                        // consume the cells of the window
@@ -1512,6 +1512,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
     const u32 lk = c.lkind[e];
     const u32 kind = lk & 3u, param = lk >> 2;
     const u32 leff = c.leff[e];
+    const u32 lq = leff / c.W, lr = leff % c.W;             // arrival window = k + lq + (x + lr >= W)
     const u32 scan_limit = min(n_tot, c.ceilb[e] * wlen);
     // carried service state
     int run_max = INT_MIN;                                  // INT: prefix max of B*a - i ; PERIOD: of a - P*i
@@ -1567,10 +1568,10 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
                 last_x = __reduce_max_sync(FULL, xmax);
                 n_acc += tot_acc;
                 // arrivals of one step fall in at most two lookahead windows
-                const u32 w_first = (t0 + x_first + leff) >> c.logW;
+                const u32 w_first = k + lq + (x_first + lr >= c.W ? 1u : 0u);
                 u32 c0 = 0;
 #pragma unroll
-                for (int q = 0; q < 4; q++) c0 += (xx[q] != 0xffffffffu) && ((t0 + xx[q] + leff) >> c.logW) == w_first;
+                for (int q = 0; q < 4; q++) c0 += (xx[q] != 0xffffffffu) && (k + lq + (xx[q] + lr >= c.W ? 1u : 0u)) == w_first;
                 c0 = __reduce_add_sync(FULL, c0);
                 if (lane == 0) {
                     atomicAdd(&c.due_cnt[(size_t)e * c.NW + (w_first & c.NWmask)], c0);
@@ -1637,7 +1638,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
             // lines due at the head per lookahead window: stage 1 of that window reads the count
         }
         if (accm) {                                          // arrivals of a chunk fall in at most two windows
-            const u32 wa = (t0 + x + leff) >> c.logW;
+            const u32 wa = k + lq + (x + lr >= c.W ? 1u : 0u);
             const u32 w_first = __shfl_sync(FULL, wa, __ffs(accm) - 1);
             const u32 m0 = __ballot_sync(FULL, acc && wa == w_first);
             if (lane == 0) {
@@ -1664,7 +1665,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 t0, u32 t1, u32 cb, u3
 __device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8_t* ws, uint8_t* hot, uint8_t* rs, u32 rank) {
     c.G = P.G; c.V = P.V; c.E = P.E; c.S = P.S; c.C = P.C; c.Wv = P.Wv; c.K = P.K; c.H = P.H;
     c.CW = P.CW; c.nwords = P.nwords; c.slots = P.slots; c.bmwords = P.bmwords;
-    c.logW = P.logW; c.W = 1u << P.logW; c.NC = P.NC; c.NW = P.NW; c.NWmask = P.NW - 1; c.kmagic = P.kdiv_magic;
+    c.W = P.Wcyc; c.NC = P.NC; c.NW = P.NW; c.NWmask = P.NW - 1; c.kmagic = P.kdiv_magic;
     c.tmax = (u32)P.max_cycles; c.flags = P.flags;
     c.fullmask = P.K >= 64 ? ~0ull : ((1ull << P.K) - 1);
     c.group = P.group; c.rank = rank;
@@ -1784,7 +1785,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
         const u32 W = c.W;
         u64 busy = 0, skipped = 0;
         for (;;) {
-            const u64 t0l = (u64)k << c.logW;
+            const u64 t0l = (u64)k * c.W;
             if (t0l >= c.tmax) { status = ASTRA_STATUS_MAX_CYCLES; break; }
             const u32 t0 = (u32)t0l;
             const u32 t1 = (u32)min((u64)c.tmax, t0l + W);
@@ -1810,10 +1811,10 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                     const u32 i = lo - 1, ch = task - c.tbase[i];
                     const u32 e = c.in_link[i];
                     const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
-                    if (fl == ASTRA_LF_DELIVER_ONLY) deliver_chunk(c, ctl, e, ch, t0, wlen, lane);
+                    if (fl == ASTRA_LF_DELIVER_ONLY) deliver_chunk(c, ctl, e, ch, k, t0, wlen, lane);
                     else if (fl == ASTRA_LF_FORWARD_ONLY) forward_chunk(c, e, ch, t0, wlen, lane);
-                    else if (fl == ASTRA_LF_CELLS) cells_chunk<1>(c, ctl, e, ch, t0, wlen, cb, lane);
-                    else arrivals_link<1>(c, ctl, i, t0, wlen, cb, lane);
+                    else if (fl == ASTRA_LF_CELLS) cells_chunk<1>(c, ctl, e, ch, k, t0, wlen, cb, lane);
+                    else arrivals_link<1>(c, ctl, i, k, t0, wlen, cb, lane);
                 }
             }
             __syncthreads();
@@ -1878,7 +1879,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                     const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
                     for (u32 task = warp; task < ng + ns; task += nwarps) {
                         if (task < ng) inject_place(c, c.g_lo + task, wlen, cb, lane);
-                        else arrivals_link<3>(c, ctl, c.i_lo + task - ng, t0, wlen, cb, lane);
+                        else arrivals_link<3>(c, ctl, c.i_lo + task - ng, k, t0, wlen, cb, lane);
                     }
                     // chunked links that marked cells: same chunks again, now with the FIFO positions known
                     const u32 ntl = ctl.ntasks;
@@ -1887,14 +1888,14 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                         while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (c.tbase[mid] > task) hi = mid; else lo = mid + 1; }
                         const u32 i = lo - 1, e = c.in_link[i];
                         if (c.lflag[e] == ASTRA_LF_CELLS && !(c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) && c.tl_base[e])
-                            cells_chunk<3>(c, ctl, e, task - c.tbase[i], t0, wlen, cb, lane);
+                            cells_chunk<3>(c, ctl, e, task - c.tbase[i], k, t0, wlen, cb, lane);
                     }
                 }
                 __syncthreads();
             }
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[3] += (u64)(ck - ck0); ck0 = ck; }
             // stage 4: link service per out-link
-            for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps) link_service(c, ctl, e, t0, t1, cb, lane);
+            for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps) link_service(c, ctl, e, k, t0, t1, cb, lane);
             __syncthreads();
             if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[4] += (u64)(ck - ck0); ck0 = ck; }
             // stage 5: next non-idle window
@@ -1921,15 +1922,16 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                 u32 dec = 0, nk = k + 1;
                 if (ctl.acked_total == c.S) dec = 1 + ASTRA_STATUS_DONE;
                 else if (ctl.err) dec = 1 + ASTRA_STATUS_INTERNAL;
+                else if ((u64)(k + 1) * c.W >= c.tmax) dec = 1 + ASTRA_STATUS_MAX_CYCLES;   // events past the watchdog cut are not looked at
                 else if (hint == ASTRA_T_INF) dec = 1 + ASTRA_STATUS_DEADLOCK;
-                else if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint >> c.logW);
+                else if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint / c.W);
                 ctl.decision = dec; ctl.next_k = nk;
             }
             __syncthreads();
             seq++;
             const u32 dec = ctl.decision;
             if (dec) { status = (int32_t)dec - 1; break; }
-            skipped += (u64)(ctl.next_k - k - 1) << c.logW;
+            skipped += (u64)(ctl.next_k - k - 1) * c.W;
             k = ctl.next_k;
         }
         __syncthreads();

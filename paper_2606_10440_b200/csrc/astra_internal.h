@@ -42,7 +42,7 @@ typedef uint64_t u64;
 #define ASTRA_CONST_TABLES(X) \
     X(in_ptr) X(in_link) X(head) X(tail) X(leff) X(next_link) X(row_ptr) \
     X(step_od) X(lines) X(cu_lo) X(cu_n) X(succ_ptr) X(succ) X(ndeps) \
-    X(step_q) X(step_r) X(first_link) X(step_alpha) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
+    X(step_q) X(step_r) X(first_link) X(step_alpha) X(step_aq) X(step_ar) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
     X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(classoff) \
     X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(gflag) X(lflag) X(lfwd)
 
@@ -82,7 +82,7 @@ struct PointDesc {
     u32 G, V, E, S;
     u32 C, Wv, K, H;
     u32 CW, nwords, slots, bmwords;
-    u32 logW, NW, kdiv_magic, NC;              // NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
+    u32 Wcyc, NW, kdiv_magic, NC;              // Wcyc lookahead window in cycles; NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
     u32 flags, group;                          // group: CTAs cooperating on this point
     u32 hot_bytes, pad0;
     u64 max_cycles;

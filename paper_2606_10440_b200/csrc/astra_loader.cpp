@@ -174,22 +174,23 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     u64 tmax = std::min<u64>(opt.max_cycles, 0xffffffffull - (1u << 25));
     P.max_cycles = tmax;
 
-    // lookahead window: largest power of two <= min Leff, capped
-    u32 logW = 0;
+    // lookahead window: min Leff (any value, not only powers of two), capped
+    u32 W = 1;
     if (!(opt.flags & ASTRA_FLAG_WINDOW_1)) {
-        while ((2u << logW) <= t.min_leff && logW + 1 <= ASTRA_WMAX_LOG2) logW++;
+        W = std::max<u32>(1, std::min<u32>(t.min_leff, 1u << ASTRA_WMAX_LOG2));
+        if (W >= 64) W &= ~63u;                 // whole 32-entry chunks per link and window at the usual bandwidths
     }
-    P.logW = logW;
-    const u32 W = 1u << logW;
+    P.Wcyc = W;
     const u32 NC = W + 1;
     P.NC = NC;
 
-    std::vector<u32> step_q(S), step_r(S), first_link(S), step_alpha(S);
+    std::vector<u32> step_q(S), step_r(S), first_link(S), step_alpha(S), step_aq(S), step_ar(S);
     u32 alpha_max = 1;
     for (u32 s = 0; s < S; s++) {
         u32 a = t.dist[(size_t)c.owner[s] * G + c.dst[s]];
         if (a == 0xffffffffu) { err = "a step's owner has no route to its dst"; return ASTRA_EUNREACHABLE; }
         step_alpha[s] = a; alpha_max = std::max(alpha_max, a);
+        step_aq[s] = a / W; step_ar[s] = a % W;             // ack window = delivery window + aq + (d + ar >= W)
         first_link[s] = t.next_link[(size_t)c.owner[s] * G + c.dst[s]];
         u32 m = c.cu_n[s] * g.Wv;
         step_q[s] = c.lines[s] / m; step_r[s] = c.lines[s] % m;
@@ -357,6 +358,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_ndeps] = coll_off[6];
     co[ASTRA_C_step_q] = blob.add(step_q); co[ASTRA_C_step_r] = blob.add(step_r);
     co[ASTRA_C_first_link] = blob.add(first_link); co[ASTRA_C_step_alpha] = blob.add(step_alpha);
+    co[ASTRA_C_step_aq] = blob.add(step_aq); co[ASTRA_C_step_ar] = blob.add(step_ar);
     co[ASTRA_C_cul_ptr] = blob.add(cul_ptr); co[ASTRA_C_cul] = blob.add(cul);
     co[ASTRA_C_rel_off] = blob.add(rel_off); co[ASTRA_C_init_rel] = blob.add(init_rel);
     co[ASTRA_C_init_rel_cnt] = blob.add(init_rel_cnt); co[ASTRA_C_ev_off] = blob.add(ev_off);
