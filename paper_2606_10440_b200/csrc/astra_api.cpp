@@ -30,8 +30,8 @@ struct astra_ctx {
     PointDesc* d_points = nullptr;
     u32 *d_order = nullptr, *d_queue = nullptr;
     GroupCtl* d_groups = nullptr;
-    u64 const_bytes = 0, ws_stride = 0, ws_total = 0, results_bytes = 0;
-    u32 n_groups = 0, group = 1, warps = 0, hot_bytes = 0;
+    u64 const_bytes = 0, ws_big_stride = 0, ws_single_stride = 0, ws_single_off = 0, ws_total = 0, results_bytes = 0;
+    u32 n_big = 0, n_slots = 0, grid = 1, group = 1, warps = 0, hot_bytes = 0;
     std::vector<uint8_t> h_results;
     float last_ms = 0.f;
     u32 last_launches = 0;
@@ -155,22 +155,49 @@ extern "C" int32_t astra_set_gpu(astra_ctx* c, uint32_t cus, uint32_t wpc, uint3
     return ASTRA_OK;
 }
 
-// CTAs per design point and warps per CTA for a batch of n points (A0 scheduling policy).
-// Few points: spread each over a group of CTAs (one node range each) so the device is used;
-// many points: one CTA per point, the queue balances.  ASTRA_FLAG_GROUP(g) overrides.
-static void choose_shape(const astra_ctx* c, u32 n, const astra_point* pts, u32 max_nodes, u32 sms, u32* group, u32* warps) {
-    u32 g = (u32)((c->flags >> 8) & 0xff);
-    if (g == 0) {
-        // heavy points = those within 4x of the most expensive one (lines issued is the proxy);
-        // give each of them as many CTAs as there are nodes, as long as they all stay co-resident
-        u64 mx = 1;
-        for (u32 i = 0; i < n; i++) mx = std::max<u64>(mx, c->colls[pts[i].coll_id].total_lines);
-        u32 heavy = 0;
-        for (u32 i = 0; i < n; i++) if (c->colls[pts[i].coll_id].total_lines * 4 >= mx) heavy++;
-        g = std::max<u32>(1, std::min<u32>(16, sms / std::max<u32>(1, heavy)));
+// A0 scheduling policy.  Points are split in two classes by a cost proxy (lookahead windows x
+// per-window overhead + line-hop events): "big" points, whose cost exceeds what one CTA's fair share
+// of the batch is, run on a group of CTAs (one node range each, one group barrier per window); the
+// rest run on one CTA each.  Groups whose queue is empty go on as single CTAs.
+// ASTRA_FLAG_GROUP(g) overrides: every point on g CTAs (g = 1: every point on one).
+static void classify(const astra_ctx* c, u32 n, const astra_point* pts, u32 n_ctas, std::vector<double>& cost,
+                     std::vector<uint8_t>& big, u32* group) {
+    cost.assign(n, 0.0); big.assign(n, 0);
+    double total = 0, cmax = 0;
+    for (u32 i = 0; i < n; i++) {
+        cost[i] = astra_point_cost(c->topos[pts[i].topo_id], c->colls[pts[i].coll_id], c->flags & 0xff);
+        total += cost[i]; cmax = std::max(cmax, cost[i]);
     }
-    *group = std::max<u32>(1, std::min<u32>(std::min<u32>(g, 16), std::max<u32>(1, max_nodes)));
-    *warps = 16;
+    u32 g = (u32)((c->flags >> 8) & 0xff);
+    if (g == 1 || n == 0) { *group = 1; return; }
+    if (g > 1) { *group = std::min<u32>(g, 16); std::fill(big.begin(), big.end(), 1); return; }
+    // Model: a group of g CTAs runs a point min(g, nodes) / 2 times faster than one CTA and costs
+    // g CTAs for that time.  Try group sizes and how many of the most expensive points get one;
+    // keep the pair with the smallest estimated makespan (critical point vs. total work / CTAs).
+    std::vector<u32> idx(n);
+    std::iota(idx.begin(), idx.end(), 0u);
+    std::sort(idx.begin(), idx.end(), [&](u32 a, u32 b) { return cost[a] > cost[b]; });
+    std::vector<double> pre(n + 1, 0.0);
+    for (u32 i = 0; i < n; i++) pre[i + 1] = pre[i] + cost[idx[i]];
+    double best = std::max(cmax, total / n_ctas);
+    u32 best_g = 1, best_r = 0;
+    const u32 gs[] = {2, 3, 4, 6, 8, 9, 12, 16};
+    for (u32 g2 : gs) {
+        for (u32 r = 1; r <= n; r = r < 4 ? r + 1 : r + (r + 1) / 2) {
+            u32 vmin = 0xffffffffu;
+            for (u32 i = 0; i < std::min<u32>(r, 8); i++) vmin = std::min(vmin, c->topos[pts[idx[i]].topo_id].V);
+            const double speed = 0.5 * std::min<u32>(g2, vmin);
+            if (speed <= 1.0) continue;
+            const u32 slots = std::max<u32>(1, std::min<u32>(r, n_ctas / g2));
+            const double t_big = std::max(cost[idx[0]] / speed, pre[r] / speed / slots);      // critical point, big queue over its slots
+            const double t_small = r < n ? cost[idx[r]] : 0.0;
+            const double t_work = (pre[n] - pre[r] + pre[r] / speed * g2) / n_ctas;
+            const double est = std::max(std::max(t_big, t_small), t_work);
+            if (est < best * 0.97) { best = est; best_g = g2; best_r = r; }
+        }
+    }
+    for (u32 i = 0; i < best_r; i++) big[idx[i]] = 1;
+    *group = best_g;
 }
 
 static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_t max_cycles) {
@@ -178,25 +205,24 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     Blob blob;
     std::map<u32, std::vector<u64>> topo_off, coll_off;
     c->descs.assign(n, PointDesc());
-    std::vector<double> cost(n, 0.0);
-    u64 roff = 0; u64 ws_max = 0;
-    u32 max_nodes = 1;
+    u64 roff = 0, ws_big_max = 0, ws_single_max = 0;
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];
         if (p.topo_id >= c->topos.size() || p.coll_id >= c->colls.size() || p.gpu_id >= c->gpus.size())
             return fail(c, ASTRA_ESTATE, "design point references an unknown id");
-        max_nodes = std::max(max_nodes, c->topos[p.topo_id].V);
     }
     int dev = 0, sms = 0, smem_max = 0;
     CUDA_TRY(c, cudaGetDevice(&dev), "cudaGetDevice");
     CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "device attribute");
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "device attribute");
-    choose_shape(c, n, pts, max_nodes, (u32)sms, &c->group, &c->warps);
+    c->warps = 16;
+    std::vector<double> cost; std::vector<uint8_t> big;
+    classify(c, n, pts, (u32)sms, cost, big, &c->group);
     PlanOptions opt;
-    opt.flags = c->flags & 0xf00ffull; opt.max_cycles = max_cycles; opt.group = c->group;
+    opt.flags = c->flags & 0xf00ffull; opt.max_cycles = max_cycles;
     const u32 fixed = astra_engine_fixed_smem(c->warps);
     opt.hot_budget = (u32)smem_max > fixed + 1024 ? (u32)smem_max - fixed - 1024 : 0;
-    u32 hot_max = 0;
+    u32 hot_max = 0, n_big = 0;
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];
         const HostTopo& t = c->topos[p.topo_id];
@@ -216,39 +242,56 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
             coll_off[p.coll_id] = o;
         }
         std::string err;
+        double unused = 0;
+        opt.group = big[i] ? c->group : 1;
         int32_t rc = astra_plan_point(t, h, c->gpus[p.gpu_id], opt, topo_off[p.topo_id].data(),
-                                      coll_off[p.coll_id].data(), blob, c->descs[i], cost[i], err);
+                                      coll_off[p.coll_id].data(), blob, c->descs[i], unused, err);
         if (rc) return fail(c, rc, "point " + std::to_string(i) + ": " + err);
         PointDesc& P = c->descs[i];
         P.r_step_ts = roff; roff += 32ull * P.S;
         P.r_link_lines = roff; roff += 8ull * P.E;
         P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
         P.r_diag = roff; roff += 128;
-        ws_max = std::max(ws_max, P.ws_bytes);
+        if (big[i]) { ws_big_max = std::max(ws_big_max, P.ws_bytes); n_big++; }
+        else ws_single_max = std::max(ws_single_max, P.ws_bytes);
         hot_max = std::max(hot_max, P.hot_bytes);
     }
     c->hot_bytes = hot_max;
     c->results_bytes = roff ? roff : 16;
-    c->ws_stride = (ws_max + 255) & ~255ull;
     std::string err;
     u32 occ = 0, nsm = 0;
     int32_t rc = astra_engine_occupancy(c->warps, c->hot_bytes, &occ, &nsm, err);
     if (rc) return fail(c, rc, err);
     if (occ == 0) return fail(c, ASTRA_ECUDA, "kernel does not fit on an SM");
     // every CTA of the grid must be resident at once (persistent CTAs, group barriers)
-    c->n_groups = std::max<u32>(1, std::min<u32>(n, occ * nsm / c->group));
+    const u32 n_ctas = occ * nsm, n_small = n - n_big;
+    c->n_big = n_big;
+    c->n_slots = n_big ? std::max<u32>(1, std::min<u32>(n_big, n_ctas / c->group)) : 0;
+    c->grid = std::max<u32>(1, std::min<u32>(n_ctas, c->n_slots * c->group + n_small));
+    if (n_big && c->grid < c->n_slots * c->group) c->grid = c->n_slots * c->group;
+    c->ws_big_stride = (ws_big_max + 255) & ~255ull;
+    c->ws_single_stride = n_small ? (ws_single_max + 255) & ~255ull : 0;
     size_t free_b = 0, total_b = 0;
     CUDA_TRY(c, cudaMemGetInfo(&free_b, &total_b), "cudaMemGetInfo");
     u64 budget = (u64)(free_b * 0.85);
     u64 fixed_b = blob.bytes.size() + c->results_bytes + n * sizeof(PointDesc) + n * 4 + 4096;
-    if (fixed_b + c->ws_stride > budget) return fail(c, ASTRA_ENOMEM, "batch does not fit in device memory");
-    while (c->n_groups > 1 && fixed_b + (u64)c->n_groups * c->ws_stride > budget) c->n_groups--;
-    c->ws_total = (u64)c->n_groups * c->ws_stride;
+    auto ws_need = [&]() { return (u64)c->n_slots * c->ws_big_stride + (u64)c->grid * c->ws_single_stride; };
+    while (fixed_b + ws_need() > budget) {       // fewer resident CTAs until the workspaces fit
+        if (c->grid > c->n_slots * c->group && c->grid > 1) c->grid--;
+        else if (c->n_slots > 1) { c->n_slots--; c->grid = std::max<u32>(1, std::min(c->grid, std::max(c->n_slots * c->group, c->grid - c->group))); }
+        else return fail(c, ASTRA_ENOMEM, "batch does not fit in device memory");
+    }
+    c->ws_single_off = (u64)c->n_slots * c->ws_big_stride;
+    c->ws_total = ws_need();
     c->const_bytes = blob.bytes.size();
 
+    // queue order: big points first (most expensive first), then the small ones (most expensive first)
     std::vector<u32> order(n);
     std::iota(order.begin(), order.end(), 0u);
-    std::stable_sort(order.begin(), order.end(), [&](u32 a, u32 b) { return cost[a] > cost[b]; });
+    std::stable_sort(order.begin(), order.end(), [&](u32 a, u32 b) {
+        if (big[a] != big[b]) return big[a] > big[b];
+        return cost[a] > cost[b];
+    });
 
     CUDA_TRY(c, cudaMalloc((void**)&c->d_const, std::max<size_t>(16, blob.bytes.size())), "cudaMalloc const");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_ws, std::max<u64>(16, c->ws_total)), "cudaMalloc workspace");
@@ -256,7 +299,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     CUDA_TRY(c, cudaMalloc((void**)&c->d_points, std::max<size_t>(16, n * sizeof(PointDesc))), "cudaMalloc points");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_order, std::max<size_t>(16, n * 4)), "cudaMalloc order");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_queue, 16), "cudaMalloc queue");
-    CUDA_TRY(c, cudaMalloc((void**)&c->d_groups, sizeof(GroupCtl) * c->n_groups), "cudaMalloc groups");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_groups, sizeof(GroupCtl) * std::max<u32>(1, c->n_slots)), "cudaMalloc groups");
     CUDA_TRY(c, cudaMemcpyAsync(c->d_const, blob.bytes.data(), blob.bytes.size(), cudaMemcpyHostToDevice, c->stream), "H2D const");
     CUDA_TRY(c, cudaMemcpyAsync(c->d_points, c->descs.data(), n * sizeof(PointDesc), cudaMemcpyHostToDevice, c->stream), "H2D points");
     CUDA_TRY(c, cudaMemcpyAsync(c->d_order, order.data(), n * 4, cudaMemcpyHostToDevice, c->stream), "H2D order");
@@ -282,8 +325,10 @@ extern "C" int32_t astra_run_batch_async(astra_ctx* c, uint32_t n, const astra_p
         if (n) {
             EngineLaunch L;
             L.d_const = c->d_const; L.d_ws = c->d_ws; L.d_results = c->d_results; L.d_points = c->d_points;
-            L.d_order = c->d_order; L.d_queue = c->d_queue; L.d_groups = c->d_groups; L.n_points = n; L.ws_stride = c->ws_stride;
-            L.n_groups = c->n_groups; L.group = c->group; L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes;
+            L.d_order = c->d_order; L.d_queue = c->d_queue; L.d_groups = c->d_groups; L.n_points = n;
+            L.n_big = c->n_big; L.n_slots = c->n_slots; L.group = c->group; L.grid = c->grid;
+            L.ws_big_stride = c->ws_big_stride; L.ws_single_off = c->ws_single_off; L.ws_single_stride = c->ws_single_stride;
+            L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes;
             std::string err;
             int32_t rc = astra_engine_launch(L, (void*)c->stream, err);
             if (rc) return fail(c, rc, err);

@@ -1528,6 +1528,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32
     if (kind != ASTRA_LK_GENERAL) {
         // 128 entries per step, four consecutive ones per lane: local running max, then one warp scan
         const int P = (int)param;
+        const u32 bmagic = 0xffffffffu / param + 1u;           // n / param == umulhi(n, bmagic) for n < 2^32 / 32 (param <= 31)
         for (u32 base = 0; base < scan_limit; base += 128) {
             const u32 j0 = base + 4 * lane;
             u64 fl[4]; int val[4]; u32 xx[4]; bool act[4];
@@ -1553,7 +1554,7 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32
             for (int q = 0; q < 4; q++) {
                 const u32 j = j0 + q;
                 const int pm = max(excl, val[q]);
-                xx[q] = kind == ASTRA_LK_INT ? (u32)((int)j + pm) / param : (u32)(P * (int)j + max(pm, xn_rel));
+                xx[q] = kind == ASTRA_LK_INT ? (param == 1 ? (u32)((int)j + pm) : __umulhi((u32)((int)j + pm), bmagic)) : (u32)(P * (int)j + max(pm, xn_rel));
                 const bool acc = act[q] && xx[q] < wlen;
                 cnt_act += act[q]; cnt_acc += acc;
                 if (acc) {
@@ -1702,7 +1703,8 @@ __device__ __forceinline__ void group_barrier(GroupCtl* gc, u32 target) {
 extern "C" __global__ void __launch_bounds__(512, 1)
 astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
-                  GroupCtl* groups, u32 n_points, u64 ws_stride, u32 group, u32 hot_off) {
+                  GroupCtl* groups, u32 n_points, u32 n_big, u32 n_slots, u32 group0,
+                  u64 ws_big_stride, u64 ws_single_off, u64 ws_single_stride, u32 hot_off) {
     extern __shared__ __align__(16) uint8_t smem[];
     Ctx& c = *reinterpret_cast<Ctx*>(smem);
     Ctl& ctl = *reinterpret_cast<Ctl*>(smem + ((sizeof(Ctx) + 15) & ~size_t(15)));
@@ -1711,20 +1713,25 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
     const u32 tid = threadIdx.x, nthr = blockDim.x;
     const u32 lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
     u32* scr = scr_all + warp * SCR_WORDS;
-    const u32 gid = blockIdx.x / group, rank = blockIdx.x % group;
-    uint8_t* ws = ws_base + (size_t)gid * ws_stride;
+    // CTAs [0, n_slots * group0) form the groups that run the big points; every CTA can run small ones
+    const bool in_slot = blockIdx.x < n_slots * group0;
+    u32 group = in_slot ? group0 : 1u;
+    u32 rank = in_slot ? blockIdx.x % group0 : 0u;
+    const u32 gid = in_slot ? blockIdx.x / group0 : 0u;
+    uint8_t* ws = in_slot ? ws_base + (size_t)gid * ws_big_stride : ws_base + ws_single_off + (size_t)blockIdx.x * ws_single_stride;
     GroupCtl* gc = groups + gid;
     u32 bar_target = 0;                 // arrivals that complete the next group barrier
 
     for (;;) {
         __syncthreads();
         if (group == 1) {
-            if (tid == 0) ctl.point = atomicAdd(queue, 1u);
+            if (tid == 0) { const u32 q = atomicAdd(&queue[1], 1u); ctl.point = q < n_points - n_big ? n_big + q : ASTRA_NONE32; }
             __syncthreads();
         } else {
             bar_target += group; group_barrier(gc, bar_target);     // everyone is done with the previous point's control block
             if (rank == 0 && tid == 0) {
-                gc->point = atomicAdd(queue, 1u);
+                const u32 q = atomicAdd(&queue[0], 1u);
+                gc->point = q < n_big ? q : ASTRA_NONE32;
                 gc->acked = 0; gc->err = 0; gc->completion = 0;
                 gc->hint[0] = gc->hint[1] = gc->hint[2] = ASTRA_T_INF;
             }
@@ -1733,7 +1740,13 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             __syncthreads();
         }
         const u32 qi = ctl.point;
-        if (qi >= n_points) break;
+        if (qi == ASTRA_NONE32) {
+            if (group == 1) break;
+            // no big point left: the CTAs of the group go on alone with the small ones
+            group = 1; rank = 0;
+            ws = ws_base + ws_single_off + (size_t)blockIdx.x * ws_single_stride;
+            continue;
+        }
         const u32 pi = order[qi];
         const PointDesc& P = points[pi];
         if (tid == 0) {
@@ -1988,12 +2001,12 @@ int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& er
     size_t sm = (size_t)fixed + L.hot_bytes;
     cudaError_t e = cudaFuncSetAttribute(astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) { err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
-    e = cudaMemsetAsync(L.d_queue, 0, sizeof(u32), (cudaStream_t)stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(L.d_groups, 0, sizeof(GroupCtl) * L.n_groups, (cudaStream_t)stream);
+    e = cudaMemsetAsync(L.d_queue, 0, 4 * sizeof(u32), (cudaStream_t)stream);
+    if (e == cudaSuccess && L.n_slots) e = cudaMemsetAsync(L.d_groups, 0, sizeof(GroupCtl) * L.n_slots, (cudaStream_t)stream);
     if (e != cudaSuccess) { err = std::string("queue reset: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
-    astra_step_kernel<<<L.n_groups * L.group, L.warps_per_cta * 32, sm, (cudaStream_t)stream>>>(
-        L.d_const, L.d_ws, L.d_results, L.d_points, L.d_order, L.d_queue, L.d_groups, L.n_points, L.ws_stride,
-        L.group, fixed);
+    astra_step_kernel<<<L.grid, L.warps_per_cta * 32, sm, (cudaStream_t)stream>>>(
+        L.d_const, L.d_ws, L.d_results, L.d_points, L.d_order, L.d_queue, L.d_groups, L.n_points, L.n_big, L.n_slots,
+        L.group, L.ws_big_stride, L.ws_single_off, L.ws_single_stride, fixed);
     e = cudaGetLastError();
     if (e != cudaSuccess) { err = std::string("kernel launch: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
     return ASTRA_OK;

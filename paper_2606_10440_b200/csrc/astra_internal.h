@@ -152,6 +152,7 @@ int32_t astra_build_coll(HostColl& c, std::string& err);
 int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g, const PlanOptions& opt,
                          const u64* topo_off, const u64* coll_off, Blob& blob, PointDesc& out, double& cost,
                          std::string& err);
+double astra_point_cost(const HostTopo& t, const HostColl& c, u64 flags);
 #define ASTRA_N_TOPO_TABLES 7
 #define ASTRA_N_COLL_TABLES 7
 
@@ -159,7 +160,13 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
 struct EngineLaunch {
     const uint8_t* d_const; uint8_t* d_ws; uint8_t* d_results;
     const PointDesc* d_points; const u32* d_order; u32* d_queue; GroupCtl* d_groups;
-    u32 n_points; u64 ws_stride; u32 n_groups, group, warps_per_cta, hot_bytes;
+    u32 n_points;
+    // scheduling classes: order[0, n_big) are the points that run on a group of `group` CTAs (n_slots
+    // groups, workspace d_ws + slot * ws_big_stride), the rest run on one CTA each (workspace
+    // d_ws + ws_single_off + cta * ws_single_stride); a group whose queue is empty turns into single CTAs
+    u32 n_big, n_slots, group, grid;
+    u64 ws_big_stride, ws_single_off, ws_single_stride;
+    u32 warps_per_cta, hot_bytes;
 };
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err);
 int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err);

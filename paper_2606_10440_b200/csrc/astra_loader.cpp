@@ -141,6 +141,29 @@ int32_t astra_build_coll(HostColl& c, std::string& err) {
     return ASTRA_OK;
 }
 
+// Cost proxy of a design point for the scheduler (A0): lookahead windows it will step through
+// (bottleneck link occupancy / window) and line-hop events.  Only ratios between points matter.
+double astra_point_cost(const HostTopo& t, const HostColl& c, u64 flags) {
+    const u32 G = t.G, E = t.E;
+    std::vector<u64> via(E, 0);
+    double events = 0;
+    u64 alpha_max = 1;
+    for (u32 s = 0; s < c.S; s++) {
+        u32 v = c.owner[s], d = c.dst[s], hops = 0;
+        if (v >= G || d >= G || t.dist[(size_t)v * G + d] == 0xffffffffu) continue;
+        alpha_max = std::max<u64>(alpha_max, t.dist[(size_t)v * G + d]);
+        while (v != d && hops <= t.V) { u32 e = t.next_link[(size_t)v * G + d]; via[e] += c.lines[s]; v = t.head[e]; hops++; }
+        events += (double)c.lines[s] * (hops + 2);
+    }
+    double cycles = 0;
+    for (u32 e = 0; e < E; e++) cycles = std::max(cycles, (double)via[e] * 256.0 / t.bw[e]);
+    cycles += 4.0 * alpha_max;
+    u32 W = 1;
+    if (!(flags & ASTRA_FLAG_WINDOW_1)) { W = std::max<u32>(1, std::min<u32>(t.min_leff, 1u << ASTRA_WMAX_LOG2)); if (W >= 64) W &= ~63u; }
+    // measured: a window costs a CTA about 20 k clocks plus 3.5 k per GPU and per link it steps; events are cheap
+    return cycles / W * (20000.0 + 3500.0 * (t.G + E)) + events * 10.0;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Plan one design point: plan tables into the blob, array placement into the descriptor.
 // topo_off / coll_off are the blob offsets of the shared topology / collective tables.
