@@ -127,6 +127,27 @@ def run_reference(args):
     }))
 
 
+def extra_workloads(device, stream):
+    """Context, not the headline: the other BASELINE configs at full size, one warm-up and one timed
+    run each, device time of the engine's launch (CUDA events on its stream)."""
+    from astra_inputs import configs
+    from paper_2606_10440_b200 import Engine
+    out = {}
+    for name, make in (("config3", configs.config3), ("config4", lambda: configs.config4(4096)), ("config5", configs.config5)):
+        w = make()
+        with Engine(device) as eng:
+            eng.set_stream(stream.cuda_stream)
+            pts = eng.load_workload(w)
+            eng.run_batch(pts, w.max_cycles)
+            eng.run_batch(pts, w.max_cycles)
+            ms = eng.last_run_info()[0]
+            ok = all(eng.read_results(i, False, False)[0].status == 0 for i in range(len(pts)))
+        out[name] = {"design_points": w.n_points, "transactions": w.total_lines(), "kernel_ms": ms,
+                     "transactions_per_sec": w.total_lines() / (ms * 1e-3), "design_points_per_sec": w.n_points / (ms * 1e-3),
+                     "all_points_finished": ok}
+    return out
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -220,13 +241,9 @@ def run_ours(args):
 
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get(w.name)
-        except Exception:
-            traffic = None
+    # dram__bytes_read.sum + dram__bytes_write.sum of one astra_step_kernel launch, `ncu --set full` capture
+    # summarised in profiles/r01_v6_ncu.md (config 2 only; other workloads were not captured)
+    traffic = {"config2": 36207872}.get(w.name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -242,10 +259,12 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "kernel": "astra_step_kernel", "kernel_ms": k_ms,
                      "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                     "note": "bytes = 72 per transaction + 20 per link hop (SURVEY 8(d)); the kernel is "
-                             "latency/issue bound, see DESIGN.md section 6",
+                     "note": "bytes = 72 per transaction + 20 per link hop (SURVEY 8(d)); state stays in L2/shared memory at "
+                             "this size, the kernel is bound by the dependent chain per lookahead window, see DESIGN.md section 6",
                      "node_cycles_stepped": busy, "device_bytes": dev_bytes},
     }
+    if rank == 0 and world == 1 and not args.no_extras:
+        line["other_workloads"] = extra_workloads(local_rank, stream)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = {k: v for k, v in oracle_baseline(w).items() if k != "seconds"}
     if rank == 0:
@@ -262,6 +281,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the one-shot runs of configs 3, 4, 5")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
