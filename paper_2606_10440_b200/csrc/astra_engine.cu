@@ -4,19 +4,22 @@
 // The paper's simulator is an event-driven CPU program.  This engine is organised
 // around one structural fact instead: a line accepted by a link at cycle a cannot reach the next
 // node before a + Leff, and an ack cannot reach its owner before t_deliv + alpha >= t_deliv +
-// min Leff.  With W = 2^k <= min Leff, nothing a node does inside the window [kW, (k+1)W) can
+// min Leff.  With W <= min Leff, nothing a node does inside the window [kW, (k+1)W) can
 // influence another node inside the same window.  So simulated time advances a whole window at a
 // time, every stage of a window is node-local, and inside a window every phase of rules R7-R12
 // is a data-parallel pass over ALL events of the window instead of a serial walk over cycles:
 //
-//   stage 1  arrivals (R7 A1)   one warp per in-link, 32 pipe entries per step: deliveries bump
-//            the step counters and post slot-addressed ack records; a transit line either goes
-//            straight to the tail of the next link's ring (that link has a single feeder) or
-//            sets one bit in the (out-link, cycle) cell at a slot fixed by (in-link, position).
-//            ack gather (R6, A3) one warp per GPU: this window's acks, counting-sorted by cycle.
-//   stage 2  release + issue (R10-R13) one warp per GPU: dependency events of the window become
-//            timed releases; the fixed-priority HBM grant scan walks only the cycles of the
-//            window where something can change; issued lines are appended / recorded.
+//   stage 1  arrivals (R7 A1) and ack discovery (R6, A3) as a flat list of chunk tasks: the lines
+//            due on every in-link are known (link service counted them per arrival window), so
+//            links are cut into independent 32-entry chunks -- deliveries (slot-addressed ack
+//            record + bitmap bit), forwards to a single-feeder link (position = base + index),
+//            forwards to multi-feeder links (one bit in the (out-link, cycle) cell at a slot fixed
+//            by (in-link, rank inside the cycle)); the ack bitmap into 32-word chunks.
+//   stage 2  release + issue (R10-R13): events -> release times; every wavefront runs through the
+//            window as if the HBM budget never bound, on a thread (wf_sim) or a warp (wf_heavy,
+//            prefix maximum over the issue index); per-cycle counts prove it (gpu_binds), or the
+//            exact fixed-priority grants are computed word by word (wf_priority_word); issues are
+//            ranked inside their cycle by wavefront id (ev_place) = FIFO position / cell slot.
 //   stage 3  merge (R7/R8 append order) per out-link with several feeders: prefix sum of the
 //            cell popcounts = FIFO position of every slot; the feeders then write their lines
 //            straight to those positions.  No atomically allocated slot, no sort.
@@ -27,8 +30,9 @@
 //
 // Hot per-node state (link cursors, cells, ready masks, wavefront records, step counters) lives
 // in shared memory whenever the loader could fit it (PointDesc::a_off placement flags); rings and
-// ack records stream through L2/HBM.  One CTA (or a group of CTAs, one node range each, with one
-// group barrier per window) simulates one design point and pulls the next from a cost-sorted queue.
+// ack records stream through L2/HBM.  One CTA, or a group of CTAs with one node range each and one
+// group barrier per window, simulates one design point; a persistent grid pulls points from two
+// cost-sorted queues (grouped / single), see classify() in astra_api.cpp.
 #include "astra_internal.h"
 #include "../../include/astra.h"
 
