@@ -322,7 +322,7 @@ __device__ void stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
     u32 nch = 0;
     if (fl) {
         if (n) {
-            nch = (n + 31) / 32;
+            nch = fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32;
             c.tl_lo[e] = lo; c.tl_n[e] = n; c.pipe_head[e] = lo + n;
             if (fl == ASTRA_LF_FORWARD_ONLY) { const u32 o = c.lfwd[e]; c.tl_base[e] = c.run[o]; c.run[o] += n; }
             else if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;          // set by a chunk that marks a cell: pass 3 needed
@@ -473,36 +473,39 @@ __device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0,
     }
 }
 
-// 32 pipe entries of a link whose lines terminate at its head or go on to multi-feeder links (R7 A1).
+// Pipe entries of a link whose lines terminate at its head or go on to multi-feeder links (R7 A1).
 // A line's cell slot is (in-link's slot base + its rank among the lines this link delivers in the
 // same cycle); lines of one cycle are consecutive in the stream, so the rank is a look at the
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
 // PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
 template <int PASS>
+__device__ void cells_half(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
+
+// A task is 64 entries: both halves' ring loads (and the look-back) are in flight before the first use.
+template <int PASS>
 __device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
-    const u32 i0 = lo + chunk * 32, ii = i0 + lane;
+    const u32 i0 = lo + chunk * 64;
     const u64* ring = c.ring + c.ring_off[e];
     const u32 rmask = c.ring_mask[e];
-    bool valid = (int32_t)(lo + n - ii) > 0;
-    u64 flit = 0; u32 d = 0xffffffffu;
-    if (valid) {
-        flit = __ldcg(&ring[ii & rmask]);
-        d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
-        valid = d < wlen;                                     // watchdog cut inside the window
-    }
-    // rank among the same-cycle lines of this link
-    const u32 d0 = __shfl_sync(FULL, d, 0);
-    u32 back = 0;
-    {
-        const u32 nb = c.ceilb[e] - 1;                        // at most ceil(B) lines per cycle
-        bool same = false;
-        if (lane < nb && (int32_t)(i0 - 1 - lane - lo) >= 0) {
-            const u64 f2 = __ldcg(&ring[(i0 - 1 - lane) & rmask]);
-            same = (((u32)(f2 >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) == d0;
-        }
-        back = __popc(__ballot_sync(FULL, same));
-    }
+    const u32 nb = c.ceilb[e] - 1;                            // at most ceil(B) lines per cycle
+    const bool in0 = (int32_t)(lo + n - (i0 + lane)) > 0, in1 = (int32_t)(lo + n - (i0 + 32 + lane)) > 0;
+    const bool inb = lane < nb && (int32_t)(i0 - 1 - lane - lo) >= 0;
+    const u64 fa = in0 ? __ldcg(&ring[(i0 + lane) & rmask]) : 0ull;
+    const u64 fb = in1 ? __ldcg(&ring[(i0 + 32 + lane) & rmask]) : 0ull;
+    const u64 fz = inb ? __ldcg(&ring[(i0 - 1 - lane) & rmask]) : 0ull;
+    const u32 da = in0 ? (((u32)(fa >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xffffffffu;
+    const u32 db = in1 ? (((u32)(fb >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xfffffffeu;
+    const u32 dz = inb ? (((u32)(fz >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xfffffffdu;
+    const u32 da0 = __shfl_sync(FULL, da, 0), db0 = __shfl_sync(FULL, db, 0);
+    const u32 back_a = __popc(__ballot_sync(FULL, dz == da0));          // same-cycle lines before the task
+    const u32 back_b = __popc(__ballot_sync(FULL, da == db0));          // ... before its second half
+    cells_half<PASS>(c, ctl, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, lane);   // d >= wlen: watchdog cut inside the window
+    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, lane);
+}
+
+template <int PASS>
+__device__ void cells_half(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
     const u32 vmask = __ballot_sync(FULL, valid);
     if (!valid) return;
     const u32 grp = __match_any_sync(vmask, d);
