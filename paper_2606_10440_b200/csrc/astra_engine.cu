@@ -1536,11 +1536,16 @@ __device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32
         // 128 entries per step, four consecutive ones per lane: local running max, then one warp scan
         const int P = (int)param;
         const u32 bmagic = 0xffffffffu / param + 1u;           // n / param == umulhi(n, bmagic) for n < 2^32 / 32 (param <= 31)
+        u64 nx[4];                                           // next step's entries, loaded one step ahead
+#pragma unroll
+        for (int q = 0; q < 4; q++) nx[q] = 4 * lane + q < scan_limit ? ring[(fh + 4 * lane + q) & rmask] : 0ull;
         for (u32 base = 0; base < scan_limit; base += 128) {
             const u32 j0 = base + 4 * lane;
             u64 fl[4]; int val[4]; u32 xx[4]; bool act[4];
 #pragma unroll
-            for (int q = 0; q < 4; q++) { act[q] = j0 + q < scan_limit; fl[q] = act[q] ? ring[(fh + j0 + q) & rmask] : 0ull; }
+            for (int q = 0; q < 4; q++) { act[q] = j0 + q < scan_limit; fl[q] = nx[q]; }
+#pragma unroll
+            for (int q = 0; q < 4; q++) nx[q] = j0 + 128 + q < scan_limit ? ring[(fh + j0 + 128 + q) & rmask] : 0ull;
             int m = INT_MIN;
 #pragma unroll
             for (int q = 0; q < 4; q++) {
