@@ -71,7 +71,7 @@ extern "C" {
 #define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
 #define ASTRA_FLAG_DIAG_RANK(r) (((uint64_t)(r) & 0xfull) << 16) /* which CTA of a group reports astra_read_diag */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g
-                                            CTAs (1..16), one node range each; 0 = engine's choice */
+                                            CTAs (1..255, at most the co-resident CTAs of the device), one node range each; 0 = engine's choice */
 
 /* Per-point simulation outcome */
 #define ASTRA_STATUS_DONE       0

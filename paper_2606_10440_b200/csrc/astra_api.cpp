@@ -170,7 +170,7 @@ static void classify(const astra_ctx* c, u32 n, const astra_point* pts, u32 n_ct
     }
     u32 g = (u32)((c->flags >> 8) & 0xff);
     if (g == 1 || n == 0) { *group = 1; return; }
-    if (g > 1) { *group = std::min<u32>(g, 16); std::fill(big.begin(), big.end(), 1); return; }
+    if (g > 1) { *group = std::min<u32>(g, std::max<u32>(2, n_ctas)); std::fill(big.begin(), big.end(), 1); return; }
     // Model: a group of g CTAs runs a point min(g, nodes) / 2 times faster than one CTA and costs
     // g CTAs for that time.  Try group sizes and how many of the most expensive points get one;
     // keep the pair with the smallest estimated makespan (critical point vs. total work / CTAs).
@@ -181,8 +181,9 @@ static void classify(const astra_ctx* c, u32 n, const astra_point* pts, u32 n_ct
     for (u32 i = 0; i < n; i++) pre[i + 1] = pre[i] + cost[idx[i]];
     double best = std::max(cmax, total / n_ctas);
     u32 best_g = 1, best_r = 0;
-    const u32 gs[] = {2, 3, 4, 6, 8, 9, 12, 16};
+    const u32 gs[] = {2, 3, 4, 6, 8, 9, 12, 16, 24, 32, 48, 64, 96, 128, 148, 192, 255};
     for (u32 g2 : gs) {
+        if (g2 > n_ctas) break;
         for (u32 r = 1; r <= n; r = r < 4 ? r + 1 : r + (r + 1) / 2) {
             u32 vmin = 0xffffffffu;
             for (u32 i = 0; i < std::min<u32>(r, 8); i++) vmin = std::min(vmin, c->topos[pts[idx[i]].topo_id].V);
