@@ -312,29 +312,36 @@ __device__ void stage1_setup_gpu(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 lane) {
     }
 }
 
-__device__ void stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
+__device__ u32 stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
     const u32 e = c.in_link[i];
-    u32* dc = &c.due_cnt[(size_t)e * c.NW + (k & c.NWmask)];
-    const u32 n = ld_vol(dc);
-    if (n) *dc = 0;
+    u32* dcb = &c.due_cnt[(size_t)e * c.NW];
+    const u32 n = ld_vol(&dcb[k & c.NWmask]);
     const u32 lo = c.pipe_head[e], hi = ld_vol(&c.fifo_head[e]);
     const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
+    // in flight beyond this window: the earliest later window with lines due (A7); all bins are read at once
+    if (fl && c.NW <= 8) {
+        u32 nextw = ASTRA_NONE32;
+        for (u32 j = c.NW - 1; j >= 1; j--) if (ld_vol(&dcb[(k + j) & c.NWmask])) nextw = j;
+        if (nextw != ASTRA_NONE32) {
+            const u64 tw = (u64)(k + nextw) * c.W;
+            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
+        }
+    } else if (fl && hi != lo + n) {                            // many bins: read the first entry that is not due instead
+        const u64 flit = __ldcg(&c.ring[c.ring_off[e] + ((lo + n) & c.ring_mask[e])]);
+        atomicMin(&ctl.next_hint, t0 + (((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26));
+    }
+    if (n) dcb[k & c.NWmask] = 0;
     u32 nch = 0;
     if (fl) {
         if (n) {
             nch = fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32;
             c.tl_lo[e] = lo; c.tl_n[e] = n; c.pipe_head[e] = lo + n;
             if (fl == ASTRA_LF_FORWARD_ONLY) { const u32 o = c.lfwd[e]; c.tl_base[e] = c.run[o]; c.run[o] += n; }
-            else if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;          // set by a chunk that marks a cell: pass 3 needed
         }
-        if (hi != lo + n) {                                     // in flight beyond this window: next arrival (A7)
-            const u64 flit = __ldcg(&c.ring[c.ring_off[e] + ((lo + n) & c.ring_mask[e])]);
-            atomicMin(&ctl.next_hint, t0 + (((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26));
-        }
-        else if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;
+        if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;             // set by a chunk that marks a cell: pass 3 needed
         if (hi - lo > c.ring_mask[e] + 1) atomicOr(&ctl.err, 1u);
     } else if (hi != lo) nch = 1;
-    c.tbase[i] = nch;
+    return nch;
 }
 
 // exclusive prefix of the per-link task counts (one warp); tbase[i_hi] = total
@@ -1819,9 +1826,19 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             busy += wlen;
             // stage 1: arrivals and ack discovery, as a flat list of chunk tasks
             for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) stage1_setup_gpu(c, ctl, g, k, lane);
-            for (u32 i = c.i_lo + tid; i < c.i_hi; i += nthr) stage1_setup_link(c, ctl, i, k, t0);
-            __syncthreads();
-            if (warp == 0) stage1_prefix(c, ctl, lane);
+            if (c.i_hi - c.i_lo <= 32) {                          // few in-links: set up and scan in one warp, one barrier less
+                if (warp == nwarps - 1) {
+                    const u32 i = c.i_lo + lane;
+                    const u32 v = i < c.i_hi ? stage1_setup_link(c, ctl, i, k, t0) : 0u;
+                    const u32 incl = warp_incl_scan(v, lane);
+                    if (i < c.i_hi) c.tbase[i] = incl - v;
+                    if (lane == 31) { c.tbase[c.i_hi] = incl; ctl.ntasks = incl; }
+                }
+            } else {
+                for (u32 i = c.i_lo + tid; i < c.i_hi; i += nthr) c.tbase[i] = stage1_setup_link(c, ctl, i, k, t0);
+                __syncthreads();
+                if (warp == 0) stage1_prefix(c, ctl, lane);
+            }
             __syncthreads();
             for (u32 g = c.g_lo; g < c.g_hi; g++) {
                 if (c.ack_n[g] == 0) continue;
