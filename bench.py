@@ -242,8 +242,8 @@ def run_ours(args):
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     # dram__bytes_read.sum + dram__bytes_write.sum of one astra_step_kernel launch, `ncu --set full` capture
-    # summarised in profiles/r01_v6_ncu.md (config 2 only; other workloads were not captured)
-    traffic = {"config2": 36207872}.get(w.name)
+    # summarised in profiles/r01_v7_ncu.md (config 2 only; other workloads were not captured)
+    traffic = {"config2": 34919936}.get(w.name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
