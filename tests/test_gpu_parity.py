@@ -108,12 +108,17 @@ def test_config2_all_22_points():
 
 
 def test_config3_reduced():
-    """Config 3 topology and collective at 1/64 of the message size (oracle finishes in seconds)."""
+    """Config 3 topology and collective at 1/8 of the message size (33 M lines; oracle finishes in seconds)."""
     check_workload(configs.config3(lines=32 * 1024 * 8))
 
 
 def test_config5_reduced():
     check_workload(configs.config5(n_nodes=4), oracle_flags=oracle.FLAG_PRUNED_SCAN)
+
+
+def test_config5_eight_nodes():
+    """A quarter of config 5's nodes (64 GPUs, 8 node and 8 rail switches): the engine spreads it over 80 CTAs."""
+    check_workload(configs.config5(n_nodes=8), oracle_flags=oracle.FLAG_PRUNED_SCAN)
 
 
 def test_config4_sample():
