@@ -21,6 +21,15 @@ EXPORTED_SYMBOLS = [
 
 FLAG_NO_WINDOW_SKIP = 1
 FLAG_WINDOW_1 = 2
+FLAG_SERIAL_ISSUE = 4          # testing: cycle-serial issue path everywhere
+FLAG_SERIAL_ARRIVALS = 8       # testing: one task per in-link
+FLAG_NO_HEAVY = 16             # testing: no warp-per-wavefront path
+FLAG_NO_PRIORITY_SWEEP = 32    # testing: budget-bound windows on the cycle-serial path
+
+
+def FLAG_DIAG_RANK(r: int) -> int:
+    """ASTRA_FLAG_DIAG_RANK(r): which CTA of a group reports astra_read_diag."""
+    return (r & 0xF) << 16
 
 
 def FLAG_GROUP(g: int) -> int:

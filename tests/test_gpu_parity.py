@@ -11,7 +11,7 @@ from tests.parity import check_workload, compare_point
 
 pytestmark = pytest.mark.gpu
 
-FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS = 1, 2, 4, 8
+FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_NO_HEAVY, FLAG_NO_PRIORITY_SWEEP = 1, 2, 4, 8, 16, 32
 
 
 def _single(topo, coll, gpu, name="case", max_cycles=1 << 22):
@@ -61,7 +61,7 @@ def test_i8_skip_equivalence(flags):
     check_workload(configs.config1(), flags=flags)
 
 
-@pytest.mark.parametrize("flags", [FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, 16, 32, FLAG_SERIAL_ISSUE | FLAG_SERIAL_ARRIVALS | 0x100])
+@pytest.mark.parametrize("flags", [FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_NO_HEAVY, FLAG_NO_PRIORITY_SWEEP, FLAG_SERIAL_ISSUE | FLAG_SERIAL_ARRIVALS | 0x100])
 def test_engine_paths_agree(flags):
     """The wavefront-parallel issue stage and the chunked arrival stage (defaults) and the cycle-serial /
     one-task-per-link paths they fall back to give the same bits; 0x100 = one CTA per point."""
