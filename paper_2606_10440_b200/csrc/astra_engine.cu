@@ -102,14 +102,14 @@ __device__ __forceinline__ int warp_incl_max(int v, u32 lane) {
 }
 
 // Mark slot `slot` of the cell (out-link o at node v, cycle t0 + d) occupied (R7/R8).
-__device__ __forceinline__ void cell_set(Ctx& c, Ctl& ctl, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
+__device__ __forceinline__ void cell_set(const Ctx& __restrict__ c, Ctl& ctl, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
     u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
     atomicOr(&c.masks[c.mask_off[o] + ci * c.nd_mw[v] + (slot >> 5)], 1u << (slot & 31));
     c.dirty[o] = 1u;
     ctl.any_merged = 1u;
 }
 // FIFO position, relative to the tail at the window start, of the line in slot `slot` of that cell.
-__device__ __forceinline__ u32 cell_pos(Ctx& c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
+__device__ __forceinline__ u32 cell_pos(const Ctx& __restrict__ c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
     u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
     const u32 mw = c.nd_mw[v];
     const u32* words = c.masks + c.mask_off[o] + ci * mw;
@@ -125,7 +125,7 @@ __device__ __forceinline__ u32 cell_pos(Ctx& c, u32 o, u32 v, u32 cb, u32 d, u32
 // sums) writes the lines that go to multi-feeder out-links at their FIFO positions.
 // ---------------------------------------------------------------------------------------------
 template <int PASS>
-__device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
+__device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 e = c.in_link[i];
     const u32 lo = c.pipe_head[e];
     u32 hi;
@@ -237,7 +237,7 @@ __device__ void arrivals_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0, u32 wlen, 
 // ---------------------------------------------------------------------------------------------
 // Cycle-serial path only: consume the window's ack bits of GPU g into ack_sorted, counting-sorted
 // by cycle (low word: cycle << 18 | wavefront << 6 | slot).
-__device__ void ack_sort(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
+__device__ void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
     const u32 bin = k & c.NWmask;
     const u32 n = c.ack_n[g];
     if (n == 0) return;
@@ -298,7 +298,7 @@ __device__ void ack_sort(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* 
 // or all go on to one single-feeder link, is cut into independent chunks of 32 pipe entries; any
 // other link stays one task (arrivals_link).  Ack discovery is cut into chunks of 32 bitmap words.
 // ---------------------------------------------------------------------------------------------
-__device__ void stage1_setup_gpu(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 lane) {
+__device__ void stage1_setup_gpu(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 lane) {
     u32 best = ASTRA_T_INF;                                     // earliest later window with acks pending (A7)
     for (u32 j = 1 + lane; j < c.NW; j += 32)
         if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
@@ -312,7 +312,7 @@ __device__ void stage1_setup_gpu(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 lane) {
     }
 }
 
-__device__ u32 stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
+__device__ u32 stage1_setup_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k, u32 t0) {
     const u32 e = c.in_link[i];
     u32* dcb = &c.due_cnt[(size_t)e * c.NW];
     const u32 n = ld_vol(&dcb[k & c.NWmask]);
@@ -345,7 +345,7 @@ __device__ u32 stage1_setup_link(Ctx& c, Ctl& ctl, u32 i, u32 k, u32 t0) {
 }
 
 // exclusive prefix of the per-link task counts (one warp); tbase[i_hi] = total
-__device__ void stage1_prefix(Ctx& c, Ctl& ctl, u32 lane) {
+__device__ void stage1_prefix(const Ctx& __restrict__ c, Ctl& ctl, u32 lane) {
     u32 carry = 0;
     for (u32 b = c.i_lo; b < c.i_hi; b += 32) {
         const u32 i = b + lane;
@@ -360,7 +360,7 @@ __device__ void stage1_prefix(Ctx& c, Ctl& ctl, u32 lane) {
 // 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3).
 // The set bits are first compacted into the warp's scratch so that every lane handles the same
 // number of acks whatever their spread over the words, four record loads in flight per lane.
-__device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32* scr, u32 lane) {
+__device__ void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32* scr, u32 lane) {
     const u32 CAP = 512;
     const u32 bin = k & c.NWmask;
     const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
@@ -438,7 +438,7 @@ __device__ void ack_chunk(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32
 }
 
 // 32 pipe entries of a link whose lines all terminate at its head GPU (R7 A1, deliveries)
-__device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 lane) {
+__device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
     const u32 ii = lo + chunk * 32 + lane;
     bool valid = (int32_t)(lo + n - ii) > 0;
@@ -486,11 +486,11 @@ __device__ void deliver_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0,
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
 // PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
 template <int PASS>
-__device__ void cells_half(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
 
 // A task is 64 entries: both halves' ring loads (and the look-back) are in flight before the first use.
 template <int PASS>
-__device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
+__device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
     const u32 i0 = lo + chunk * 64;
     const u64* ring = c.ring + c.ring_off[e];
@@ -512,7 +512,7 @@ __device__ void cells_chunk(Ctx& c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u
 }
 
 template <int PASS>
-__device__ void cells_half(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
     const u32 vmask = __ballot_sync(FULL, valid);
     if (!valid) return;
     const u32 grp = __match_any_sync(vmask, d);
@@ -561,7 +561,7 @@ __device__ void cells_half(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 f
 
 // 32 pipe entries of a link whose lines all go on to the single-feeder link lfwd[e] (R7 A1, transit):
 // stream order is FIFO order, so the position is the base plus the index in the stream
-__device__ void forward_chunk(Ctx& c, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
+__device__ void forward_chunk(const Ctx& __restrict__ c, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
     const u32 lo = c.tl_lo[e], n = c.tl_n[e];
     const u32 ii = lo + chunk * 32 + lane;
     if ((int32_t)(lo + n - ii) <= 0) return;
@@ -579,7 +579,7 @@ __device__ void forward_chunk(Ctx& c, u32 e, u32 chunk, u32 t0, u32 wlen, u32 la
 // A step's timestamp of kind `kind` was stamped at cycle `time` on GPU g: count down its
 // successors (R3, R10).  A successor whose last dependency this was is released at the max over
 // its dependencies' times and joins g's pending-release list.  Whole warp, warp-uniform p.
-__device__ __forceinline__ void on_event(Ctx& c, u32 g, u32 p, u32 kind, u32 time, u32 lane) {
+__device__ __forceinline__ void on_event(const Ctx& __restrict__ c, u32 g, u32 p, u32 kind, u32 time, u32 lane) {
     const u32 lo = c.succ_ptr[p], hi = c.succ_ptr[p + 1];
     for (u32 b = lo; b < hi; b += 32) {
         const u32 i = b + lane; bool ready = false; u32 s2 = 0;
@@ -607,7 +607,7 @@ __device__ __forceinline__ void on_event(Ctx& c, u32 g, u32 p, u32 kind, u32 tim
 // Walk wavefront (g, wf)'s in-order list from `cur` to the first entry that is not released by
 // cycle t or has quota for it (R11).  Returns true when quota was loaded (the wavefront wants to
 // issue).
-__device__ __forceinline__ bool wf_advance(Ctx& c, u32 g, u32 wf, u32& cur, u32& rem, u32 t) {
+__device__ __forceinline__ bool wf_advance(const Ctx& __restrict__ c, u32 g, u32 wf, u32& cur, u32& rem, u32 t) {
     const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
     rem = ASTRA_NOTLOADED;
     while (cur < end) {
@@ -623,7 +623,7 @@ __device__ __forceinline__ bool wf_advance(Ctx& c, u32 g, u32 wf, u32& cur, u32&
 // ---------------------------------------------------------------------------------------------
 // stage 2: release + issue of GPU g over [t0, t1)   (R10 - R13, slot return of R7 A3)
 // ---------------------------------------------------------------------------------------------
-__device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 ack_n = c.ack_n[g];
     const u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32* plist = c.plist + c.rel_off[g];
@@ -861,7 +861,7 @@ __device__ void issue_window(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u3
 // ---------------------------------------------------------------------------------------------
 
 // stage 2a: dependency events -> release times (R10); the set of wavefronts to look at; the mode.
-__device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
+__device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
     {
         const u32 nev = c.ev_cnt[g];
         for (u32 j = 0; j < nev; j++) {
@@ -917,7 +917,7 @@ __device__ void gpu_prepare(Ctx& c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
 // if the HBM budget never bound.  Issues go to the bucket of their cycle (first H of a cycle are
 // kept: more than H means the budget binds and the GPU-window is redone cycle-serially).  The new
 // wavefront state is written in place, the old one kept in the undo arrays for that case.
-__device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+__device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am0 = c.amask[(size_t)g * nwords + wi];
     if (am0 == 0) return;
@@ -1071,7 +1071,7 @@ __device__ void wf_sim(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u
 // issue of the window needs a slot -- one of the F0 slots free at the window start, else the
 // (i - F0)-th ack in cycle order -- and its step released, and comes at least one cycle after the
 // (i-1)-th: x_i = max(x_{i-1} + 1, c_i), a prefix maximum of c_j - j.  Same result as wf_sim.
-__device__ void wf_heavy(Ctx& c, Ctl& ctl, u32 g, u32 wf, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+__device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wf, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
     const u32 W = c.W, H = c.H, K = c.K, nwords = c.nwords;
     const u64 fullmask = c.fullmask;
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
@@ -1191,7 +1191,7 @@ __device__ void wf_heavy(Ctx& c, Ctl& ctl, u32 g, u32 wf, u32 k, u32 t0, u32 t1,
 }
 
 // The budget bound: put the wavefronts of GPU g back to their state at the window start.
-__device__ void wf_restore(Ctx& c, u32 g, u32 lane) {
+__device__ void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
     for (u32 wi = 0; wi < c.nwords; wi++) {
         const u32 am = c.amask[(size_t)g * c.nwords + wi];
         if (am == 0) continue;
@@ -1212,7 +1212,7 @@ __device__ void wf_restore(Ctx& c, u32 g, u32 lane) {
 // lower id are granted at t; occ[t] (the cnt array) holds the grants of all lower words, so the 32
 // wavefronts of a word step together through the cycles where one of them is ready and occ[t] < H,
 // a ballot giving the rank inside the word.  That rank is the bucket position of the issue.
-__device__ void wf_priority_word(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+__device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am = c.amask[(size_t)g * nwords + wi];
     if (am == 0) return;
@@ -1343,14 +1343,14 @@ __device__ void wf_priority_word(Ctx& c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0,
 // stage 2c: did the HBM budget bind in any cycle (R12)?  If not, the run stands: exclusive prefix of
 // the per-cycle counts (item enumeration), FIFO positions of every (direct out-link, cycle), new
 // tails, and the window's ack bits / released steps are consumed.
-__device__ bool gpu_binds(Ctx& c, u32 g, u32 wlen, u32 lane) {
+__device__ bool gpu_binds(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 lane) {
     const u32* cnt = c.cnt + (size_t)g * c.W;
     bool bind = false;
     for (u32 tt = lane; tt < wlen; tt += 32) if (cnt[tt] > c.H) bind = true;
     return __any_sync(FULL, bind);
 }
 
-__device__ void gpu_finalize(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
+__device__ void gpu_finalize(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
     const u32 W = c.W;
     u32* cnt = c.cnt + (size_t)g * W;
     u32 carry = 0;
@@ -1399,7 +1399,7 @@ __device__ void gpu_finalize(Ctx& c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane)
 // put each line where that rank says: FIFO position on a direct out-link, cell slot + injection
 // record on a multi-feeder one.  Item i of the window is entry i - cnt[tt] of the bucket of the
 // last cycle tt with cnt[tt] <= i (cnt = exclusive prefix of the per-cycle issue counts).
-__device__ void ev_place(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 t0, u32 cb, u32 lane) {
+__device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 t0, u32 cb, u32 lane) {
     const u32 nev = c.sel[(size_t)g * c.H];
     const u32 i = chunk * 32 + lane;
     const bool act = i < nev;
@@ -1444,7 +1444,7 @@ __device__ void ev_place(Ctx& c, Ctl& ctl, u32 g, u32 chunk, u32 t0, u32 cb, u32
 // stage 3a: FIFO positions of the cells of multi-feeder out-link o: exclusive prefix over the
 // cell popcounts of the window (R7/R8: cycle by cycle, slot order inside a cycle).
 // ---------------------------------------------------------------------------------------------
-__device__ void link_prefix(Ctx& c, u32 o, u32 wlen, u32 cb, u32 lane) {
+__device__ void link_prefix(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, u32 lane) {
     const u32 v = c.tail[o];
     const u32 mw = c.nd_mw[v];
     const u32* masks = c.masks + c.mask_off[o];
@@ -1465,7 +1465,7 @@ __device__ void link_prefix(Ctx& c, u32 o, u32 wlen, u32 cb, u32 lane) {
 
 // stage 3b: GPU g's recorded injections go to their FIFO positions; the ones that enter at the
 // first cycle of the next window stay recorded.
-__device__ void inject_place(Ctx& c, u32 g, u32 wlen, u32 cb, u32 lane) {
+__device__ void inject_place(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 cb, u32 lane) {
     const u32 n = c.inj_n[g];
     if (n == 0) return;
     u64* inj = c.inj_list + c.inj_off[g];
@@ -1497,7 +1497,7 @@ __device__ void inject_place(Ctx& c, u32 g, u32 wlen, u32 cb, u32 lane) {
 // ---------------------------------------------------------------------------------------------
 // stage 4: link e over [t0, t1): acceptance times of the whole FIFO (R9), arrival stamps.
 // ---------------------------------------------------------------------------------------------
-__device__ void link_service(Ctx& c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 wlen = t1 - t0;
     const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
     if (c.dirty[e]) {                                        // consume the cells of the window
