@@ -69,9 +69,10 @@ _BW_CHOICES = (64, 128, 256, 512, 1024, 2048)
 _ALGOS = ("ring", "direct", "dbt", "hd")
 
 
-def config4_point(point: int):
-    """Draw one design point of the config-4 sweep.  Draw order: topology bit, bandwidth,
-    latency, algorithm, message bytes (log-uniform), CUs, wavefronts/CU, outstanding cap."""
+def config4_params(point: int) -> dict:
+    """Draw the parameters of one design point of the config-4 sweep (no arrays are built).
+    Draw order: topology bit, bandwidth, latency, algorithm, message bytes (log-uniform), CUs,
+    wavefronts/CU, outstanding cap."""
     r = SplitMix64(config_seed(4, point))
     topo_kind = r.randint(0, 1)
     bw = _BW_CHOICES[r.randint(0, 5)]
@@ -84,7 +85,16 @@ def config4_point(point: int):
     cus = r.randint(8, 256)
     wpc = r.randint(1, 16)
     k = r.randint(4, 64)
-    topo = T.ring(16, bw, lat) if topo_kind == 0 else T.torus2d(4, 4, bw, lat)
+    return {"topo": "ring16" if topo_kind == 0 else "torus4x4", "bw_q8": bw, "latency": lat,
+            "algo": algo, "lines": m, "cus": cus, "wpc": wpc, "k": k}
+
+
+def config4_point(point: int):
+    """Build one design point of the config-4 sweep from its drawn parameters."""
+    meta = config4_params(point)
+    bw, lat, m, cus = meta["bw_q8"], meta["latency"], meta["lines"], meta["cus"]
+    topo = T.ring(16, bw, lat) if meta["topo"] == "ring16" else T.torus2d(4, 4, bw, lat)
+    algo = meta["algo"]
     if algo == "ring":
         coll, _ = C.ring_allreduce(16, m, cus)
     elif algo == "direct":
@@ -93,16 +103,15 @@ def config4_point(point: int):
         coll = C.double_binary_tree_allreduce(16, m, cus)
     else:
         coll = C.halving_doubling_allreduce(16, m, cus)
-    gpu = GpuCfg(cus, wpc, k, 32)       # H = 32 (fill)
-    meta = {"topo": "ring16" if topo_kind == 0 else "torus4x4", "bw_q8": bw, "latency": lat,
-            "algo": algo, "lines": m, "cus": cus, "wpc": wpc, "k": k}
+    gpu = GpuCfg(cus, meta["wpc"], meta["k"], 32)       # H = 32 (fill)
     return topo, coll, gpu, meta
 
 
-def config4(n_points: int = 4096, first: int = 0) -> Workload:
-    """Design-space sweep of 4096 seeded points on a 16-GPU ring / 4x4 torus."""
+def config4(n_points: int = 4096, first: int = 0, indices=None) -> Workload:
+    """Design-space sweep of 4096 seeded points on a 16-GPU ring / 4x4 torus (`indices`: only these
+    points of the sweep, in the order given)."""
     w = Workload(name="config4")
-    for p in range(first, first + n_points):
+    for p in (range(first, first + n_points) if indices is None else indices):
         topo, coll, gpu, meta = config4_point(p)
         w.topologies.append(topo)
         w.collectives.append(coll)

@@ -1,21 +1,28 @@
 #!/usr/bin/env python
-"""bench.py -- simulated 128 B cache-line transactions/sec of the CUDA engine on BASELINE config 2
-(8 GPUs on one switch, ring + direct all-reduce, 64 KiB .. 64 MiB, 22 design points in one batch).
+"""bench.py -- simulated 128 B cache-line transactions/sec and design points/sec of the CUDA engine on
+BASELINE config 4: the 4,096-point design-space sweep (16-GPU ring / 4x4 torus, ring / direct / double
+binary tree / halving-doubling all-reduce, 4 KiB .. 16 MiB), one batch, one kernel launch per step.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
 
-One "step" = one pass of the whole hot path (A0 excluded, A1-A8 included: state init, every
-simulated cycle, result write-out) over the 22-point batch.  `value` is measured with the tables
-resident in HBM (CUDA events on the launching stream); `e2e` goes through the C-ABI from host
-arrays: load_infragraph + load_collective + set_gpu + run_batch + read_results, host<->device
-copies included.  N > 1 (torchrun): every rank runs the same batch on its own GPU (the path
-shards by design point with no collective; weak scaling), time = max over ranks.
+One "step" = one pass of the whole hot path (A0 excluded, A1-A8 included: state init, every simulated
+lookahead window, result write-out) over the batch.  `value` is measured with the tables resident in
+HBM (CUDA events on the launching stream, 256 MiB L2 flush between iterations); `e2e` goes through the
+C-ABI from HOST arrays: load_infragraph + load_collective + set_gpu + run_batch + read_results, with
+the host<->device copies inside the timed region.
 
-`--impl reference` times the CPU oracle (oracle/) as it stands on the host cores.
+N > 1 (torchrun, one rank per GPU): the job is the first 4,096 x N points of the same seeded sweep,
+partitioned by paper_2606_10440_b200.shard (longest-first greedy, no collective on the data path), so
+per-GPU work stays fixed ("weak"); time = max over ranks, value = all ranks' transactions / that time.
+
+`other_workloads` carries configs 2, 3 and 5 at full size (>= 3 timed repeats each, same flush), with
+their own algorithmic bytes and roofline fraction.  `--impl reference` times the CPU oracle (oracle/)
+as it stands on the host cores on a bounded sample of the same workload.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -30,12 +37,13 @@ if ROOT not in sys.path:
 METRIC = "simulated_128B_cacheline_transactions_per_sec"
 UNIT = "transactions/s"
 BYTES_PER_TX_BASE, BYTES_PER_HOP = 72, 20          # SURVEY.md 8(d) algorithmic bytes per transaction
+POINTS_PER_GPU = 4096
 
 
-def get_workload(name: str):
+def get_workload(name: str, n_points: int = POINTS_PER_GPU, indices=None):
     from astra_inputs import configs
     if name == "config4":
-        return configs.config4(4096)
+        return configs.config4(n_points, indices=indices)
     return configs.by_name(name)
 
 
@@ -43,10 +51,44 @@ def measured_peak_gbs():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         try:
-            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def engine_source_sha256() -> str:
+    """Digest of the engine's sources: profiles/traffic.json is valid for exactly one such digest."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_10440_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cpp", ".h", ".cuh")):
+            h.update(f.encode()); h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()
+
+
+def profiled_traffic(workload_name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one astra_step_kernel launch from the committed
+    `ncu --set full` summary (profiles/traffic.json), or None when that capture was taken on other
+    engine sources than the ones running now."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        t = json.load(open(p))
+        if t.get("engine_source_sha256") == engine_source_sha256():
+            return t.get("dram_bytes_per_launch", {}).get(workload_name)
+    except Exception:
+        pass
+    return None
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 class ClockSampler(threading.Thread):
@@ -80,71 +122,137 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(sm)}
 
 
-def oracle_baseline(w, budget_s: float = 25.0):
-    """Time the oracle as it stands (plain scan, one design point per process) on a bounded sample:
-    the points of the workload in order of size until ~budget_s of CPU work."""
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline, --impl reference): the only places that execute oracle/
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(w, stride: int):
+    """A bounded, size-stratified sample of a workload's design points: every `stride`-th point in
+    index order (the sweep is seeded uniformly, so a stride keeps the size / parameter mix)."""
+    return list(range(0, w.n_points, max(1, stride)))
+
+
+def oracle_time(w, sample, cores: int):
     from oracle import oracle
     oracle.build()
-    cores = max(1, min(os.cpu_count() or 1, w.n_points))
-    order = sorted(range(w.n_points), key=lambda i: w.collectives[w.points[i][1]].total_lines)
-    # config 2 in full is ~11 s of single-core work; larger workloads are cut to the cheapest points
-    est, sample = 0.0, []
-    for i in order:
-        est += w.collectives[w.points[i][1]].total_lines / 2.5e6
-        sample.append(i)
-        if est > budget_s * cores:
-            break
     t0 = time.perf_counter()
-    res = oracle.run_workload(w, sample, processes=cores)
+    res = oracle.run_workload(w, sample, processes=cores)          # plain scan, one point per process
     dt = time.perf_counter() - t0
     lines = sum(r.total_lines for r in res)
-    return {"value": lines / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{len(sample)} of {w.n_points} design points of {w.name} ({lines} lines), plain scan, "
-                      f"one point per process, {dt:.2f} s wall",
-            "points_per_sec": len(sample) / dt, "seconds": dt}
+    return lines, dt
+
+
+def oracle_baseline(w, stride_all: int, stride_one: int):
+    """The oracle as it stands (plain scan) on the box's host cores: all cores with one design point per
+    process, and one core, each on a bounded sample of the same workload."""
+    cores = max(1, min(os.cpu_count() or 1, 64))
+    sa = oracle_sample(w, stride_all)
+    lines_a, dt_a = oracle_time(w, sa, min(cores, len(sa)))
+    s1 = oracle_sample(w, stride_one)
+    lines_1, dt_1 = oracle_time(w, s1, 1)
+    return {"value": lines_a / dt_a, "unit": UNIT, "cores": min(cores, len(sa)), "kind": "oracle",
+            "sample": f"every {stride_all}th design point of {w.name}: {len(sa)} of {w.n_points} points, {lines_a} "
+                      f"transactions, plain scan, one point per process, {dt_a:.2f} s wall",
+            "design_points_per_sec": len(sa) / dt_a,
+            "one_core": {"value": lines_1 / dt_1, "unit": UNIT, "design_points_per_sec": len(s1) / dt_1,
+                         "sample": f"every {stride_one}th point: {len(s1)} points, {lines_1} transactions, {dt_1:.2f} s"},
+            "cpu_model": cpu_model(), "host_cores": os.cpu_count(), "seconds": dt_a}
+
+
+def strides_for(w):
+    # config 4: 4,096 points, ~1.95 G transactions; the plain-scan oracle does ~1.5 M transactions/s/core
+    if w.n_points >= 1024:
+        return 16, 256
+    return 1, max(1, w.n_points // 4)
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     w = get_workload(args.workload)
-    runs = []
-    for _ in range(args.warmup and 1):
-        oracle_baseline(w, budget_s=2.0)
-    for _ in range(max(1, args.steps)):
-        runs.append(oracle_baseline(w, budget_s=20.0 / max(1, args.steps)))
-    dt = sum(r["seconds"] for r in runs) / len(runs)
-    val = sum(r["value"] for r in runs) / len(runs)
-    base = dict(runs[-1]); base["value"] = val
+    sa, _ = strides_for(w)
+    stride = sa * 4 if w.n_points >= 1024 else 1        # each step a bounded sample (~3-5 s on 16 cores)
+    sample = oracle_sample(w, stride)
+    cores = max(1, min(os.cpu_count() or 1, len(sample), 64))
+    for _ in range(1 if args.warmup else 0):
+        oracle_time(w, sample[:cores], cores)
+    runs = [oracle_time(w, sample, cores) for _ in range(max(1, args.steps))]
+    lines = runs[0][0]
+    dt = sum(r[1] for r in runs) / len(runs)
+    val = lines / dt
+    desc = (f"every {stride}th design point of {w.name}: {len(sample)} of {w.n_points} points, {lines} transactions per "
+            f"step, plain scan, one point per process")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-        "config": {"workload": w.name, "design_points": w.n_points, "sample": base["sample"]},
-        "cpu_baseline": base,
+        "config": {"workload": w.name, "design_points": w.n_points, "sample": desc},
+        "design_points_per_sec": len(sample) / dt,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "cpu_model": cpu_model(), "host_cores": os.cpu_count()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
-def extra_workloads(device, stream):
-    """Context, not the headline: the other BASELINE configs at full size, one warm-up and one timed
-    run each, device time of the engine's launch (CUDA events on its stream)."""
+# ---------------------------------------------------------------------------------------------
+# engine legs
+# ---------------------------------------------------------------------------------------------
+def algorithmic_bytes(eng, n_points: int, total_lines: int) -> int:
+    hops = 0
+    for i in range(n_points):
+        hops += int(eng.read_results(i, False, True)[2].sum())
+    return BYTES_PER_TX_BASE * total_lines + BYTES_PER_HOP * hops
+
+
+def check_closed_forms(w, summaries):
+    """Bench-path spot check against closed forms that hold for the workload (no oracle call here):
+    config 2 ring points 14(350 + ceil(n/4)) + 350."""
+    if w.name != "config2":
+        return
+    for s, m in zip(summaries, w.meta):
+        if m["algo"] == "ring":
+            n = m["lines"] // 8
+            assert s.completion_cycle == 14 * (350 + -(-n // 4)) + 350, "config 2 ring closed form violated"
+
+
+def time_workload(eng, pts, w, stream, flush, steps: int):
+    """`steps` timed launches with an L2 flush before each; device time per launch from the engine's own
+    CUDA events on its stream."""
+    ms = []
+    for _ in range(steps):
+        flush.zero_()
+        eng.run_batch(pts, w.max_cycles, asynchronous=True)
+        eng.sync()
+        ms.append(eng.last_run_info()[0])
+    return ms
+
+
+def extra_workloads(device, stream, flush, peak):
+    """Configs 2, 3, 5 at full size: one preparing run, one warm-up, three timed repeats with the L2
+    flush; device time of the engine's launch, algorithmic bytes from the run's own link counts."""
+    import numpy as np
     from astra_inputs import configs
     from paper_2606_10440_b200 import Engine
     out = {}
-    for name, make in (("config3", configs.config3), ("config4", lambda: configs.config4(4096)), ("config5", configs.config5)):
+    for name, make in (("config2", configs.config2), ("config3", configs.config3), ("config5", configs.config5)):
         w = make()
         with Engine(device) as eng:
             eng.set_stream(stream.cuda_stream)
             pts = eng.load_workload(w)
             eng.run_batch(pts, w.max_cycles)
-            eng.run_batch(pts, w.max_cycles)
-            ms = eng.last_run_info()[0]
-            ok = all(eng.read_results(i, False, False)[0].status == 0 for i in range(len(pts)))
-        out[name] = {"design_points": w.n_points, "transactions": w.total_lines(), "kernel_ms": ms,
-                     "transactions_per_sec": w.total_lines() / (ms * 1e-3), "design_points_per_sec": w.n_points / (ms * 1e-3),
-                     "all_points_finished": ok}
+            summ = [eng.read_results(i, False, False)[0] for i in range(len(pts))]
+            ok = all(s.status == 0 for s in summ)
+            check_closed_forms(w, summ)
+            alg = algorithmic_bytes(eng, len(pts), w.total_lines())
+            time_workload(eng, pts, w, stream, flush, 1)
+            ms = time_workload(eng, pts, w, stream, flush, 3)
+        k_ms = float(np.mean(ms))
+        ach = alg / (k_ms * 1e-3) / 1e9
+        out[name] = {"design_points": w.n_points, "transactions": w.total_lines(), "kernel_ms": k_ms, "kernel_ms_runs": ms,
+                     "transactions_per_sec": w.total_lines() / (k_ms * 1e-3),
+                     "design_points_per_sec": w.n_points / (k_ms * 1e-3), "all_points_finished": ok,
+                     "algorithmic_bytes_per_launch": alg,
+                     "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                                  "traffic": profiled_traffic(name)}}
     return out
 
 
@@ -162,15 +270,42 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    from paper_2606_10440_b200 import Engine, build as engine_build
+    from paper_2606_10440_b200 import Engine, build as engine_build, shard
     engine_build.build()
-    w = get_workload(args.workload)
+
+    # ---- this rank's share of the job (N = 1: the whole config) ----
+    if world > 1 and args.workload == "config4":
+        from astra_inputs import configs
+        n_job = POINTS_PER_GPU * world
+        costs = [float(configs.config4_params(i)["lines"]) for i in range(n_job)]
+        mine = shard.shard_points(costs, world)[rank]
+        w = get_workload("config4", indices=mine)
+
+        class job:                       # what run_sharded needs to know about the whole job
+            n_points = n_job
+    else:
+        n_job = None
+        w = get_workload(args.workload)          # single-point configs: replicas only
     total_lines = w.total_lines()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    def allsum(x):
+        if world == 1:
+            return x
+        t = torch.tensor([float(x)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def allmax(x):
+        if world == 1:
+            return x
+        t = torch.tensor([float(x)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
 
     stream = torch.cuda.Stream()            # a real (non-default) stream shared by torch and the engine
     torch.cuda.set_stream(stream)
@@ -180,14 +315,10 @@ def run_ours(args):
     eng.set_stream(stream.cuda_stream)
     pts = eng.load_workload(w)
     eng.run_batch(pts, w.max_cycles)                                     # prepares the batch (A0) + 1 run
-    # ---- correctness spot check against stored closed forms (no oracle call on this path) ----
     summ = [eng.read_results(i, False, False)[0] for i in range(len(pts))]
     assert all(s.status == 0 for s in summ), "a design point did not finish"
-    hops_lines = 0
-    for i in range(len(pts)):
-        _, _, ll = eng.read_results(i, False, True)
-        hops_lines += int(ll.sum())
-    alg_bytes = BYTES_PER_TX_BASE * total_lines + BYTES_PER_HOP * hops_lines
+    check_closed_forms(w, summ)
+    alg_bytes = algorithmic_bytes(eng, len(pts), total_lines)
     busy = sum(s.busy_cycles for s in summ)
 
     for _ in range(max(0, args.warmup - 1)):
@@ -196,77 +327,74 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    kernel_ms = []
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record(stream)
-    for _ in range(args.steps):
-        flush.zero_()                                                    # L2 flush between iterations
-        eng.run_batch(pts, w.max_cycles, asynchronous=True)
-        eng.sync()
-        kernel_ms.append(eng.last_run_info()[0])
+    kernel_ms = time_workload(eng, pts, w, stream, flush, args.steps)    # L2 flush before every launch
     ev1.record(stream)
     barrier()
     clocks = sampler.stop()
-    total_ms = ev0.elapsed_time(ev1)
-    if world > 1:
-        tt = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
-    ms_per_step = total_ms / args.steps
-    value = world * total_lines / (ms_per_step * 1e-3)
+    ms_per_step = allmax(ev0.elapsed_time(ev1)) / args.steps
+    job_lines = allsum(total_lines)
+    job_points = allsum(w.n_points)
+    value = job_lines / (ms_per_step * 1e-3)
     k_ms = float(np.mean(kernel_ms))
     _, launches, dev_bytes = eng.last_run_info()
     eng.close()
 
-    # ---- end to end through the C-ABI from host arrays ----
+    # ---- end to end through the C-ABI from host arrays (sharded at N > 1) ----
+    def simulate(wl, indices):
+        with Engine(local_rank) as e2:
+            p2 = e2.load_workload(wl)
+            e2.run_batch([p2[i] for i in indices], wl.max_cycles)
+            res = [e2.read_results(i) for i in range(len(indices))]
+            simulate.bytes = e2.last_transfer_bytes()
+        return [(r[0].status, r[0].completion_cycle) for r in res]
+
     e2e_times = []
-    h2d = d2h = 0
-    for it in range(min(3, max(1, args.steps))):
+    for _ in range(min(3, max(1, args.steps))):
         barrier()
         t0 = time.perf_counter()
-        with Engine(local_rank) as e2:
-            p2 = e2.load_workload(w)
-            e2.run_batch(p2, w.max_cycles)
-            outs = [e2.read_results(i) for i in range(len(p2))]
-            h2d, d2h = e2.last_transfer_bytes()
+        if n_job:       # the N > 1 path: shard.run_sharded partitions, runs this rank's share, gathers every point's result
+            outs = shard.run_sharded(job, lambda _job, idx: simulate(w, range(len(idx))), rank, world, costs=costs)
+        else:
+            outs = simulate(w, range(w.n_points))
         torch.cuda.synchronize()
         e2e_times.append(time.perf_counter() - t0)
-        assert all(o[0].status == 0 for o in outs)
-    e2e_s = min(e2e_times)
-    if world > 1:
-        tt = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+        assert all(o[0] == 0 for o in outs)
+    e2e_s = allmax(min(e2e_times))
+    h2d, d2h = simulate.bytes
 
     peak, peak_src = measured_peak_gbs()
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-    # dram__bytes_read.sum + dram__bytes_write.sum of one astra_step_kernel launch, `ncu --set full` capture
-    # summarised in profiles/r01_v7_ncu.md (config 2 only; other workloads were not captured)
-    traffic = {"config2": 34919936}.get(w.name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64", "data": "synthetic",
-        "config": {"workload": w.name, "design_points": w.n_points, "transactions_per_step": total_lines,
+        "config": {"workload": w.name, "design_points": int(job_points), "transactions_per_step": int(job_lines),
                    "l2": "256 MiB device write between timed iterations (inside the timed region)",
-                   "parallelism": f"design points x {world} GPU(s), no collective"},
-        "design_points_per_sec": world * w.n_points / (ms_per_step * 1e-3),
+                   "parallelism": (f"design points sharded over {world} GPU(s) by shard.shard_points, no collective"
+                                   if n_job else f"{world} replica(s)")},
+        "design_points_per_sec": job_points / (ms_per_step * 1e-3),
         "gpu_launches": launches * args.steps,
         "clocks": clocks,
-        "e2e": {"value": world * total_lines / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h), "seconds_per_step": e2e_s},
+        "e2e": {"value": job_lines / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h), "seconds_per_step": e2e_s,
+                "design_points_per_sec": job_points / e2e_s},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "kernel": "astra_step_kernel", "kernel_ms": k_ms,
+                     "traffic": profiled_traffic(w.name), "kernel": "astra_step_kernel", "kernel_ms": k_ms,
                      "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src,
-                     "note": "bytes = 72 per transaction + 20 per link hop (SURVEY 8(d)); state stays in L2/shared memory at "
-                             "this size, the kernel is bound by the dependent chain per lookahead window, see DESIGN.md section 6",
+                     "note": "bytes = 72 per transaction + 20 per link hop (SURVEY 8(d)), rank 0's launch; the live state "
+                             "of a design point sits in shared memory / L2, the kernel is bound by the dependent chain per "
+                             "lookahead window, see DESIGN.md section 6; traffic is null unless profiles/traffic.json was "
+                             "captured on these engine sources",
                      "node_cycles_stepped": busy, "device_bytes": dev_bytes},
     }
     if rank == 0 and world == 1 and not args.no_extras:
-        line["other_workloads"] = extra_workloads(local_rank, stream)
+        line["other_workloads"] = extra_workloads(local_rank, stream, flush, peak)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = {k: v for k, v in oracle_baseline(w).items() if k != "seconds"}
+        sa, s1 = strides_for(w)
+        line["cpu_baseline"] = {k: v for k, v in oracle_baseline(w, sa, s1).items() if k != "seconds"}
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -279,9 +407,9 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--workload", default="config4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-extras", action="store_true", help="skip the one-shot runs of configs 3, 4, 5")
+    ap.add_argument("--no-extras", action="store_true", help="skip the timed runs of configs 2, 3, 5")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

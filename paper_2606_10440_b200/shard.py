@@ -36,12 +36,14 @@ def shard_points(costs: Sequence[float], world_size: int) -> List[List[int]]:
     return shards
 
 
-def run_sharded(workload, simulate, rank: int, world_size: int, gather=None):
+def run_sharded(workload, simulate, rank: int, world_size: int, gather=None, costs=None):
     """Run this rank's share of `workload` through `simulate(workload, indices) -> list of per-point
     results` and gather all shares.  `gather(obj) -> list of one obj per rank` defaults to
     torch.distributed.all_gather_object on the default process group (world_size > 1).
+    `costs` (one per point) replaces point_costs(workload); `workload` then only needs `n_points`,
+    so a rank can build just its own points inside `simulate`.
     Returns the results of ALL points in workload order (on every rank)."""
-    shards = shard_points(point_costs(workload), world_size)
+    shards = shard_points(point_costs(workload) if costs is None else costs, world_size)
     mine = shards[rank]
     local = simulate(workload, mine) if mine else []
     if len(local) != len(mine):

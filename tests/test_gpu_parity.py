@@ -37,6 +37,18 @@ def test_p2_p3():
     check_workload(_single(T.line(2, 1024, 7), C.single_transfer(2, 0, 1, 10, 0, 2), GpuCfg(2, 4, 64, 8)))
 
 
+@pytest.mark.parametrize("key", __import__("tests.pin_cases", fromlist=["ROUND2"]).ROUND2)
+def test_round2_hand_traces(key):
+    """Grant order when H binds, general-credit bandwidths, ISSUED/ACKED release timing: the engine
+    against the oracle AND against the hand-derived values of the golden file."""
+    from tests import pin_cases
+    topo, coll, gpu = pin_cases.build(key)
+    res, _ = check_workload(_single(topo, coll, gpu, name=key))
+    g = pin_cases.GOLD[key]
+    want = g["step_ts"] if isinstance(g["step_ts"][0], list) else [g["step_ts"]]
+    assert res[0][1].tolist() == want
+
+
 def test_config1_bit_exact_and_pin():
     gpu, _ = check_workload(configs.config1())
     assert gpu[0][0].completion_cycle == 38623          # SURVEY 8(c) P4

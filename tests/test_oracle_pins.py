@@ -204,3 +204,30 @@ def test_routing_fat_tree_d_mod_k():
     for d in range(8, 64):
         assert int(topo.head[nl[leaf0, d]]) == spine0 + d % 4
     assert int(dist[0, 9]) == 4000 and int(dist[0, 1]) == 350 and int(dist[0, 8]) == 4000
+
+
+# ---- round 2: hand traces for the rules the pins above leave open (derivations in the golden file) ----
+from tests import pin_cases
+
+
+@pytest.mark.parametrize("key", pin_cases.ROUND2)
+def test_round2_hand_traces(key):
+    """R12 grant order when H binds (lowest ready wavefront id first), R9 saturating
+    credit at bandwidths that are neither integer nor 1/P, R10 release timing of ISSUED- and
+    ACKED-kind dependencies.  Expected values are hand-derived (golden file, 'derivation')."""
+    g = GOLD[key]
+    topo, coll, gpu = pin_cases.build(key)
+    r = oracle.run_point(topo, coll, gpu, trace_cap=10000)
+    assert r.status == 0
+    want = g["step_ts"] if isinstance(g["step_ts"][0], list) else [g["step_ts"]]
+    assert r.step_ts.tolist() == want
+    if "link_lines" in g:
+        assert r.link_lines.tolist() == g["link_lines"]
+    if "issue_cycle_wavefront" in g:
+        got = [[int(x[0]), int(x[3]) & 0xffff] for x in r.trace if int(x[1]) == oracle.TR_ISSUE]
+        assert got == g["issue_cycle_wavefront"]
+    if "accept" in g:
+        assert _times(r, oracle.TR_ACCEPT) == g["accept"]
+    # the pruned scan takes the same decisions
+    r2 = oracle.run_point(topo, coll, gpu, flags=oracle.FLAG_PRUNED_SCAN)
+    assert (r2.step_ts == r.step_ts).all()
