@@ -25,6 +25,12 @@
  *   - Results are copied into caller-allocated host buffers.
  *   - astra_ctx owns all host and device memory it allocates; astra_destroy frees it.  One ctx is
  *     not thread-safe; separate ctxs are independent.  Loaded objects live until astra_destroy.
+ *   - A batch runs as ONE cooperative kernel launch whose CTAs wait on each other (one CTA group per
+ *     large design point): the CUDA runtime either makes the whole grid resident or refuses the
+ *     launch.  While another kernel (another ctx, another stream, another process under MPS)
+ *     occupies SMs, astra_run_batch may therefore fail with ASTRA_ELIMIT / ASTRA_ECUDA instead of
+ *     running; it never hangs: group barriers give up after a few seconds without progress and the
+ *     call returns ASTRA_ECUDA.
  *   - Every call returns 0 or a negative ASTRA_E* code and never throws or aborts;
  *     astra_last_error gives a message valid until the next call on the same ctx.
  *   - There is no CPU fallback: without a usable CUDA device astra_create fails with ASTRA_ECUDA.
@@ -54,7 +60,10 @@ extern "C" {
 #define ASTRA_MAX_GPUS             65535u
 #define ASTRA_MAX_LINK_LATENCY     (1u << 24) /* latency + node_latency           */
 #define ASTRA_MAX_BW_Q8            (31u * 256u) /* at most 31 lines/cycle per link */
-#define ASTRA_MAX_HBM_LINES        1024u
+#define ASTRA_MAX_HBM_LINES        1023u      /* hbm_lines_per_cycle (10-bit slot index inside a cycle's cell) */
+#define ASTRA_MAX_CYCLES           (0xffffffffull - (1ull << 25)) /* cycle counters are 32 bits on the device:
+                                                 astra_run_batch CLAMPS max_cycles to this value, so a run that
+                                                 needs more cycles reports ASTRA_STATUS_MAX_CYCLES at this cycle */
 
 /* Dependency kinds: which timestamp of the producer step the consumer waits for (R3). */
 #define ASTRA_DEP_DELIVERED 0    /* producer's last line reached its dst;  needs dst(p)   == owner(s) */
@@ -69,7 +78,8 @@ extern "C" {
 #define ASTRA_FLAG_NO_HEAVY        16ull  /* no warp-per-wavefront issue path (testing)         */
 #define ASTRA_FLAG_NO_PRIORITY_SWEEP 32ull /* budget-bound windows take the cycle-serial path (testing) */
 #define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
-#define ASTRA_FLAG_DIAG_RANK(r) (((uint64_t)(r) & 0xfull) << 16) /* which CTA of a group reports astra_read_diag */
+#define ASTRA_FLAG_WARPS(w) (((uint64_t)(w) & 0x3full) << 20) /* CTA shape: w in {1,2,4,8,16} warps per CTA, 16/w CTAs per SM
+                                            (0 = engine's choice) */
 #define ASTRA_FLAG_GROUP(g) (((uint64_t)(g) & 0xffull) << 8) /* run every design point on a group of g
                                             CTAs (1..255, at most the co-resident CTAs of the device), one node range each; 0 = engine's choice */
 
@@ -139,7 +149,7 @@ int32_t astra_set_gpu(astra_ctx* ctx, uint32_t cus, uint32_t wavefronts_per_cu,
                       uint32_t max_outstanding, uint32_t hbm_lines_per_cycle, uint32_t* out_gpu_id);
 
 /* Simulate n_points independent design points, each from t = 0 with empty queues (R1), until
- * every step is acked (R14) or cycle max_cycles is reached.  Synchronous: returns when the
+ * every step is acked (R14) or cycle max_cycles (clamped to ASTRA_MAX_CYCLES) is reached.  Synchronous: returns when the
  * results are ready on the device.  EINVAL when a point's collective and topology disagree on
  * n_gpus or a CU range exceeds the GPU's CUs; EUNREACHABLE when a step has no route. */
 int32_t astra_run_batch(astra_ctx* ctx, uint32_t n_points, const astra_point* points,
@@ -159,13 +169,17 @@ int32_t astra_sync(astra_ctx* ctx);
 int32_t astra_read_results(astra_ctx* ctx, uint32_t point, astra_summary* out,
                            uint64_t* step_ts, uint64_t* link_lines);
 
-/* Diagnostics of design point `point` of the last batch, out16[16]: [0] lookahead windows stepped,
- * [1..4] SM clocks the point's first CTA spent in the stages of a window (arrivals + ack gather,
- * release + issue, multi-feeder merge, link service + next-non-idle decision), [5] SM clocks of
- * state initialisation, [6] GPU-windows that took the cycle-serial issue path, [8..12] SM clocks of
- * the parts of stage 2 (prepare, wavefront runs, check + cycle-serial path, placement), [13] SM clocks
- * waiting at the group barrier.  Same errors as astra_read_results. */
-int32_t astra_read_diag(astra_ctx* ctx, uint32_t point, uint64_t* out16);
+/* Diagnostics (libraries built with -DASTRA_DIAG only, ESTATE otherwise; the default build carries no
+ * instrumentation): SM clocks of CTA `cta_rank` of the group that ran design point `point` of the last
+ * batch.  out144[144]: [0] lookahead windows stepped, [5] state initialisation, [6] budget-bound
+ * GPU-windows; then for each of the CTA's 16 warp sets s (a set steps one simulated node at a time)
+ * eight counters at [16 + 8 s ..]: arrivals + ack discovery, release events, wavefront runs, budget check /
+ * commit / cycle-serial path, placement, multi-feeder merge, link service, wait at the end-of-window barrier
+ * -- clocks of the set's first warp, summed over the set's nodes and all windows. */
+int32_t astra_read_diag(astra_ctx* ctx, uint32_t point, uint32_t cta_rank, uint64_t* out144);
+
+/* Number of CTAs the engine assigned to design point `point` of the prepared batch (1 = one CTA). */
+int32_t astra_point_group(astra_ctx* ctx, uint32_t point, uint32_t* group);
 
 /* Diagnostics: device milliseconds (CUDA events on the ctx's stream) of the last batch and the
  * number of kernels it launched; bytes of device memory held by the prepared batch. */

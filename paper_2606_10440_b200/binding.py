@@ -10,13 +10,14 @@ from typing import List, Optional, Sequence, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "libastra_b200.so")
+# ASTRA_DIAG=1 in the environment selects the instrumented build (build.build(diag=True)); diagnostics only
+_LIBPATH = os.path.join(_HERE, "libastra_b200_diag.so" if os.environ.get("ASTRA_DIAG") == "1" else "libastra_b200.so")
 
 EXPORTED_SYMBOLS = [
     "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",
     "astra_load_infragraph", "astra_load_collective", "astra_set_gpu",
     "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
-    "astra_last_run_info", "astra_last_transfer_bytes", "astra_read_diag",
+    "astra_last_run_info", "astra_last_transfer_bytes", "astra_read_diag", "astra_point_group",
 ]
 
 FLAG_NO_WINDOW_SKIP = 1
@@ -27,9 +28,9 @@ FLAG_NO_HEAVY = 16             # testing: no warp-per-wavefront path
 FLAG_NO_PRIORITY_SWEEP = 32    # testing: budget-bound windows on the cycle-serial path
 
 
-def FLAG_DIAG_RANK(r: int) -> int:
-    """ASTRA_FLAG_DIAG_RANK(r): which CTA of a group reports astra_read_diag."""
-    return (r & 0xF) << 16
+def FLAG_WARPS(w: int) -> int:
+    """ASTRA_FLAG_WARPS(w): w warps per CTA, 16 / w CTAs per SM."""
+    return (w & 0x3F) << 20
 
 
 def FLAG_GROUP(g: int) -> int:
@@ -95,7 +96,8 @@ def load_library(path: Optional[str] = None):
     lib.astra_run_batch_async.argtypes = [vp, u32, vp, u64]
     lib.astra_sync.argtypes = [vp]
     lib.astra_read_results.argtypes = [vp, u32, ctypes.POINTER(_Summary), vp, vp]
-    lib.astra_read_diag.argtypes = [vp, u32, vp]
+    lib.astra_read_diag.argtypes = [vp, u32, u32, vp]
+    lib.astra_point_group.argtypes = [vp, u32, ctypes.POINTER(u32)]
     lib.astra_last_run_info.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u32), ctypes.POINTER(u64)]
     lib.astra_last_transfer_bytes.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     for name in EXPORTED_SYMBOLS:
@@ -202,10 +204,15 @@ class Engine:
                 step_ts[:4 * s.n_steps].reshape(s.n_steps, 4) if want_steps else None,
                 link_lines[:s.n_links] if want_links else None)
 
-    def read_diag(self, point: int) -> np.ndarray:
-        out = np.zeros(16, dtype=np.uint64)
-        self._check(self._lib.astra_read_diag(self._ctx, point, _ptr(out)))
+    def read_diag(self, point: int, cta_rank: int = 0) -> np.ndarray:
+        out = np.zeros(144, dtype=np.uint64)
+        self._check(self._lib.astra_read_diag(self._ctx, point, cta_rank, _ptr(out)))
         return out
+
+    def point_group(self, point: int) -> int:
+        g = ctypes.c_uint32()
+        self._check(self._lib.astra_point_group(self._ctx, point, ctypes.byref(g)))
+        return g.value
 
     def last_run_info(self):
         ms, n, b = ctypes.c_float(), ctypes.c_uint32(), ctypes.c_uint64()

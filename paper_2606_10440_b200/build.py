@@ -7,6 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libastra_b200.so")
+LIB_DIAG = os.path.join(_HERE, "libastra_b200_diag.so")      # same sources with -DASTRA_DIAG (per-stage clocks)
 SOURCES = ["astra_engine.cu", "astra_loader.cpp", "astra_api.cpp"]
 HEADERS = ["astra_internal.h", os.path.join("..", "..", "include", "astra.h")]
 
@@ -21,29 +22,33 @@ def _nvcc() -> str:
     return "nvcc"
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
+def needs_build(lib: str = LIB) -> bool:
+    if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(LIB)
+    t = os.path.getmtime(lib)
     deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
-        return LIB
+def build(force: bool = False, verbose: bool = False, diag: bool = False) -> str:
+    """The product library (default), or the instrumented one (diag=True: -DASTRA_DIAG adds per-stage SM
+    clock counters read by astra_read_diag; never used for a timing that is reported as a result)."""
+    lib = LIB_DIAG if diag else LIB
+    if not force and not needs_build(lib):
+        return lib
     objs = []
     for s in SOURCES:
-        o = os.path.join(CSRC, os.path.splitext(s)[0] + ".o")
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        o = os.path.join(CSRC, os.path.splitext(s)[0] + (".diag.o" if diag else ".o"))
+        cmd = [_nvcc()] + NVCC_FLAGS + (["-DASTRA_DIAG"] if diag else []) + (["-Xptxas", "-v"] if verbose else []) + \
               ["-x", "cu", "-c", os.path.join(CSRC, s), "-o", o]
         subprocess.check_call(cmd)
         objs.append(o)
-    tmp = LIB + f".tmp{os.getpid()}"
+    tmp = lib + f".tmp{os.getpid()}"
     subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose=True))
+    import sys
+    print(build(force=True, verbose=True, diag="--diag" in sys.argv))

@@ -216,13 +216,20 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     CUDA_TRY(c, cudaGetDevice(&dev), "cudaGetDevice");
     CUDA_TRY(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "device attribute");
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev), "device attribute");
+    // CTA shape: 16 warps, one CTA per SM -- or, with ASTRA_FLAG_WARPS(w), 16 / w CTAs of w warps per SM
+    // (128 registers per thread; the shared memory of the SM is split evenly between them)
     c->warps = 16;
+    { const u32 wf = (u32)((c->flags >> 20) & 0x3f); if (wf == 1 || wf == 2 || wf == 4 || wf == 8 || wf == 16) c->warps = wf; }
+    const u32 ctas_per_sm = 16 / c->warps;
     std::vector<double> cost; std::vector<uint8_t> big;
-    classify(c, n, pts, (u32)sms, cost, big, &c->group);
+    classify(c, n, pts, (u32)sms * ctas_per_sm, cost, big, &c->group);
     PlanOptions opt;
-    opt.flags = c->flags & 0xf00ffull; opt.max_cycles = max_cycles;
+    opt.flags = c->flags & 0xffull; opt.max_cycles = max_cycles;
     const u32 fixed = astra_engine_fixed_smem(c->warps);
-    opt.hot_budget = (u32)smem_max > fixed + 1024 ? (u32)smem_max - fixed - 1024 : 0;
+    int smem_sm = 0;
+    CUDA_TRY(c, cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev), "device attribute");
+    const u32 smem_cta = std::min<u32>((u32)smem_max, (u32)smem_sm / ctas_per_sm - 1024);    // 1 KB per CTA is reserved by the system
+    opt.hot_budget = smem_cta > fixed + 1024 ? smem_cta - fixed - 1024 : 0;
     u32 hot_max = 0, n_big = 0;
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];
@@ -252,7 +259,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         P.r_step_ts = roff; roff += 32ull * P.S;
         P.r_link_lines = roff; roff += 8ull * P.E;
         P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
-        P.r_diag = roff; roff += 128;
+        P.r_diag = roff; roff += 8ull * ASTRA_DIAG_WORDS * P.group;      // per CTA of the group (written by ASTRA_DIAG builds)
         if (big[i]) { ws_big_max = std::max(ws_big_max, P.ws_bytes); n_big++; }
         else ws_single_max = std::max(ws_single_max, P.ws_bytes);
         hot_max = std::max(hot_max, P.hot_bytes);
@@ -349,6 +356,11 @@ extern "C" int32_t astra_sync(astra_ctx* c) {
     CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
     CUDA_TRY(c, cudaStreamSynchronize(c->stream), "kernel execution");
     CUDA_TRY(c, cudaEventElapsedTime(&c->last_ms, c->ev0, c->ev1), "event elapsed");
+    if (c->d_queue && c->last_launches) {           // did a group barrier time out (kernel-wide abort flag)?
+        u32 q[4] = {0, 0, 0, 0};
+        CUDA_TRY(c, cudaMemcpy(q, c->d_queue, sizeof(q), cudaMemcpyDeviceToHost), "D2H queue");
+        if (q[2]) return fail(c, ASTRA_ECUDA, "a CTA group barrier timed out: the batch was abandoned");
+    }
     c->ran = true;
     return ASTRA_OK;
 }
@@ -385,12 +397,22 @@ extern "C" int32_t astra_read_results(astra_ctx* c, uint32_t point, astra_summar
     return ASTRA_OK;
 }
 
-extern "C" int32_t astra_read_diag(astra_ctx* c, uint32_t point, uint64_t* out16) {
+extern "C" int32_t astra_read_diag(astra_ctx* c, uint32_t point, uint32_t cta_rank, uint64_t* out144) {
     if (!c) return ASTRA_EINVAL;
-    if (!out16) return fail(c, ASTRA_EINVAL, "null argument");
+    if (!out144) return fail(c, ASTRA_EINVAL, "null argument");
+    if (!astra_engine_has_diag()) return fail(c, ASTRA_ESTATE, "this library was built without ASTRA_DIAG");
     int32_t rc = astra_read_results(c, point, nullptr, nullptr, nullptr);
     if (rc) return rc;
-    std::memcpy(out16, c->h_results.data() + c->descs[point].r_diag, 128);
+    if (cta_rank >= c->descs[point].group) return fail(c, ASTRA_ESTATE, "cta_rank beyond the point's CTA group");
+    std::memcpy(out144, c->h_results.data() + c->descs[point].r_diag + 8ull * ASTRA_DIAG_WORDS * cta_rank, 8ull * ASTRA_DIAG_WORDS);
+    return ASTRA_OK;
+}
+
+extern "C" int32_t astra_point_group(astra_ctx* c, uint32_t point, uint32_t* group) {
+    if (!c) return ASTRA_EINVAL;
+    if (!group) return fail(c, ASTRA_EINVAL, "null argument");
+    if (!c->prepared || point >= c->descs.size()) return fail(c, ASTRA_ESTATE, "no such point in the prepared batch");
+    *group = c->descs[point].group;
     return ASTRA_OK;
 }
 

@@ -39,10 +39,10 @@
 #include <cuda_runtime.h>
 
 #define FULL 0xffffffffu
-#define SCR_WORDS ((1u << ASTRA_WMAX_LOG2) + 64)   // per-warp scratch words
+#define SCR_WORDS 1088u   // per-warp scratch words: 32 lanes x 64 16-bit ack keys (wf_sim, wf_priority_word), 513 counters (ack_sort), 512 (ack_chunk)
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
-    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, W, NC, NWmask, NW, kmagic, tmax, flags;
+    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, W, NC, NWmask, NW, kmagic, tmax, flags, alcap;
     u32 group, rank, v_lo, v_hi, g_lo, g_hi, e_lo, e_hi, i_lo, i_hi;
     u64 fullmask;
 #define X(n) const u32* n;
@@ -56,18 +56,27 @@ struct Ctx {   // resolved pointers of the point a CTA is running; lives in shar
 
 struct Ctl {   // per-CTA control block in shared memory
     u32 point;          // index into the order array
-    u32 acked;          // steps fully acked by this CTA's GPUs since the last group reduction
+    u32 acked;          // steps fully acked by this CTA's GPUs (single CTA: running total; group: since the last reduction)
     u32 completion;     // max t_ack
     u32 err;            // engine self-check flags
-    u32 next_hint;      // min over everything pending of its next event time
-    u32 decision;       // 0 = run window `next_k`, else 1 + status
-    u32 next_k;
-    u32 any_merged;     // some multi-feeder out-link received lines this window
-    u32 ntasks;         // link tasks of stage 1 this window
-    u32 acked_total;
-    u64 busy, skipped;
-    u64 clk[16];        // diagnostics: [0] windows, [1..4] SM clocks in stage groups, [5] init, [6] serial GPU-windows, [8..15] stage-2 parts
+    u32 hint[3];        // min over everything pending of its next event time; slot seq % 3 is the window's (A7)
+    u32 g_hint, g_acked, g_err, g_completion;   // group mode: the group-wide values after the window's group barrier
+    u32 abort;          // a group barrier timed out somewhere: leave the kernel
+#ifdef ASTRA_DIAG
+    u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows
+    u64 sclk[16][8];    // per warp set (clocks of its first warp, summed over its nodes and windows): 0 arrivals+acks,
+                        // 1 release events, 2 wavefront runs, 3 budget check / commit, 4 placement, 5 merge, 6 link service,
+                        // 7 waiting at the end-of-window barrier (block + group)
+#endif
 };
+
+#ifdef ASTRA_DIAG
+#define DIAG_CLK(slot) do { if (diag_lane) { const long long ck_ = clock64(); ctl.sclk[set][slot] += (u64)(ck_ - dck); dck = ck_; } } while (0)
+#define DIAG_ADD(slot, v) do { atomicAdd((unsigned long long*)&ctl.clk[slot], (unsigned long long)(v)); } while (0)
+#else
+#define DIAG_CLK(slot) do { } while (0)
+#define DIAG_ADD(slot, v) do { } while (0)
+#endif
 
 __device__ const unsigned char k_arr_init[ASTRA_A_COUNT] = {
 #define X(n, t, i) i,
@@ -78,15 +87,6 @@ __device__ const unsigned char k_arr_init[ASTRA_A_COUNT] = {
 // Arrays that the loader may place in shared OR global memory and that another CTA of a group may
 // have written: a volatile generic load (never served from a stale L1 line, legal on both spaces).
 __device__ __forceinline__ u32 ld_vol(const u32* p) { return *(const volatile u32*)p; }
-
-// SM clock read that cannot issue before the preceding __syncthreads() has completed (the barrier is
-// non-blocking at issue; a shared-memory load after it is not).
-__device__ __forceinline__ long long clock_after_barrier(const volatile u32* smem_word) {
-    const u32 dep = *smem_word;
-    long long ck;
-    asm volatile("mov.u64 %0, %%clock64;\n\t// %1" : "=l"(ck) : "r"(dep) : "memory");
-    return ck;
-}
 
 __device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
@@ -102,11 +102,10 @@ __device__ __forceinline__ int warp_incl_max(int v, u32 lane) {
 }
 
 // Mark slot `slot` of the cell (out-link o at node v, cycle t0 + d) occupied (R7/R8).
-__device__ __forceinline__ void cell_set(const Ctx& __restrict__ c, Ctl& ctl, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
+__device__ __forceinline__ void cell_set(const Ctx& __restrict__ c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
     u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
     atomicOr(&c.masks[c.mask_off[o] + ci * c.nd_mw[v] + (slot >> 5)], 1u << (slot & 31));
     c.dirty[o] = 1u;
-    ctl.any_merged = 1u;
 }
 // FIFO position, relative to the tail at the window start, of the line in slot `slot` of that cell.
 __device__ __forceinline__ u32 cell_pos(const Ctx& __restrict__ c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
@@ -125,12 +124,11 @@ __device__ __forceinline__ u32 cell_pos(const Ctx& __restrict__ c, u32 o, u32 v,
 // sums) writes the lines that go to multi-feeder out-links at their FIFO positions.
 // ---------------------------------------------------------------------------------------------
 template <int PASS>
-__device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
+__device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 i, u32 n_due, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 e = c.in_link[i];
     const u32 lo = c.pipe_head[e];
-    u32 hi;
-    if (PASS == 1) hi = ld_vol(&c.fifo_head[e]);
-    else hi = lo + c.ndue[e];
+    // pass 1: the lines due this window were counted by the link's service when it accepted them
+    const u32 hi = lo + (PASS == 1 ? n_due : c.ndue[e]);
     if (lo == hi) return;
     const u32 v = c.head[e];
     const u64* ring = c.ring + c.ring_off[e];
@@ -168,7 +166,7 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k,
             const bool direct = transit && moff == ASTRA_NONE32;
             const bool merged = transit && !direct;
             if (PASS == 1) {
-                if (merged) { cell_set(c, ctl, o, v, cb, d, coff + r); any_p3 = true; }
+                if (merged) { cell_set(c, o, v, cb, d, coff + r); any_p3 = true; }
                 const u32 dm = __ballot_sync(FULL, direct);
                 if (dm) {       // this stream is the only feeder of o: append in stream order
                     u32 grp = 0, base = 0;
@@ -195,7 +193,10 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k,
                         const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
                         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
                         const u32 mb = __match_any_sync(dmask, bin);
-                        if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+                        u32 lpos = 0;
+                        if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+                        lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
+                        if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
                         hint = min(hint, ta);
                         const u32 m = __match_any_sync(dmask, step);
                         const u32 dmax = __reduce_max_sync(m, d);
@@ -226,7 +227,7 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k,
         if (lane == 0) {
             if (any_p3) c.ndue[e] = ndue;           // pass 3 walks the same entries again
             else c.pipe_head[e] = lo + ndue;
-            if (hint != ASTRA_T_INF) atomicMin(&ctl.next_hint, hint);
+            if (hint != ASTRA_T_INF) atomicMin(hp, hint);
         }
     } else if (lane == 0) {
         c.pipe_head[e] = lo + ndue;
@@ -298,7 +299,7 @@ __device__ void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 
 // or all go on to one single-feeder link, is cut into independent chunks of 32 pipe entries; any
 // other link stays one task (arrivals_link).  Ack discovery is cut into chunks of 32 bitmap words.
 // ---------------------------------------------------------------------------------------------
-__device__ void stage1_setup_gpu(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 lane) {
+__device__ void stage1_setup_gpu(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 k, u32 lane) {
     u32 best = ASTRA_T_INF;                                     // earliest later window with acks pending (A7)
     for (u32 j = 1 + lane; j < c.NW; j += 32)
         if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
@@ -306,57 +307,82 @@ __device__ void stage1_setup_gpu(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
     if (lane == 0) {
         if (best != ASTRA_T_INF) {
             const u64 tw = (u64)(k + best) * c.W;
-            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
+            atomicMin(hp, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
         }
         c.ack_n[g] = ld_vol(&c.bin_cnt[g * c.NW + (k & c.NWmask)]);
     }
 }
 
-__device__ u32 stage1_setup_link(const Ctx& __restrict__ c, Ctl& ctl, u32 i, u32 k, u32 t0) {
-    const u32 e = c.in_link[i];
-    u32* dcb = &c.due_cnt[(size_t)e * c.NW];
-    const u32 n = ld_vol(&dcb[k & c.NWmask]);
-    const u32 lo = c.pipe_head[e], hi = ld_vol(&c.fifo_head[e]);
-    const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
-    // in flight beyond this window: the earliest later window with lines due (A7); all bins are read at once
-    if (fl && c.NW <= 8) {
-        u32 nextw = ASTRA_NONE32;
-        for (u32 j = c.NW - 1; j >= 1; j--) if (ld_vol(&dcb[(k + j) & c.NWmask])) nextw = j;
-        if (nextw != ASTRA_NONE32) {
-            const u64 tw = (u64)(k + nextw) * c.W;
-            atomicMin(&ctl.next_hint, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
-        }
-    } else if (fl && hi != lo + n) {                            // many bins: read the first entry that is not due instead
-        const u64 flit = __ldcg(&c.ring[c.ring_off[e] + ((lo + n) & c.ring_mask[e])]);
-        atomicMin(&ctl.next_hint, t0 + (((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26));
+// In-link e has lines in flight that arrive after this window: the earliest later window with lines
+// due is a candidate for the next non-idle window (A7).  Arrival windows of a link lie at most
+// Leff / W + 1 windows ahead.  One link per lane.  Also the ring overflow guard of the reading side.
+__device__ __forceinline__ void link_inflight_hint(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 lo, u32 k) {
+    const u32* dcb = &c.due_cnt[(size_t)e * c.NW];
+    const u32 span = min(c.NW - 1, c.leff[e] / c.W + 2);
+    u32 best = ASTRA_T_INF;
+    for (u32 j = span; j >= 1; j--)
+        if (ld_vol(&dcb[(k + j) & c.NWmask])) best = j;
+    if (best != ASTRA_T_INF) {
+        const u64 tw = (u64)(k + best) * c.W;
+        atomicMin(hp, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
     }
-    if (n) dcb[k & c.NWmask] = 0;
-    u32 nch = 0;
-    if (fl) {
-        if (n) {
-            nch = fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32;
-            c.tl_lo[e] = lo; c.tl_n[e] = n; c.pipe_head[e] = lo + n;
-            if (fl == ASTRA_LF_FORWARD_ONLY) { const u32 o = c.lfwd[e]; c.tl_base[e] = c.run[o]; c.run[o] += n; }
-        }
-        if (fl == ASTRA_LF_CELLS) c.tl_base[e] = 0;             // set by a chunk that marks a cell: pass 3 needed
-        if (hi - lo > c.ring_mask[e] + 1) atomicOr(&ctl.err, 1u);
-    } else if (hi != lo) nch = 1;
-    return nch;
+    if (ld_vol(&c.fifo_head[e]) - lo > c.ring_mask[e] + 1) atomicOr(&ctl.err, 1u);
 }
 
-// exclusive prefix of the per-link task counts (one warp); tbase[i_hi] = total
-__device__ void stage1_prefix(const Ctx& __restrict__ c, Ctl& ctl, u32 lane) {
-    u32 carry = 0;
-    for (u32 b = c.i_lo; b < c.i_hi; b += 32) {
-        const u32 i = b + lane;
-        const u32 v = (i < c.i_hi) ? c.tbase[i] : 0;
-        const u32 incl = warp_incl_scan(v, lane);
-        if (i < c.i_hi) c.tbase[i] = carry + incl - v;
-        carry += __shfl_sync(FULL, incl, 31);
+// 128 entries of the discovery list of GPU g's ack bin (deliveries appended the slot ids of their acks, in
+// any order): per-step ack counts, t_ack, ACKED events, amask (R6, A3).  Everything here commutes.
+__device__ void ack_list_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 n, u32 k, u32 t1, u32 lane) {
+    const u32 bin = k & c.NWmask;
+    const u32* list = c.ack_list + (size_t)(g * c.NW + bin) * c.alcap;
+    const u64* rec = c.ack_rec + (size_t)g * c.slots;
+    u32* am = c.amask + (size_t)g * c.nwords;
+    const u32 K = c.K, kmagic = c.kmagic;
+    const u32* lines = c.lines;
+    const u32 j0 = chunk * 128;
+    u32 idx[4]; u64 rc[4];
+#pragma unroll
+    for (int q = 0; q < 4; q++) { const u32 j = j0 + q * 32 + lane; idx[q] = j < n ? __ldcg(&list[j]) : 0xffffffffu; }
+#pragma unroll
+    for (int q = 0; q < 4; q++) rc[q] = idx[q] != 0xffffffffu ? __ldcg(&rec[idx[q]]) : 0ull;
+    u32 tmax = 0, cs = 0xffffffffu, cc = 0, cm = 0;
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        if (idx[q] == 0xffffffffu) continue;
+        const u32 ta = (u32)rc[q];
+        const u32 wf = K == 1 ? idx[q] : (u32)(((u64)idx[q] * kmagic) >> 32);   // idx / K
+        atomicOr(&am[wf >> 5], 1u << (wf & 31));
+        if (ta >= t1) continue;                              // beyond the watchdog cut: not processed
+        const u32 step = (u32)(rc[q] >> 32);
+        tmax = max(tmax, ta);
+        if (step != cs) {
+            if (cc) {
+                atomicMax(&c.t_ack[cs], cm);
+                if (atomicAdd(&c.ack_cnt[cs], cc) + cc == lines[cs]) {
+                    c.ev_list[c.ev_off[g] + atomicAdd(&c.ev_cnt[g], 1u)] = cs | ((u32)ASTRA_DEP_ACKED << 30);
+                    atomicAdd(&ctl.acked, 1u);
+                }
+            }
+            cs = step; cc = 0; cm = 0;
+        }
+        cc++; cm = max(cm, ta);
     }
-    if (lane == 0) { c.tbase[c.i_hi] = carry; ctl.ntasks = carry; }
+    {   // final flush, aggregated over the lanes that hold the same step
+        const u32 key = cc ? cs : 0xffffffffu;
+        const u32 m = __match_any_sync(FULL, key);
+        const u32 csum = __reduce_add_sync(m, cc), cmax = __reduce_max_sync(m, cm);
+        if (cc && (m & lanemask_lt()) == 0) {
+            atomicMax(&c.t_ack[cs], cmax);
+            if (atomicAdd(&c.ack_cnt[cs], csum) + csum == lines[cs]) {
+                c.ev_list[c.ev_off[g] + atomicAdd(&c.ev_cnt[g], 1u)] = cs | ((u32)ASTRA_DEP_ACKED << 30);
+                atomicAdd(&ctl.acked, 1u);
+            }
+        }
+    }
+    tmax = __reduce_max_sync(FULL, tmax);
+    if (lane == 0 && tmax) atomicMax(&ctl.completion, tmax);
 }
 
+// Fallback when a bin received more acks than its list holds: the bitmap itself is scanned.
 // 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3).
 // The set bits are first compacted into the warp's scratch so that every lane handles the same
 // number of acks whatever their spread over the words, four record loads in flight per lane.
@@ -438,8 +464,7 @@ __device__ void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk,
 }
 
 // 32 pipe entries of a link whose lines all terminate at its head GPU (R7 A1, deliveries)
-__device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 lane) {
-    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+__device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 lo, u32 n, u32 chunk, u32 k, u32 t0, u32 wlen, u32 lane) {
     const u32 ii = lo + chunk * 32 + lane;
     bool valid = (int32_t)(lo + n - ii) > 0;
     u64 flit0 = 0;
@@ -462,7 +487,10 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 ch
         const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
         const u32 mb = __match_any_sync(amk, bin);
-        if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+        u32 lpos = 0;
+        if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+        lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
+        if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
         hint = ta;
         const u32 m = __match_any_sync(amk, step);
         const u32 dmax = __reduce_max_sync(m, d);
@@ -476,7 +504,7 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 ch
             }
         }
         hint = __reduce_min_sync(amk, hint);
-        if ((amk & lanemask_lt()) == 0) atomicMin(&ctl.next_hint, hint);
+        if ((amk & lanemask_lt()) == 0) atomicMin(hp, hint);
     }
 }
 
@@ -486,12 +514,11 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 ch
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
 // PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
 template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
 
 // A task is 64 entries: both halves' ring loads (and the look-back) are in flight before the first use.
 template <int PASS>
-__device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
-    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+__device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 lo, u32 n, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 i0 = lo + chunk * 64;
     const u64* ring = c.ring + c.ring_off[e];
     const u32 rmask = c.ring_mask[e];
@@ -507,12 +534,12 @@ __device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 chun
     const u32 da0 = __shfl_sync(FULL, da, 0), db0 = __shfl_sync(FULL, db, 0);
     const u32 back_a = __popc(__ballot_sync(FULL, dz == da0));          // same-cycle lines before the task
     const u32 back_b = __popc(__ballot_sync(FULL, da == db0));          // ... before its second half
-    cells_half<PASS>(c, ctl, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, lane);   // d >= wlen: watchdog cut inside the window
-    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, lane);
+    cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, lane);   // d >= wlen: watchdog cut inside the window
+    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, lane);
 }
 
 template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
     const u32 vmask = __ballot_sync(FULL, valid);
     if (!valid) return;
     const u32 grp = __match_any_sync(vmask, d);
@@ -524,7 +551,7 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u3
     const bool deliver = dstg == v;
     if (!deliver) {
         const u32 o = c.next_link[(size_t)v * c.G + dstg];
-        if (PASS == 1) { cell_set(c, ctl, o, v, cb, d, c.classoff[e] + r); c.tl_base[e] = 1u; }
+        if (PASS == 1) { cell_set(c, o, v, cb, d, c.classoff[e] + r); c.tl_base[e] = 1u; }
         else {
             const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, c.classoff[e] + r);
             c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
@@ -541,7 +568,10 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u3
             const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
             atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
             const u32 mb = __match_any_sync(dmask, bin);
-            if ((mb & lanemask_lt()) == 0) atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+            u32 lpos = 0;
+            if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
+            lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
+            if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
             const u32 m = __match_any_sync(dmask, step);
             const u32 dmax = __reduce_max_sync(m, d);
             if ((m & lanemask_lt()) == 0) {
@@ -554,22 +584,21 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u3
                 }
             }
             const u32 hint = __reduce_min_sync(dmask, ta);
-            if ((dmask & lanemask_lt()) == 0) atomicMin(&ctl.next_hint, hint);
+            if ((dmask & lanemask_lt()) == 0) atomicMin(hp, hint);
         }
     }
 }
 
 // 32 pipe entries of a link whose lines all go on to the single-feeder link lfwd[e] (R7 A1, transit):
 // stream order is FIFO order, so the position is the base plus the index in the stream
-__device__ void forward_chunk(const Ctx& __restrict__ c, u32 e, u32 chunk, u32 t0, u32 wlen, u32 lane) {
-    const u32 lo = c.tl_lo[e], n = c.tl_n[e];
+__device__ void forward_chunk(const Ctx& __restrict__ c, u32 e, u32 lo, u32 n, u32 base, u32 chunk, u32 t0, u32 wlen, u32 lane) {
     const u32 ii = lo + chunk * 32 + lane;
     if ((int32_t)(lo + n - ii) <= 0) return;
     const u64 flit = __ldcg(&c.ring[c.ring_off[e] + (ii & c.ring_mask[e])]);
     const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
     if (d >= wlen) return;                                      // watchdog cut inside the window
     const u32 o = c.lfwd[e];
-    const u32 pos = c.tl_base[e] + (ii - lo);
+    const u32 pos = base + (ii - lo);
     c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
 }
 
@@ -623,7 +652,7 @@ __device__ __forceinline__ bool wf_advance(const Ctx& __restrict__ c, u32 g, u32
 // ---------------------------------------------------------------------------------------------
 // stage 2: release + issue of GPU g over [t0, t1)   (R10 - R13, slot return of R7 A3)
 // ---------------------------------------------------------------------------------------------
-__device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 ack_n = c.ack_n[g];
     const u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32* plist = c.plist + c.rel_off[g];
@@ -795,7 +824,7 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0,
             const u32 mm = __ballot_sync(FULL, merged);
             if (mm) {
                 if (merged) {
-                    cell_set(c, ctl, o, g, cb, d, injoff + j);
+                    cell_set(c, o, g, cb, d, injoff + j);
                     const u32 p = n_inj + __popc(mm & lanemask_lt());
                     if (p < inj_cap) inj[p] = payload | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
                     else atomicOr(&ctl.err, 4u);
@@ -843,7 +872,7 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0,
     }
     if (lane == 0) {
         c.inj_n[g] = n_inj;
-        if (t != ASTRA_T_INF) atomicMin(&ctl.next_hint, t);
+        if (t != ASTRA_T_INF) atomicMin(hp, t);
     }
 }
 
@@ -917,7 +946,7 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
 // if the HBM budget never bound.  Issues go to the bucket of their cycle (first H of a cycle are
 // kept: more than H means the budget binds and the GPU-window is redone cycle-serially).  The new
 // wavefront state is written in place, the old one kept in the undo arrays for that case.
-__device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+__device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am0 = c.amask[(size_t)g * nwords + wi];
     if (am0 == 0) return;
@@ -962,8 +991,9 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
         const u32* const cul = c.cul;
       if (!heavy) {
         c.undo_cur[gw] = cur; c.undo_rem[gw] = rem; c.undo_busy[gw] = busy;
-        // the wavefront's acks of the window, sorted by cycle: (cycle - t0) << 6 | slot
-        u32 aq[64];
+        // the wavefront's acks of the window, sorted by cycle: (cycle - t0) << 6 | slot, 15 bits each, in the
+        // warp's shared-memory scratch (entry j of this lane at aq[32 j]: no bank conflicts, no local memory)
+        unsigned short* const aq = reinterpret_cast<unsigned short*>(scr) + lane;
         u32 na = 0, ai = 0;
         if (rb) {
             const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
@@ -975,12 +1005,12 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
 #pragma unroll
                 for (int q = 0; q < 4; q++) v[q] = (q < m) ? (u32)__ldcg(&rec[b[q]]) : 0u;
 #pragma unroll
-                for (int q = 0; q < 4; q++) if (q < m) aq[na++] = ((v[q] - t0) << 6) | b[q];
+                for (int q = 0; q < 4; q++) if (q < m) aq[32 * na++] = (unsigned short)(((v[q] - t0) << 6) | b[q]);
             }
             for (u32 i = 1; i < na; i++) {
-                const u32 xv = aq[i]; u32 j = i;
-                while (j > 0 && aq[j - 1] > xv) { aq[j] = aq[j - 1]; j--; }
-                aq[j] = xv;
+                const u32 xv = aq[32 * i]; u32 j = i;
+                while (j > 0 && aq[32 * (j - 1)] > xv) { aq[32 * j] = aq[32 * (j - 1)]; j--; }
+                aq[32 * j] = (unsigned short)xv;
             }
         }
         u32 nq = na ? aq[0] : 0xffffffffu;                       // earliest ack not applied yet (packed)
@@ -1011,7 +1041,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
             }
             while ((nq >> 6) <= tt) {                           // slots returned by this cycle (A3 before D)
                 busy &= ~(1ull << (nq & 63u)); ai++;
-                nq = ai < na ? aq[ai] : 0xffffffffu;
+                nq = ai < na ? aq[32 * ai] : 0xffffffffu;
             }
             if (tt >= wlen) break;
             const u32 slot = __ffsll((long long)~busy) - 1;
@@ -1045,7 +1075,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
                 if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
             }
         }
-        for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));   // acks later in the window than the last look
+        for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));   // acks later in the window than the last look
         c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
         wantb = rem != ASTRA_NOTLOADED;
         freebit = busy != fullmask;
@@ -1063,7 +1093,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
         c.undo_want[(size_t)g * nwords + wi] = ow; c.undo_freeb[(size_t)g * nwords + wi] = of;
         *want = (ow & ~am) | wm;
         *freeb = (of & ~am) | fm;
-        if (anyh) atomicMin(&ctl.next_hint, t1);
+        if (anyh) atomicMin(hp, t1);
     }
 }
 
@@ -1071,7 +1101,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k
 // issue of the window needs a slot -- one of the F0 slots free at the window start, else the
 // (i - F0)-th ack in cycle order -- and its step released, and comes at least one cycle after the
 // (i-1)-th: x_i = max(x_{i-1} + 1, c_i), a prefix maximum of c_j - j.  Same result as wf_sim.
-__device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wf, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+__device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wf, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
     const u32 W = c.W, H = c.H, K = c.K, nwords = c.nwords;
     const u64 fullmask = c.fullmask;
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
@@ -1185,7 +1215,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wf, u32
         const u32 bit = 1u << (wf & 31);
         if (wantb) atomicOr(want, bit); else atomicAnd(want, ~bit);
         if (freebit) atomicOr(freeb, bit); else atomicAnd(freeb, ~bit);
-        if ((wantb && freebit) || last_issue == wlen - 1) atomicMin(&ctl.next_hint, t1);
+        if ((wantb && freebit) || last_issue == wlen - 1) atomicMin(hp, t1);
     }
     __syncwarp();
 }
@@ -1212,7 +1242,7 @@ __device__ void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
 // lower id are granted at t; occ[t] (the cnt array) holds the grants of all lower words, so the 32
 // wavefronts of a word step together through the cycles where one of them is ready and occ[t] < H,
 // a ballot giving the rank inside the word.  That rank is the bucket position of the issue.
-__device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32 lane) {
+__device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am = c.amask[(size_t)g * nwords + wi];
     if (am == 0) return;
@@ -1229,7 +1259,7 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
     const size_t gw = (size_t)g * c.CW + wf;
     u32 cur = 0, rem = ASTRA_NOTLOADED, end = 0;
     u64 busy = fullmask;
-    u32 aq[64];
+    unsigned short* const aq = reinterpret_cast<unsigned short*>(scr) + lane;      // as in wf_sim: entry j at aq[32 j]
     u32 na = 0, ai = 0;
     if (active) {
         cur = c.wf_cur[gw]; rem = c.wf_rem[gw]; busy = c.wf_busy[gw];
@@ -1247,11 +1277,11 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
             rb &= fullmask;
         }
         const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
-        while (rb) { const u32 b = __ffsll((long long)rb) - 1; rb &= rb - 1; aq[na++] = (((u32)__ldcg(&rec[b]) - t0) << 6) | b; }
+        while (rb) { const u32 b = __ffsll((long long)rb) - 1; rb &= rb - 1; aq[32 * na++] = (unsigned short)((((u32)__ldcg(&rec[b]) - t0) << 6) | b); }
         for (u32 i = 1; i < na; i++) {
-            const u32 xv = aq[i]; u32 j = i;
-            while (j > 0 && aq[j - 1] > xv) { aq[j] = aq[j - 1]; j--; }
-            aq[j] = xv;
+            const u32 xv = aq[32 * i]; u32 j = i;
+            while (j > 0 && aq[32 * (j - 1)] > xv) { aq[32 * j] = aq[32 * (j - 1)]; j--; }
+            aq[32 * j] = (unsigned short)xv;
         }
     }
     u32 nq = na ? aq[0] : 0xffffffffu;
@@ -1262,7 +1292,7 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
         // bring the lane to cycle T: slots returned by T, step loaded if released by T
         u32 np = 0xffffffffu;                                   // earliest cycle this lane can be ready
         if (active) {
-            while ((nq >> 6) <= T) { busy &= ~(1ull << (nq & 63u)); ai++; nq = ai < na ? aq[ai] : 0xffffffffu; }
+            while ((nq >> 6) <= T) { busy &= ~(1ull << (nq & 63u)); ai++; nq = ai < na ? aq[32 * ai] : 0xffffffffu; }
             if (rem == ASTRA_NOTLOADED) {
                 while (cur < end) {
                     const u32 s2 = cul[cur];
@@ -1313,7 +1343,7 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
     }
     bool wantb = false, freebit = false, hint = false;
     if (active) {
-        for (; ai < na; ai++) busy &= ~(1ull << (aq[ai] & 63u));
+        for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));
         if (rem == ASTRA_NOTLOADED) {                           // a step released by the end of the window is loaded (as in wf_sim)
             while (cur < end) {
                 const u32 s2 = cul[cur];
@@ -1335,7 +1365,7 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32
         u32* freeb = c.freeb + (size_t)g * nwords + wi;
         *want = (*want & ~am) | wm;
         *freeb = (*freeb & ~am) | fm;
-        if (anyh) atomicMin(&ctl.next_hint, t1);
+        if (anyh) atomicMin(hp, t1);
     }
     __syncwarp();
 }
@@ -1382,9 +1412,13 @@ __device__ void gpu_finalize(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, 
         }
     }
     // consume the acks of the window's bin and the releases
-    if (c.ack_n[g]) {
+    const u32 n_ack = c.ack_n[g];
+    if (n_ack) {
         u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
-        for (u32 i = lane; i < c.bmwords; i += 32) bm[i] = 0;
+        if (n_ack <= c.alcap) {     // every bit of the bin's words is consumed this window: whole words can go
+            const u32* list = c.ack_list + (size_t)(g * c.NW + (k & c.NWmask)) * c.alcap;
+            for (u32 i = lane; i < n_ack; i += 32) bm[__ldcg(&list[i]) >> 5] = 0;
+        } else for (u32 i = lane; i < c.bmwords; i += 32) bm[i] = 0;
     }
     for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
     if (lane == 0) {
@@ -1429,7 +1463,7 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
         const u32 pos = (deg == 1 ? c.run[o] - nev + st : c.hist[(size_t)o * W + tt]) + jo;
         c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
     } else {
-        cell_set(c, ctl, o, g, cb, d, c.nd_injoff[g] + j);
+        cell_set(c, o, g, cb, d, c.nd_injoff[g] + j);
         const u32 p = atomicAdd(&c.inj_n[g], 1u);
         if (p < c.inj_off[g + 1] - c.inj_off[g]) c.inj_list[c.inj_off[g] + p] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
         else atomicOr(&ctl.err, 4u);
@@ -1497,7 +1531,7 @@ __device__ void inject_place(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 cb,
 // ---------------------------------------------------------------------------------------------
 // stage 4: link e over [t0, t1): acceptance times of the whole FIFO (R9), arrival stamps.
 // ---------------------------------------------------------------------------------------------
-__device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 wlen = t1 - t0;
     const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
     if (c.dirty[e]) {                                        // consume the cells of the window
@@ -1514,7 +1548,6 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, 
             u32 any = 0;
             for (u32 w = 0; w < mw; w++) any |= masks[ci * mw + w];
             c.dirty[e] = any ? 1u : 0u;
-            if (any) ctl.any_merged = 1u;
         }
     }
     const u32 n_back = tl - fh, n_new = tn - tl;
@@ -1674,11 +1707,11 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32 e, u32 k, 
         c.ltail[e] = tn;
         if (n_acc) {
             c.link_lines[e] += n_acc;
-            atomicMin(&ctl.next_hint, t0 + first_x + leff);
+            atomicMin(hp, t0 + first_x + leff);
             if (kind == ASTRA_LK_PERIOD) c.lstate0[e] = t0 + last_x + param;
         }
         if (kind == ASTRA_LK_GENERAL) { c.lstate0[e] = cr; c.lstate1[e] = tc; }
-        if (n_tot > n_acc) atomicMin(&ctl.next_hint, t1);
+        if (n_tot > n_acc) atomicMin(hp, t1);
     }
 }
 
@@ -1686,7 +1719,7 @@ __device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8
     c.G = P.G; c.V = P.V; c.E = P.E; c.S = P.S; c.C = P.C; c.Wv = P.Wv; c.K = P.K; c.H = P.H;
     c.CW = P.CW; c.nwords = P.nwords; c.slots = P.slots; c.bmwords = P.bmwords;
     c.W = P.Wcyc; c.NC = P.NC; c.NW = P.NW; c.NWmask = P.NW - 1; c.kmagic = P.kdiv_magic;
-    c.tmax = (u32)P.max_cycles; c.flags = P.flags;
+    c.tmax = (u32)P.max_cycles; c.flags = P.flags; c.alcap = P.alcap;
     c.fullmask = P.K >= 64 ? ~0ull : ((1ull << P.K) - 1);
     c.group = P.group; c.rank = rank;
 #define X(n) c.n = (const u32*)(cb + P.c_off[ASTRA_C_##n]);
@@ -1706,17 +1739,212 @@ __device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8
     c.r_diag = (u64*)(rs + P.r_diag);
 }
 
-// Barrier over the CTAs of a group (all co-resident: the grid never exceeds what fits on the
-// device).  `target` = number of arrivals that completes this barrier.
-__device__ __forceinline__ void group_barrier(GroupCtl* gc, u32 target) {
+// Barrier over the CTAs of a group.  The grid is launched cooperatively (astra_engine_launch), so all
+// CTAs are co-resident or the launch fails; the spin is bounded all the same: after ASTRA_SPIN_CLOCKS
+// without progress the CTA raises the kernel-wide abort flag and every CTA leaves.
+// `target` = number of arrivals that completes this barrier.  Returns false on abort.
+#define ASTRA_SPIN_CLOCKS (1ll << 34)     // about 8 s at 2 GHz
+__device__ __forceinline__ bool group_barrier(GroupCtl* gc, u32 target, u32* abort_flag, Ctl& ctl) {
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
         atomicAdd(&gc->bar, 1u);
-        while ((int32_t)(*(volatile u32*)&gc->bar - target) < 0) { }
+        const long long start = clock64();
+        u32 spins = 0;
+        while ((int32_t)(*(volatile u32*)&gc->bar - target) < 0) {
+            if ((++spins & 0x3ffu) == 0) {
+                if (*(volatile u32*)abort_flag) { ctl.abort = 1u; break; }
+                if (clock64() - start > ASTRA_SPIN_CLOCKS) { atomicExch(abort_flag, 1u); ctl.abort = 1u; break; }
+            }
+        }
         __threadfence();
     }
     __syncthreads();
+    return ctl.abort == 0u;
+}
+
+// Barrier over the `ws` warps that work on one simulated node (named barrier 1 + set; a single warp
+// needs only its own lanes).  Orders the set's shared- and global-memory accesses like __syncthreads.
+__device__ __forceinline__ void set_sync(u32 ws, u32 set) {
+    if (ws == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" :: "r"(set + 1u), "r"(ws * 32u) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// One lookahead window of one simulated node v, by the warp set that owns it (sw = warp index in the
+// set of ws warps).  Inside a window nothing a node does can reach another node (W <= min Leff), so
+// the stages of a node order only against each other: set barriers, no block barrier.
+// ---------------------------------------------------------------------------------------------
+__device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
+                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane) {
+#ifdef ASTRA_DIAG
+    long long dck = clock64();
+#endif
+    const u32 wlen = t1 - t0;
+    const bool is_gpu = v < c.G;
+    const u32 i_lo = c.in_ptr[v], i_hi = c.in_ptr[v + 1];
+    const u32 e_lo = c.row_ptr[v], e_hi = c.row_ptr[v + 1];
+    const bool serial_arr = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) != 0;
+    const u32 kb = k & c.NWmask;
+
+    // ---- stage 1: ack discovery (A3) and arrivals (A1) as chunk tasks over the set's warps ----
+    bool any_fwd = false;
+    if (is_gpu) {
+        if (sw == 0) stage1_setup_gpu(c, ctl, hp, v, k, lane);
+        const u32 n_ack = ld_vol(&c.bin_cnt[v * c.NW + kb]);
+        if (n_ack && n_ack <= c.alcap) {
+            for (u32 ch = sw; ch * 128 < n_ack; ch += ws) ack_list_chunk(c, ctl, v, ch, n_ack, k, t1, lane);
+        } else if (n_ack) {
+            const u32 nch = (c.bmwords + 31) / 32;
+            for (u32 ch = sw; ch < nch; ch += ws) ack_chunk(c, ctl, v, ch, k, t1, scr, lane);
+        }
+    }
+    // the node's in-links, one per lane: id, lines due this window (counted by the link's service when it
+    // accepted them), read cursor, arrival path -- all loads of a batch of 32 links in flight at once
+    u32 e_l = 0, n_l = 0, lo_l = 0, fl_l = 0;
+    for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+        const u32 i = ib + lane;
+        u32 e_b = 0, n_b = 0, lo_b = 0, fl_b = 0;
+        if (i < i_hi) {
+            e_b = c.in_link[i];
+            n_b = ld_vol(&c.due_cnt[(size_t)e_b * c.NW + kb]);
+            lo_b = c.pipe_head[e_b];
+            fl_b = serial_arr ? 0u : c.lflag[e_b];
+            if (sw == (i - i_lo) % ws) link_inflight_hint(c, ctl, hp, e_b, lo_b, k);
+        }
+        if (ib == i_lo) { e_l = e_b; n_l = n_b; lo_l = lo_b; fl_l = fl_b; }     // first batch stays in registers for stages 3 and 4
+        u32 nm = __ballot_sync(FULL, n_b != 0u);
+        while (nm) {
+            const u32 src = __ffs(nm) - 1; nm &= nm - 1;
+            const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
+            const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
+            const u32 rot = (ib - i_lo + src) % ws;
+            if (fl == 0u) { if (sw == rot) arrivals_link<1>(c, ctl, hp, ib + src, n, k, t0, wlen, cb, lane); continue; }
+            const u32 first = (sw + ws - rot) % ws;
+            if (fl == ASTRA_LF_DELIVER_ONLY) {
+                for (u32 ch = first; ch * 32 < n; ch += ws) deliver_chunk(c, ctl, hp, e, lo, n, ch, k, t0, wlen, lane);
+            } else if (fl == ASTRA_LF_FORWARD_ONLY) {
+                const u32 base = c.run[c.lfwd[e]];
+                for (u32 ch = first; ch * 32 < n; ch += ws) forward_chunk(c, e, lo, n, base, ch, t0, wlen, lane);
+                any_fwd = true;
+            } else {
+                for (u32 ch = first; ch * 64 < n; ch += ws) cells_chunk<1>(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
+            }
+        }
+    }
+    set_sync(ws, set);
+    if (any_fwd && sw == 0) {                    // forwarded lines are now in the next link's FIFO
+        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+            const u32 i = ib + lane;
+            if (i >= i_hi) continue;
+            const u32 e = ib == i_lo ? e_l : c.in_link[i];
+            if (!serial_arr && c.lflag[e] == ASTRA_LF_FORWARD_ONLY) c.run[c.lfwd[e]] += ld_vol(&c.due_cnt[(size_t)e * c.NW + kb]);
+        }
+    }
+    DIAG_CLK(0);
+
+    // ---- stage 2: release + issue of GPU v (R10 - R13) ----
+    if (is_gpu) {
+        const u32 g = v;
+        if (sw == 0) gpu_prepare(c, ctl, g, t0, t1, lane);
+        set_sync(ws, set);
+        DIAG_CLK(1);
+        u32 mode = c.gmode[g];
+        if (mode == 1u) {
+            for (u32 wi = sw; wi < c.nwords; wi += ws) wf_sim(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+            set_sync(ws, set);
+            const u32 nh = c.nheavy[g];
+            if (nh) {
+                for (u32 j = sw; j < nh; j += ws) wf_heavy(c, ctl, hp, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
+                set_sync(ws, set);
+            }
+            DIAG_CLK(2);
+            if (sw == 0) {
+                if (!gpu_binds(c, g, wlen, lane)) gpu_finalize(c, ctl, g, k, wlen, lane);
+                else {
+                    // the budget binds: back to the window start, then exact grants
+                    if (lane == 0) DIAG_ADD(6, 1);
+                    wf_restore(c, g, lane);
+                    if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
+                    else {
+                        const u32 deg = e_hi - e_lo;
+                        for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
+                        if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
+                        __syncwarp();
+                        for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+                        gpu_finalize(c, ctl, g, k, wlen, lane);
+                    }
+                }
+            }
+            set_sync(ws, set);
+            mode = c.gmode[g];
+        }
+        if (mode == 2u) {                        // cycle-serial path
+            if (sw == 0) {
+                ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
+                issue_window(c, ctl, hp, g, t0, t1, cb, lane);
+                for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
+            }
+            set_sync(ws, set);
+            DIAG_CLK(3);
+        } else if (mode == 1u) {
+            DIAG_CLK(3);
+            const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
+            for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
+            set_sync(ws, set);
+            DIAG_CLK(4);
+        }
+    } else if (any_fwd) set_sync(ws, set);
+
+    // ---- stage 3: merge into multi-feeder out-links of v (skipped when none received a line) ----
+    bool any_dirty = false;
+    for (u32 e = e_lo + lane; e < e_hi; e += 32) any_dirty |= c.dirty[e] != 0u;
+    any_dirty = __any_sync(FULL, any_dirty);
+    if (any_dirty) {
+        for (u32 e = e_lo + sw; e < e_hi; e += ws)
+            if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
+        set_sync(ws, set);
+        if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
+        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+            const u32 i = ib + lane;
+            u32 e_b = e_l, n_b = n_l, lo_b = lo_l, fl_b = fl_l;
+            if (ib != i_lo) {
+                e_b = n_b = lo_b = fl_b = 0;
+                if (i < i_hi) {
+                    e_b = c.in_link[i]; n_b = ld_vol(&c.due_cnt[(size_t)e_b * c.NW + kb]);
+                    lo_b = c.pipe_head[e_b]; fl_b = serial_arr ? 0u : c.lflag[e_b];
+                }
+            }
+            // links that marked cells in pass 1 go over the same lines again, now with the FIFO positions known
+            const bool again = i < i_hi && (fl_b == 0u ? c.ndue[e_b] != 0u : (fl_b == ASTRA_LF_CELLS && c.tl_base[e_b] != 0u));
+            u32 nm = __ballot_sync(FULL, again);
+            while (nm) {
+                const u32 src = __ffs(nm) - 1; nm &= nm - 1;
+                const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
+                const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
+                const u32 rot = (ib - i_lo + src) % ws;
+                if (fl == 0u) { if (sw == rot) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); continue; }
+                for (u32 ch = (sw + ws - rot) % ws; ch * 64 < n; ch += ws) cells_chunk<3>(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
+            }
+        }
+        set_sync(ws, set);
+    }
+    DIAG_CLK(5);
+
+    // ---- stage 4: link service of v's out-links (R9); the in-links' cursors move past the window ----
+    if (sw == ws - 1) {
+        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+            const u32 i = ib + lane;
+            if (i >= i_hi) continue;
+            u32 e = e_l, n = n_l, fl = fl_l;
+            if (ib != i_lo) { e = c.in_link[i]; n = ld_vol(&c.due_cnt[(size_t)e * c.NW + kb]); fl = serial_arr ? 0u : c.lflag[e]; }
+            if (n == 0) continue;
+            c.due_cnt[(size_t)e * c.NW + kb] = 0;
+            if (fl != 0u) { c.pipe_head[e] += n; c.tl_base[e] = 0; }
+        }
+    }
+    for (u32 e = e_lo + sw; e < e_hi; e += ws) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
+    DIAG_CLK(6);
 }
 
 extern "C" __global__ void __launch_bounds__(512, 1)
@@ -1732,6 +1960,7 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
     const u32 tid = threadIdx.x, nthr = blockDim.x;
     const u32 lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
     u32* scr = scr_all + warp * SCR_WORDS;
+    u32* const abort_flag = queue + 2;
     // CTAs [0, n_slots * group0) form the groups that run the big points; every CTA can run small ones
     const bool in_slot = blockIdx.x < n_slots * group0;
     u32 group = in_slot ? group0 : 1u;
@@ -1740,21 +1969,27 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
     uint8_t* ws = in_slot ? ws_base + (size_t)gid * ws_big_stride : ws_base + ws_single_off + (size_t)blockIdx.x * ws_single_stride;
     GroupCtl* gc = groups + gid;
     u32 bar_target = 0;                 // arrivals that complete the next group barrier
+    if (tid == 0) ctl.abort = 0u;
 
     for (;;) {
         __syncthreads();
         if (group == 1) {
-            if (tid == 0) { const u32 q = atomicAdd(&queue[1], 1u); ctl.point = q < n_points - n_big ? n_big + q : ASTRA_NONE32; }
+            if (tid == 0) {
+                const u32 q = *(volatile u32*)abort_flag ? ASTRA_NONE32 : atomicAdd(&queue[1], 1u);
+                ctl.point = q < n_points - n_big ? n_big + q : ASTRA_NONE32;
+            }
             __syncthreads();
         } else {
-            bar_target += group; group_barrier(gc, bar_target);     // everyone is done with the previous point's control block
+            bar_target += group;
+            if (!group_barrier(gc, bar_target, abort_flag, ctl)) break;     // everyone is done with the previous point's control block
             if (rank == 0 && tid == 0) {
                 const u32 q = atomicAdd(&queue[0], 1u);
                 gc->point = q < n_big ? q : ASTRA_NONE32;
                 gc->acked = 0; gc->err = 0; gc->completion = 0;
                 gc->hint[0] = gc->hint[1] = gc->hint[2] = ASTRA_T_INF;
             }
-            bar_target += group; group_barrier(gc, bar_target);
+            bar_target += group;
+            if (!group_barrier(gc, bar_target, abort_flag, ctl)) break;
             if (tid == 0) ctl.point = *(volatile u32*)&gc->point;
             __syncthreads();
         }
@@ -1770,12 +2005,17 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
         const PointDesc& P = points[pi];
         if (tid == 0) {
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
-            ctl.acked = 0; ctl.completion = 0; ctl.err = 0; ctl.next_hint = ASTRA_T_INF; ctl.any_merged = 0;
-            ctl.acked_total = 0;
-            ctl.busy = 0; ctl.skipped = 0;
+            ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
+            ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
+            ctl.g_hint = ASTRA_T_INF; ctl.g_acked = 0; ctl.g_err = 0; ctl.g_completion = 0;
+#ifdef ASTRA_DIAG
             for (int i = 0; i < 16; i++) ctl.clk[i] = 0;
+            for (int i = 0; i < 128; i++) (&ctl.sclk[0][0])[i] = 0;
+#endif
         }
-        long long ck0 = clock64();
+#ifdef ASTRA_DIAG
+        long long dck = clock64();
+#endif
         __syncthreads();
         // ---- state init: shared-memory arrays by their CTA, global arrays split over the group ----
         for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
@@ -1791,13 +2031,14 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             if (in_smem || group == 1) { for (u64 i = tid; i < n16; i += nthr) p[i] = v4; }
             else { for (u64 i = (u64)rank * nthr + tid; i < n16; i += (u64)group * nthr) p[i] = v4; }
         }
-        if (group > 1) { bar_target += group; group_barrier(gc, bar_target); } else __syncthreads();
+        if (group > 1) { bar_target += group; if (!group_barrier(gc, bar_target, abort_flag, ctl)) break; } else __syncthreads();
         for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.lstate0[e] = c.lstate0_init[e];
         for (u32 s = tid; s < c.S; s += nthr) {
             const u32 ow = c.step_od[s] >> 16;
             if (ow < c.g_lo || ow >= c.g_hi) continue;
             c.ndep_left[s] = c.ndeps[s];
-            c.t_release[s] = c.ndeps[s] ? ASTRA_TS_NONE32 : 0u;      // steps without deps are released at t = 0 (R10)
+            // steps without deps are released at t = 0 (R10) -- unless the watchdog allows no cycle at all
+            c.t_release[s] = (c.ndeps[s] || c.tmax == 0u) ? ASTRA_TS_NONE32 : 0u;
         }
         for (u32 gq = c.g_lo; gq < c.g_hi; gq++) {
             for (u32 j = c.rel_off[gq] + tid; j < c.rel_off[gq + 1]; j += nthr) c.plist[j] = c.init_rel[j];
@@ -1808,176 +2049,84 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             }
             if (tid == 0) c.pcnt[gq] = c.init_rel_cnt[gq];
         }
-        if (group > 1) { bar_target += group; group_barrier(gc, bar_target); } else __syncthreads();
-        if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[5] += (u64)(ck - ck0); ck0 = ck; }
+        if (group > 1) { bar_target += group; if (!group_barrier(gc, bar_target, abort_flag, ctl)) break; } else __syncthreads();
+#ifdef ASTRA_DIAG
+        if (tid == 0) ctl.clk[5] = (u64)(clock64() - dck);
+#endif
+
+        // ---- warp sets: the CTA's nodes are dealt round robin to nsets sets of ws warps each ----
+        const u32 n_nodes = c.v_hi - c.v_lo;
+        const u32 nsets = max(1u, min(n_nodes, nwarps));
+        const u32 wset = nwarps / nsets;                   // warps per set (left-over warps idle through the window)
+        const u32 set = warp / wset, sw = warp % wset;
+        const bool in_set = set < nsets;
 
         // ---- window loop ----
         u32 k = 0, seq = 0;
         int32_t status = ASTRA_STATUS_DONE;
         const u32 W = c.W;
         u64 busy = 0, skipped = 0;
+        bool aborted = false;
         for (;;) {
-            const u64 t0l = (u64)k * c.W;
+            const u64 t0l = (u64)k * W;
             if (t0l >= c.tmax) { status = ASTRA_STATUS_MAX_CYCLES; break; }
             const u32 t0 = (u32)t0l;
             const u32 t1 = (u32)min((u64)c.tmax, t0l + W);
-            const u32 wlen = t1 - t0;
             const u32 cb = t0 % c.NC;
-            busy += wlen;
-            // stage 1: arrivals and ack discovery, as a flat list of chunk tasks
-            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) stage1_setup_gpu(c, ctl, g, k, lane);
-            if (c.i_hi - c.i_lo <= 32) {                          // few in-links: set up and scan in one warp, one barrier less
-                if (warp == nwarps - 1) {
-                    const u32 i = c.i_lo + lane;
-                    const u32 v = i < c.i_hi ? stage1_setup_link(c, ctl, i, k, t0) : 0u;
-                    const u32 incl = warp_incl_scan(v, lane);
-                    if (i < c.i_hi) c.tbase[i] = incl - v;
-                    if (lane == 31) { c.tbase[c.i_hi] = incl; ctl.ntasks = incl; }
-                }
-            } else {
-                for (u32 i = c.i_lo + tid; i < c.i_hi; i += nthr) c.tbase[i] = stage1_setup_link(c, ctl, i, k, t0);
-                __syncthreads();
-                if (warp == 0) stage1_prefix(c, ctl, lane);
-            }
-            __syncthreads();
-            for (u32 g = c.g_lo; g < c.g_hi; g++) {
-                if (c.ack_n[g] == 0) continue;
-                const u32 nch = (c.bmwords + 31) / 32;
-                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ack_chunk(c, ctl, g, ch, k, t1, scr, lane);
-            }
-            {
-                const u32 ntl = ctl.ntasks;
-                for (u32 task = nwarps - 1 - warp; task < ntl; task += nwarps) {
-                    u32 lo = c.i_lo, hi = c.i_hi;               // first in-link with tbase > task
-                    while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (c.tbase[mid] > task) hi = mid; else lo = mid + 1; }
-                    const u32 i = lo - 1, ch = task - c.tbase[i];
-                    const u32 e = c.in_link[i];
-                    const u32 fl = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e];
-                    if (fl == ASTRA_LF_DELIVER_ONLY) deliver_chunk(c, ctl, e, ch, k, t0, wlen, lane);
-                    else if (fl == ASTRA_LF_FORWARD_ONLY) forward_chunk(c, e, ch, t0, wlen, lane);
-                    else if (fl == ASTRA_LF_CELLS) cells_chunk<1>(c, ctl, e, ch, k, t0, wlen, cb, lane);
-                    else arrivals_link<1>(c, ctl, i, k, t0, wlen, cb, lane);
-                }
-            }
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[1] += (u64)(ck - ck0); ck0 = ck; ctl.clk[0]++; }
-            // stage 2: release + issue.  2a events/releases/mode per GPU; 2b unconstrained wavefront runs,
-            // counted; 2c budget check + bucket bases; 2d commit (or the cycle-serial path); 2e placement.
-            long long ck1 = ck0;
-            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) gpu_prepare(c, ctl, g, t0, t1, lane);
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[8] += (u64)(ck - ck1); ck1 = ck; }
-            for (u32 g = c.g_lo; g < c.g_hi; g++) {
-                if (c.gmode[g] != 1u) continue;
-                for (u32 wi = (warp + nwarps - g % nwarps) % nwarps; wi < c.nwords; wi += nwarps) wf_sim(c, ctl, g, wi, k, t0, t1, lane);
-            }
-            __syncthreads();
-            for (u32 g = c.g_lo; g < c.g_hi; g++) {
-                if (c.gmode[g] != 1u) continue;
-                const u32 nh = c.nheavy[g];
-                for (u32 j = (warp + nwarps - g % nwarps) % nwarps; j < nh; j += nwarps) wf_heavy(c, ctl, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
-            }
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[9] += (u64)(ck - ck1); ck1 = ck; }
-            for (u32 g = c.g_lo + warp; g < c.g_hi; g += nwarps) {
-                if (c.gmode[g] == 1u) {
-                    if (!gpu_binds(c, g, wlen, lane)) { gpu_finalize(c, ctl, g, k, wlen, lane); continue; }
-                    // the budget binds: back to the window start, then exact grants
-                    if (lane == 0) atomicAdd((unsigned long long*)&ctl.clk[6], 1ull);
-                    wf_restore(c, g, lane);
-                    if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
-                    else {
-                        const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-                        for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
-                        if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e0 * c.W + i] = 0;
-                        __syncwarp();
-                        for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, g, wi, k, t0, t1, lane);
-                        gpu_finalize(c, ctl, g, k, wlen, lane);
-                        continue;
-                    }
-                }
-                if (c.gmode[g] != 2u) continue;                  // cycle-serial path
-                ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
-                issue_window(c, ctl, g, t0, t1, cb, lane);
-                for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
-            }
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[10] += (u64)(ck - ck1); ck1 = ck; }
-            for (u32 g = c.g_lo; g < c.g_hi; g++) {
-                if (c.gmode[g] != 1u) continue;
-                const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
-                for (u32 ch = (warp + nwarps - g % nwarps) % nwarps; ch < nch; ch += nwarps) ev_place(c, ctl, g, ch, t0, cb, lane);
-            }
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[11] += (u64)(ck - ck1); ck1 = ck; }
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[2] += (u64)(ck - ck0); ck0 = ck; }
-            // stage 3: merge into multi-feeder out-links (skipped when none received a line)
-            if (ctl.any_merged) {
-                for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps)
-                    if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
-                __syncthreads();
-                if (tid == 0) ctl.any_merged = 0;
-                {
-                    const u32 ng = c.g_hi - c.g_lo, ns = c.i_hi - c.i_lo;
-                    for (u32 task = warp; task < ng + ns; task += nwarps) {
-                        if (task < ng) inject_place(c, c.g_lo + task, wlen, cb, lane);
-                        else arrivals_link<3>(c, ctl, c.i_lo + task - ng, k, t0, wlen, cb, lane);
-                    }
-                    // chunked links that marked cells: same chunks again, now with the FIFO positions known
-                    const u32 ntl = ctl.ntasks;
-                    for (u32 task = nwarps - 1 - warp; task < ntl; task += nwarps) {
-                        u32 lo = c.i_lo, hi = c.i_hi;
-                        while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (c.tbase[mid] > task) hi = mid; else lo = mid + 1; }
-                        const u32 i = lo - 1, e = c.in_link[i];
-                        if (c.lflag[e] == ASTRA_LF_CELLS && !(c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) && c.tl_base[e])
-                            cells_chunk<3>(c, ctl, e, task - c.tbase[i], k, t0, wlen, cb, lane);
-                    }
-                }
-                __syncthreads();
-            }
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[3] += (u64)(ck - ck0); ck0 = ck; }
-            // stage 4: link service per out-link
-            for (u32 e = c.e_lo + warp; e < c.e_hi; e += nwarps) link_service(c, ctl, e, k, t0, t1, cb, lane);
-            __syncthreads();
-            if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[4] += (u64)(ck - ck0); ck0 = ck; }
-            // stage 5: next non-idle window
+            u32* const hp = &ctl.hint[seq % 3];
+            busy += t1 - t0;
+            if (in_set)
+                for (u32 j = set; j < n_nodes; j += nsets)
+                    node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0);
+            // ---- stage 5: next non-idle window (A7), one block barrier per window ----
+#ifdef ASTRA_DIAG
+            dck = clock64();
+#endif
+            u32 hint, acked_total, err;
             if (group > 1) {
+                __syncthreads();
                 if (tid == 0) {
-                    atomicMin(&gc->hint[seq % 3], ctl.next_hint);
-                    if (ctl.acked) { atomicAdd(&gc->acked, ctl.acked); atomicMax(&gc->completion, ctl.completion); }
+                    atomicMin(&gc->hint[seq % 3], *hp);
+                    if (ctl.acked) { atomicAdd(&gc->acked, ctl.acked); atomicMax(&gc->completion, ctl.completion); ctl.acked = 0; }
                     if (ctl.err) atomicOr(&gc->err, ctl.err);
                     if (rank == 0) gc->hint[(seq + 1) % 3] = ASTRA_T_INF;
-                    ctl.acked = 0;
+                    ctl.hint[(seq + 2) % 3] = ASTRA_T_INF;
                 }
-                bar_target += group; group_barrier(gc, bar_target);
-                if (tid == 0) { const long long ck = clock_after_barrier(&ctl.point); ctl.clk[13] += (u64)(ck - ck0); ck0 = ck; }
+                bar_target += group;
+                if (!group_barrier(gc, bar_target, abort_flag, ctl)) { aborted = true; break; }
                 if (tid == 0) {
-                    ctl.next_hint = *(volatile u32*)&gc->hint[seq % 3];
-                    ctl.acked_total = *(volatile u32*)&gc->acked;
-                    ctl.err |= *(volatile u32*)&gc->err;
-                    ctl.completion = *(volatile u32*)&gc->completion;
+                    ctl.g_hint = *(volatile u32*)&gc->hint[seq % 3];
+                    ctl.g_acked = *(volatile u32*)&gc->acked;
+                    ctl.g_err = *(volatile u32*)&gc->err;
+                    ctl.g_completion = *(volatile u32*)&gc->completion;
                 }
-            } else if (tid == 0) { ctl.acked_total += ctl.acked; ctl.acked = 0; }
-            if (tid == 0) {
-                const u32 hint = ctl.next_hint;
-                ctl.next_hint = ASTRA_T_INF;
-                u32 dec = 0, nk = k + 1;
-                if (ctl.acked_total == c.S) dec = 1 + ASTRA_STATUS_DONE;
-                else if (ctl.err) dec = 1 + ASTRA_STATUS_INTERNAL;
-                else if ((u64)(k + 1) * c.W >= c.tmax) dec = 1 + ASTRA_STATUS_MAX_CYCLES;   // events past the watchdog cut are not looked at
-                else if (hint == ASTRA_T_INF) dec = 1 + ASTRA_STATUS_DEADLOCK;
-                else if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint / c.W);
-                ctl.decision = dec; ctl.next_k = nk;
+                __syncthreads();
+                hint = ctl.g_hint; acked_total = ctl.g_acked; err = ctl.g_err;
+            } else {
+                __syncthreads();
+                hint = *hp; acked_total = ctl.acked; err = ctl.err;
+                // slot (seq + 2) % 3 was last read before this barrier and is next written after the next one
+                if (tid == 0) ctl.hint[(seq + 2) % 3] = ASTRA_T_INF;
             }
-            __syncthreads();
+#ifdef ASTRA_DIAG
+            if (in_set && sw == 0 && lane == 0) ctl.sclk[set][7] += (u64)(clock64() - dck);
+            if (tid == 0) ctl.clk[0]++;
+#endif
             seq++;
-            const u32 dec = ctl.decision;
-            if (dec) { status = (int32_t)dec - 1; break; }
-            skipped += (u64)(ctl.next_k - k - 1) * c.W;
-            k = ctl.next_k;
+            // every thread takes the same decision from the same values
+            if (acked_total == c.S) { status = ASTRA_STATUS_DONE; break; }
+            if (err) { status = ASTRA_STATUS_INTERNAL; break; }
+            if ((u64)(k + 1) * W >= c.tmax) { status = ASTRA_STATUS_MAX_CYCLES; break; }   // events past the watchdog cut are not looked at
+            if (hint == ASTRA_T_INF) { status = ASTRA_STATUS_DEADLOCK; break; }
+            u32 nk = k + 1;
+            if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint / W);
+            skipped += (u64)(nk - k - 1) * W;
+            k = nk;
         }
+        if (aborted) break;
         __syncthreads();
         // ---- A8: write-out (each CTA the steps / links of its own nodes) ----
+        u32 cmax = 0;                                       // completion = max t_ack over fully acked steps (R14)
         for (u32 s = tid; s < c.S; s += nthr) {
             const u32 n = c.lines[s];
             const u32 od = c.step_od[s];
@@ -1986,12 +2135,27 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
                 const u32 a = c.t_release[s];
                 c.r_step_ts[4 * (size_t)s + 0] = a == ASTRA_TS_NONE32 ? ~0ull : a;
                 c.r_step_ts[4 * (size_t)s + 1] = c.issued_cnt[s] == n ? (u64)c.t_issued[s] : ~0ull;
-                c.r_step_ts[4 * (size_t)s + 3] = c.ack_cnt[s] == n ? (u64)c.t_ack[s] : ~0ull;
+                const bool acked = c.ack_cnt[s] == n;
+                c.r_step_ts[4 * (size_t)s + 3] = acked ? (u64)c.t_ack[s] : ~0ull;
+                if (acked) cmax = max(cmax, c.t_ack[s]);
             }
             if (ds >= c.g_lo && ds < c.g_hi)
                 c.r_step_ts[4 * (size_t)s + 2] = c.deliv_cnt[s] == n ? (u64)c.t_deliv[s] : ~0ull;
         }
         for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.r_link_lines[e] = c.link_lines[e];
+        cmax = __reduce_max_sync(FULL, cmax);
+        if (tid == 0) ctl.completion = 0;
+        __syncthreads();
+        if (lane == 0 && cmax) atomicMax(&ctl.completion, cmax);
+        __syncthreads();
+        if (group > 1) {
+            if (tid == 0) { gc->completion = 0; }
+            bar_target += group; if (!group_barrier(gc, bar_target, abort_flag, ctl)) break;
+            if (tid == 0) atomicMax(&gc->completion, ctl.completion);
+            bar_target += group; if (!group_barrier(gc, bar_target, abort_flag, ctl)) break;
+            if (tid == 0) ctl.completion = *(volatile u32*)&gc->completion;
+            __syncthreads();
+        }
         if (tid == 0 && rank == 0) {
             DeviceSummary sm;
             sm.status = status; sm.n_steps = c.S; sm.n_links = c.E; sm.window = W;
@@ -1999,15 +2163,25 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
             sm.busy_cycles = busy; sm.skipped_cycles = skipped;
             *c.r_summary = sm;
         }
-        if (tid == 0 && rank == min(group - 1, (c.flags >> 16) & 0xfu)) {     // diagnostics of one CTA of the group
-            for (int i = 0; i < 16; i++) c.r_diag[i] = ctl.clk[i];
-        }
+#ifdef ASTRA_DIAG
+        __syncthreads();
+        if (tid < 16) c.r_diag[(size_t)rank * ASTRA_DIAG_WORDS + tid] = ctl.clk[tid];
+        if (tid < 128) c.r_diag[(size_t)rank * ASTRA_DIAG_WORDS + 16 + tid] = (&ctl.sclk[0][0])[tid];
+#endif
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
+bool astra_engine_has_diag() {
+#ifdef ASTRA_DIAG
+    return true;
+#else
+    return false;
+#endif
+}
+
 u32 astra_engine_fixed_smem(u32 warps) {
     size_t s = ((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)) + (size_t)warps * SCR_WORDS * sizeof(u32);
     return (u32)((s + 127) & ~size_t(127));
@@ -2033,10 +2207,19 @@ int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& er
     e = cudaMemsetAsync(L.d_queue, 0, 4 * sizeof(u32), (cudaStream_t)stream);
     if (e == cudaSuccess && L.n_slots) e = cudaMemsetAsync(L.d_groups, 0, sizeof(GroupCtl) * L.n_slots, (cudaStream_t)stream);
     if (e != cudaSuccess) { err = std::string("queue reset: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
-    astra_step_kernel<<<L.grid, L.warps_per_cta * 32, sm, (cudaStream_t)stream>>>(
-        L.d_const, L.d_ws, L.d_results, L.d_points, L.d_order, L.d_queue, L.d_groups, L.n_points, L.n_big, L.n_slots,
-        L.group, L.ws_big_stride, L.ws_single_off, L.ws_single_stride, fixed);
-    e = cudaGetLastError();
-    if (e != cudaSuccess) { err = std::string("kernel launch: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+    // Cooperative launch: the CTAs of a group spin on each other, so the whole grid must be co-resident.
+    // The runtime guarantees that or refuses the launch (cudaErrorCooperativeLaunchTooLarge) -- never a hang.
+    const uint8_t* a0 = L.d_const; uint8_t* a1 = L.d_ws; uint8_t* a2 = L.d_results; const PointDesc* a3 = L.d_points;
+    const u32* a4 = L.d_order; u32* a5 = L.d_queue; GroupCtl* a6 = L.d_groups;
+    u32 a7 = L.n_points, a8 = L.n_big, a9 = L.n_slots, a10 = L.group;
+    u64 a11 = L.ws_big_stride, a12 = L.ws_single_off, a13 = L.ws_single_stride; u32 a14 = fixed;
+    void* args[] = {&a0, &a1, &a2, &a3, &a4, &a5, &a6, &a7, &a8, &a9, &a10, &a11, &a12, &a13, &a14};
+    e = cudaLaunchCooperativeKernel((const void*)astra_step_kernel, dim3(L.grid), dim3(L.warps_per_cta * 32), args, sm,
+                                    (cudaStream_t)stream);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        err = std::string("cooperative kernel launch: ") + cudaGetErrorString(e);
+        return e == cudaErrorCooperativeLaunchTooLarge ? ASTRA_ELIMIT : ASTRA_ECUDA;
+    }
     return ASTRA_OK;
 }

@@ -26,6 +26,7 @@ typedef uint64_t u64;
 #define ASTRA_NONE32 0xffffffffu
 #define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles
 #define ASTRA_NW_MAX 256                  // ack window bins per GPU
+#define ASTRA_ACK_LIST_CAP 4096u           // ack discovery list entries per (GPU, window bin); beyond: bitmap scan
 #define ASTRA_HEAVY_MIN 8u                // possible issues in a window from which a wavefront gets a warp of its own
 #define ASTRA_HEAVY_MAX_PER_WORD 16        // more such wavefronts among 32 consecutive ones: they stay on their threads
 #define ASTRA_LF_DELIVER_ONLY 1u           // lflag: every line over the link terminates at its head
@@ -58,7 +59,7 @@ typedef uint64_t u64;
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
     X(hlist, u32, 3) X(undo_busy, u64, 3) X(undo_rem, u32, 3) X(undo_cur, u32, 3) X(undo_want, u32, 3) X(undo_freeb, u32, 3) \
-    X(bitmap, u32, 0) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
+    X(bitmap, u32, 0) X(ack_list, u32, 3) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
 
 enum AstraConstId {
 #define X(n) ASTRA_C_##n,
@@ -73,6 +74,7 @@ enum AstraArrId {
     ASTRA_A_COUNT
 };
 
+#define ASTRA_DIAG_WORDS 144                // u64 per CTA: 16 common + 16 warp sets x 8 stage clocks (ASTRA_DIAG builds)
 #define ASTRA_PLACE_SMEM (1ull << 63)     // a_off flag: offset is into the CTA's shared-memory hot region
 
 // Per design point descriptor.  c_off are byte offsets into the batch's constant blob, a_off byte
@@ -84,7 +86,7 @@ struct PointDesc {
     u32 CW, nwords, slots, bmwords;
     u32 Wcyc, NW, kdiv_magic, NC;              // Wcyc lookahead window in cycles; NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
     u32 flags, group;                          // group: CTAs cooperating on this point
-    u32 hot_bytes, pad0;
+    u32 hot_bytes, alcap;                      // alcap: entries per (GPU, window bin) ack discovery list
     u64 max_cycles;
     u64 total_lines;
     u64 ws_bytes;
@@ -171,3 +173,4 @@ struct EngineLaunch {
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err);
 int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err);
 u32 astra_engine_fixed_smem(u32 warps_per_cta);
+bool astra_engine_has_diag();

@@ -194,7 +194,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     P.total_lines = c.total_lines;
     P.flags = (u32)opt.flags;
     P.group = group;
-    u64 tmax = std::min<u64>(opt.max_cycles, 0xffffffffull - (1u << 25));
+    u64 tmax = std::min<u64>(opt.max_cycles, ASTRA_MAX_CYCLES);       // documented clamp (include/astra.h)
     P.max_cycles = tmax;
 
     // lookahead window: min Leff (any value, not only powers of two), capped
@@ -297,7 +297,6 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         if (nd_cellcap[v] == 0) nd_cellcap[v] = 1;
         nd_mw[v] = (nd_cellcap[v] + 31) / 32;
     }
-    if (g.H > 1023) { err = "hbm_lines_per_cycle above the engine limit"; return ASTRA_ELIMIT; }
     std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), inj_off(G + 1, 0);
     u64 ring_total = 0, mask_total = 0, pre_total = 0;
     for (u32 e = 0; e < E; e++) {
@@ -344,6 +343,28 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         for (int it = 0; it < 50; it++) { double mid = 0.5 * (lo + hi); if (fill(mid, nullptr)) hi = mid; else lo = mid; }
         fill(hi, &part);
         part[group] = V;
+        // The bottleneck is usually one heavy node (a switch), and the greedy fill then packs the light nodes
+        // into few ranges and leaves CTAs without nodes.  A node costs its CTA time whatever its load (every
+        // stage of a window is a chain of dependent accesses), so the spare CTAs take the largest ranges apart:
+        // split the heaviest range with more than one node at its best balance point until every CTA has nodes.
+        std::vector<u32> cuts;
+        for (u32 j = 0; j <= group; j++) if (j == 0 || part[j] != part[j - 1]) cuts.push_back(part[j]);
+        if (cuts.back() != V) cuts.push_back(V);
+        std::vector<double> pre(V + 1, 0.0);
+        for (u32 v = 0; v < V; v++) pre[v + 1] = pre[v] + w[v];
+        while (cuts.size() - 1 < group) {
+            size_t best = cuts.size(); double bw = -1.0;
+            for (size_t j = 0; j + 1 < cuts.size(); j++)
+                if (cuts[j + 1] - cuts[j] >= 2 && pre[cuts[j + 1]] - pre[cuts[j]] > bw) { bw = pre[cuts[j + 1]] - pre[cuts[j]]; best = j; }
+            if (best == cuts.size()) break;
+            u32 a = cuts[best], b = cuts[best + 1], cut = a + 1; double bal = 1e300;
+            for (u32 m = a + 1; m < b; m++) {
+                const double d = std::max(pre[m] - pre[a], pre[b] - pre[m]);
+                if (d < bal) { bal = d; cut = m; }
+            }
+            cuts.insert(cuts.begin() + best + 1, cut);
+        }
+        for (u32 j = 0; j <= group; j++) part[j] = j < cuts.size() ? cuts[j] : V;
     }
 
     // all_merged[e]: every link that lines arriving over e are forwarded to has several feeders
@@ -418,6 +439,8 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_wf_busy] = ab[ASTRA_A_undo_busy] = 8ull * GW;
     ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = ab[ASTRA_A_hlist] = 4ull * GW;
     ab[ASTRA_A_bitmap] = 4ull * G * P.NW * P.bmwords;
+    P.alcap = std::min<u32>(slots, ASTRA_ACK_LIST_CAP);
+    ab[ASTRA_A_ack_list] = 4ull * G * P.NW * P.alcap;
     ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
     ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
     ab[ASTRA_A_ring] = 8ull * ring_total;
@@ -428,7 +451,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         // reads or writes: link cursors seen from both ends, ack records / bitmap / bin counts (written
         // at the destination, read at the owner).  Every other array is only ever touched by the CTA
         // that owns the node, so each CTA keeps its own shared-memory copy and uses its nodes' part.
-        bool global_only = a == ASTRA_A_bitmap || a == ASTRA_A_ack_rec || a == ASTRA_A_ack_tmp ||
+        bool global_only = a == ASTRA_A_bitmap || a == ASTRA_A_ack_list || a == ASTRA_A_ack_rec || a == ASTRA_A_ack_tmp ||
                            a == ASTRA_A_ack_sorted || a == ASTRA_A_ring || a == ASTRA_A_evb ||
                            (group > 1 && (a == ASTRA_A_pipe_head || a == ASTRA_A_fifo_head || a == ASTRA_A_bin_cnt || a == ASTRA_A_due_cnt));
         if (!global_only && hot + ab[a] <= opt.hot_budget) { P.a_off[a] = hot | ASTRA_PLACE_SMEM; hot += ab[a]; }

@@ -76,3 +76,29 @@ def test_dbt_each_rank_is_leaf_in_exactly_one_tree():
             assert all(len(c) <= 2 for c in children)
         leaf = [[all(p != r for p in par[t]) for r in range(n)] for t in range(2)]
         assert all(leaf[0][r] != leaf[1][r] for r in range(n))
+
+
+def test_full_size_golden_file_is_complete():
+    """tests/golden/full_size.json (written by tests/golden/make_full_size.py from the oracle) holds a digest
+    record for config 3, config 5 and every one of the 4,096 config-4 points, and a sample of them is
+    reproduced by the oracle here (cheapest points, both scans)."""
+    import hashlib
+    import json
+    import os
+    import numpy as np
+    from oracle import oracle
+    path = os.path.join(os.path.dirname(__file__), "golden", "full_size.json")
+    gold = json.load(open(path))
+    assert set(gold["config3"]) == {"0"} and set(gold["config5"]) == {"0"}
+    assert set(gold["config4"]) == {str(i) for i in range(4096)}
+    for rec in list(gold["config4"].values()) + [gold["config3"]["0"], gold["config5"]["0"]]:
+        status, completion, total, h_ts, h_ll, scan = rec
+        assert status == 0 and completion > 0 and total > 0 and len(h_ts) == 64 and len(h_ll) == 64 and scan in ("plain", "pruned")
+    assert gold["config3"]["0"][2] == 264241152 and gold["config3"]["0"][5] == "plain" and gold["config5"]["0"][5] == "plain"
+    cheap = sorted(range(4096), key=lambda i: gold["config4"][str(i)][2])[:12]
+    for i in cheap:
+        topo, coll, gpu, _ = configs.config4_point(i)
+        for flags in (0, oracle.FLAG_PRUNED_SCAN):
+            r = oracle.run_point(topo, coll, gpu, max_cycles=1 << 26, flags=flags)
+            dig = lambda a: hashlib.sha256(np.ascontiguousarray(a, dtype="<u8").tobytes()).hexdigest()
+            assert [r.status, r.completion, r.total_lines, dig(r.step_ts), dig(r.link_lines)] == gold["config4"][str(i)][:5]
