@@ -11,7 +11,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 # ASTRA_DIAG=1 in the environment selects the instrumented build (build.build(diag=True)); diagnostics only
-_LIBPATH = os.path.join(_HERE, "libastra_b200_diag.so" if os.environ.get("ASTRA_DIAG") == "1" else "libastra_b200.so")
+_LIBPATH = os.path.join(_HERE, "libastra_b200_diag.so" if os.environ.get("ASTRA_DIAG") == "1" else
+                        f"libastra_b200{os.environ.get('ASTRA_LIB_SUFFIX', '')}.so")
 
 EXPORTED_SYMBOLS = [
     "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",

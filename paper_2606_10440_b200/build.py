@@ -34,12 +34,17 @@ def build(force: bool = False, verbose: bool = False, diag: bool = False) -> str
     """The product library (default), or the instrumented one (diag=True: -DASTRA_DIAG adds per-stage SM
     clock counters read by astra_read_diag; never used for a timing that is reported as a result)."""
     lib = LIB_DIAG if diag else LIB
+    # experiments: ASTRA_EXTRA_DEFS="-DX -DY" ASTRA_LIB_SUFFIX=_x builds libastra_b200_x.so with those defines
+    extra = os.environ.get("ASTRA_EXTRA_DEFS", "").split()
+    suffix = os.environ.get("ASTRA_LIB_SUFFIX", "")
+    if suffix:
+        lib = os.path.join(_HERE, f"libastra_b200{suffix}.so")
     if not force and not needs_build(lib):
         return lib
     objs = []
     for s in SOURCES:
-        o = os.path.join(CSRC, os.path.splitext(s)[0] + (".diag.o" if diag else ".o"))
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-DASTRA_DIAG"] if diag else []) + (["-Xptxas", "-v"] if verbose else []) + \
+        o = os.path.join(CSRC, os.path.splitext(s)[0] + suffix + (".diag.o" if diag else ".o"))
+        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-DASTRA_DIAG"] if diag else []) + (["-Xptxas", "-v"] if verbose else []) + \
               ["-x", "cu", "-c", os.path.join(CSRC, s), "-o", o]
         subprocess.check_call(cmd)
         objs.append(o)

@@ -31,7 +31,7 @@ struct astra_ctx {
     u32 *d_order = nullptr, *d_queue = nullptr;
     GroupCtl* d_groups = nullptr;
     u64 const_bytes = 0, ws_big_stride = 0, ws_single_stride = 0, ws_single_off = 0, ws_total = 0, results_bytes = 0;
-    u32 n_big = 0, n_slots = 0, grid = 1, group = 1, warps = 0, hot_bytes = 0;
+    u32 n_big = 0, n_slots = 0, grid = 1, group = 1, warps = 0, hot_bytes = 0, variant = 1;
     std::vector<uint8_t> h_results;
     float last_ms = 0.f;
     u32 last_launches = 0;
@@ -220,6 +220,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     // (128 registers per thread; the shared memory of the SM is split evenly between them)
     c->warps = 16;
     { const u32 wf = (u32)((c->flags >> 20) & 0x3f); if (wf == 1 || wf == 2 || wf == 4 || wf == 8 || wf == 16) c->warps = wf; }
+    c->variant = 1u;
     const u32 ctas_per_sm = 16 / c->warps;
     std::vector<double> cost; std::vector<uint8_t> big;
     classify(c, n, pts, (u32)sms * ctas_per_sm, cost, big, &c->group);
@@ -268,7 +269,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     c->results_bytes = roff ? roff : 16;
     std::string err;
     u32 occ = 0, nsm = 0;
-    int32_t rc = astra_engine_occupancy(c->warps, c->hot_bytes, &occ, &nsm, err);
+    int32_t rc = astra_engine_occupancy(c->warps, c->hot_bytes, c->variant, &occ, &nsm, err);
     if (rc) return fail(c, rc, err);
     if (occ == 0) return fail(c, ASTRA_ECUDA, "kernel does not fit on an SM");
     // every CTA of the grid must be resident at once (persistent CTAs, group barriers)
@@ -336,7 +337,7 @@ extern "C" int32_t astra_run_batch_async(astra_ctx* c, uint32_t n, const astra_p
             L.d_order = c->d_order; L.d_queue = c->d_queue; L.d_groups = c->d_groups; L.n_points = n;
             L.n_big = c->n_big; L.n_slots = c->n_slots; L.group = c->group; L.grid = c->grid;
             L.ws_big_stride = c->ws_big_stride; L.ws_single_off = c->ws_single_off; L.ws_single_stride = c->ws_single_stride;
-            L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes;
+            L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes; L.variant = c->variant;
             std::string err;
             int32_t rc = astra_engine_launch(L, (void*)c->stream, err);
             if (rc) return fail(c, rc, err);

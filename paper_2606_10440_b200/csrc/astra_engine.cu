@@ -193,10 +193,8 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
                         const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
                         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
                         const u32 mb = __match_any_sync(dmask, bin);
-                        u32 lpos = 0;
-                        if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
-                        lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
-                        if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
+                        u32 lpos = 0;                                        // discovery list of the bin: position from the count
+                        if ((mb & lanemask_lt()) == 0) { if (c.alcap) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); else atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); }
                         hint = min(hint, ta);
                         const u32 m = __match_any_sync(dmask, step);
                         const u32 dmax = __reduce_max_sync(m, d);
@@ -205,6 +203,7 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
                             c.deliv_cnt[step] = dc;
                             if (dc == c.lines[step]) { c.t_deliv[step] = t0 + dmax; completed = true; }
                         }
+                        if (c.alcap) { lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt()); if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit; }
                     }
                     if (completed) {      // DELIVERED event at GPU v (dst of the step)
                         const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
@@ -487,10 +486,8 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
         const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
         atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
         const u32 mb = __match_any_sync(amk, bin);
-        u32 lpos = 0;
-        if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
-        lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
-        if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
+        u32 lpos = 0;                                        // discovery list of the bin: position from the count
+        if ((mb & lanemask_lt()) == 0) { if (c.alcap) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); else atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); }
         hint = ta;
         const u32 m = __match_any_sync(amk, step);
         const u32 dmax = __reduce_max_sync(m, d);
@@ -505,6 +502,7 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
         }
         hint = __reduce_min_sync(amk, hint);
         if ((amk & lanemask_lt()) == 0) atomicMin(hp, hint);
+        if (c.alcap) { lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt()); if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit; }
     }
 }
 
@@ -514,7 +512,7 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
 // PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
 template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane);
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 rel, u32 lane);
 
 // A task is 64 entries: both halves' ring loads (and the look-back) are in flight before the first use.
 template <int PASS>
@@ -534,12 +532,12 @@ __device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e,
     const u32 da0 = __shfl_sync(FULL, da, 0), db0 = __shfl_sync(FULL, db, 0);
     const u32 back_a = __popc(__ballot_sync(FULL, dz == da0));          // same-cycle lines before the task
     const u32 back_b = __popc(__ballot_sync(FULL, da == db0));          // ... before its second half
-    cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, lane);   // d >= wlen: watchdog cut inside the window
-    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, lane);
+    cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, chunk * 64 + lane, lane);   // d >= wlen: watchdog cut inside the window
+    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, chunk * 64 + 32 + lane, lane);
 }
 
 template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 lane) {
+__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 rel, u32 lane) {
     const u32 vmask = __ballot_sync(FULL, valid);
     if (!valid) return;
     const u32 grp = __match_any_sync(vmask, d);
@@ -549,10 +547,14 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, 
     const u32 od = c.step_od[step];
     const u32 dstg = od & 0xffffu;
     const bool deliver = dstg == v;
+    if (PASS == 1) c.lscr[c.lscr_off[e] + rel] = ASTRA_NONE32;      // overwritten below for a line that goes on
     if (!deliver) {
         const u32 o = c.next_link[(size_t)v * c.G + dstg];
-        if (PASS == 1) { cell_set(c, o, v, cb, d, c.classoff[e] + r); c.tl_base[e] = 1u; }
-        else {
+        if (PASS == 1) {
+            const u32 slot = c.classoff[e] + r;
+            cell_set(c, o, v, cb, d, slot); c.tl_base[e] = 1u;
+            c.lscr[c.lscr_off[e] + rel] = (o << 12) | slot;           // the placement pass reads this instead of routing again
+        } else {
             const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, c.classoff[e] + r);
             c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
         }
@@ -568,10 +570,8 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, 
             const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
             atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
             const u32 mb = __match_any_sync(dmask, bin);
-            u32 lpos = 0;
-            if ((mb & lanemask_lt()) == 0) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb));
-            lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt());
-            if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit;     // discovery list of the bin (any order)
+            u32 lpos = 0;                                        // discovery list of the bin: position from the count
+            if ((mb & lanemask_lt()) == 0) { if (c.alcap) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); else atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); }
             const u32 m = __match_any_sync(dmask, step);
             const u32 dmax = __reduce_max_sync(m, d);
             if ((m & lanemask_lt()) == 0) {
@@ -585,7 +585,32 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, 
             }
             const u32 hint = __reduce_min_sync(dmask, ta);
             if ((dmask & lanemask_lt()) == 0) atomicMin(hp, hint);
+            if (c.alcap) { lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt()); if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit; }
         }
+    }
+}
+
+// Placement pass of such a link (after the cell prefix sums): the lines that go on are written to their
+// FIFO positions; out-link and cell slot of every line were recorded by pass 1.
+__device__ void cells_place_chunk(const Ctx& __restrict__ c, u32 e, u32 lo, u32 n, u32 chunk, u32 t0, u32 wlen, u32 cb, u32 lane) {
+    const u64* ring = c.ring + c.ring_off[e];
+    const u32 rmask = c.ring_mask[e];
+    const u32* scr = c.lscr + c.lscr_off[e];
+    const u32 v = c.head[e];
+    const u32 r0 = chunk * 64 + lane, r1 = r0 + 32;
+    const u64 fa = r0 < n ? __ldcg(&ring[(lo + r0) & rmask]) : 0ull;
+    const u64 fb = r1 < n ? __ldcg(&ring[(lo + r1) & rmask]) : 0ull;
+    const u32 sa = r0 < n ? scr[r0] : ASTRA_NONE32;
+    const u32 sb = r1 < n ? scr[r1] : ASTRA_NONE32;
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        const u64 flit = h ? fb : fa;
+        const u32 sc = h ? sb : sa;
+        const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
+        if ((h ? r1 : r0) >= n || d >= wlen || sc == ASTRA_NONE32) continue;     // d >= wlen: watchdog cut inside the window
+        const u32 o = sc >> 12;
+        const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, sc & 0xfffu);
+        c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
     }
 }
 
@@ -1057,7 +1082,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
 #pragma unroll
                 for (int q = 0; q < 4; q++) if ((u32)q < nb) {
                     const u32 t2 = bb[q] >> 6;
-                    if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT);
+                    if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
                     if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
                 }
                 nb = 0;
@@ -1071,7 +1096,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
 #pragma unroll
             for (int q = 0; q < 4; q++) if ((u32)q < nb) {
                 const u32 t2 = bb[q] >> 6;
-                if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT);
+                if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
                 if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
             }
         }
@@ -1194,7 +1219,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
                 const u32 slot = i < F0 ? scr[128 + i] : (key & 63u);
                 if (slot < 32) im_lo |= 1u << slot; else im_hi |= 1u << (slot - 32);
                 const u32 p = atomicAdd(&cnt[x], 1u);
-                if (p < H) evb[(size_t)x * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(x + 1) << ASTRA_FLIT_TIME_SHIFT);
+                if (p < H) evb[(size_t)x * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(x + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
                 if (deg > 1) atomicAdd(&h[ox * W + x], 1u);
             }
             if (nv) {
@@ -1330,7 +1355,7 @@ __device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u
             if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; have_s = true; }
             const u32 slot = __ffsll((long long)~busy) - 1;
             busy |= 1ull << slot;
-            evb[(size_t)T * H + rank] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(T + 1) << ASTRA_FLIT_TIME_SHIFT);
+            evb[(size_t)T * H + rank] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(T + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
             if (deg > 1) atomicAdd(&h[ox * W + T], 1u);
             last_issue = T;
             if (--rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
@@ -1380,38 +1405,47 @@ __device__ bool gpu_binds(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 lane) 
     return __any_sync(FULL, bind);
 }
 
-__device__ void gpu_finalize(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 wlen, u32 lane) {
+// The run stands (no cycle exceeded H, or the exact grants were computed): three independent parts that
+// different warps of the set take -- (a) exclusive prefix of the per-cycle issue counts = item enumeration
+// of the window (written to pfx: cnt stays readable for the budget check of the other warps), (b) per
+// out-link the absolute FIFO position of each cycle's first line, (c) the window's ack bits are consumed.
+__device__ void gpu_finalize_counts(const Ctx& __restrict__ c, u32 g, u32 k, u32 wlen, u32 lane) {
     const u32 W = c.W;
-    u32* cnt = c.cnt + (size_t)g * W;
+    const u32* cnt = c.cnt + (size_t)g * W;
+    u32* pfx = c.pfx + (size_t)g * W;
     u32 carry = 0;
     for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
         const u32 v = (i < wlen) ? cnt[i] : 0;
         const u32 incl = warp_incl_scan(v, lane);
-        if (i < W) cnt[i] = carry + incl - v;
+        if (i < W) pfx[i] = carry + incl - v;
         carry += __shfl_sync(FULL, incl, 31);
     }
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-    if (deg == 1) {
-        if (lane == 0 && carry && c.mask_off[e0] == ASTRA_NONE32) c.run[e0] += carry;
-    } else if (carry) {
-        for (u32 x = 0; x < deg; x++) {                         // per out-link: absolute FIFO position of each cycle's first line
-            u32* h = c.hist + (size_t)(e0 + x) * W;
-            const bool direct = c.mask_off[e0 + x] == ASTRA_NONE32;
-            u32 acc = direct ? c.run[e0 + x] : 0u;
-            const u32 acc0 = acc;
-            for (u32 b = 0; b < W; b += 32) {
-                const u32 i = b + lane;
-                const u32 v = (i < wlen) ? h[i] : 0;
-                const u32 incl = warp_incl_scan(v, lane);
-                if (i < W) h[i] = acc + incl - v;
-                acc += __shfl_sync(FULL, incl, 31);
-            }
-            __syncwarp();
-            if (lane == 0 && direct && acc != acc0) c.run[e0 + x] = acc;
-        }
+    if (lane == 0) {
+        if (deg == 1 && carry && c.mask_off[e0] == ASTRA_NONE32) c.run[e0] += carry;
+        c.sel[(size_t)g * c.H] = carry;                         // issues of the GPU this window (sel is free on this path)
+        c.pcnt[g] = 0;
+        c.bin_cnt[g * c.NW + (k & c.NWmask)] = 0;
     }
-    // consume the acks of the window's bin and the releases
+}
+__device__ void gpu_finalize_link(const Ctx& __restrict__ c, u32 e, u32 wlen, u32 lane) {
+    const u32 W = c.W;
+    u32* h = c.hist + (size_t)e * W;
+    const bool direct = c.mask_off[e] == ASTRA_NONE32;
+    u32 acc = direct ? c.run[e] : 0u;
+    const u32 acc0 = acc;
+    for (u32 b = 0; b < W; b += 32) {
+        const u32 i = b + lane;
+        const u32 v = (i < wlen) ? h[i] : 0;
+        const u32 incl = warp_incl_scan(v, lane);
+        if (i < W) h[i] = acc + incl - v;
+        acc += __shfl_sync(FULL, incl, 31);
+    }
+    __syncwarp();
+    if (lane == 0 && direct && acc != acc0) c.run[e] = acc;
+}
+__device__ void gpu_finalize_acks(const Ctx& __restrict__ c, u32 g, u32 k, u32 lane) {
     const u32 n_ack = c.ack_n[g];
     if (n_ack) {
         u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
@@ -1421,11 +1455,12 @@ __device__ void gpu_finalize(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, 
         } else for (u32 i = lane; i < c.bmwords; i += 32) bm[i] = 0;
     }
     for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
-    if (lane == 0) {
-        c.sel[(size_t)g * c.H] = carry;                         // issues of the GPU this window (sel is free on this path)
-        c.pcnt[g] = 0;
-        c.bin_cnt[g * c.NW + (k & c.NWmask)] = 0;
-    }
+}
+__device__ void gpu_finalize(const Ctx& __restrict__ c, u32 g, u32 k, u32 wlen, u32 lane) {   // all parts on one warp
+    gpu_finalize_counts(c, g, k, wlen, lane);
+    const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
+    if (deg > 1) for (u32 x = 0; x < deg; x++) gpu_finalize_link(c, e0 + x, wlen, lane);
+    gpu_finalize_acks(c, g, k, lane);
     __syncwarp();
 }
 
@@ -1435,36 +1470,47 @@ __device__ void gpu_finalize(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, 
 // last cycle tt with cnt[tt] <= i (cnt = exclusive prefix of the per-cycle issue counts).
 __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 t0, u32 cb, u32 lane) {
     const u32 nev = c.sel[(size_t)g * c.H];
-    const u32 i = chunk * 32 + lane;
+    const u32 cs = chunk * 32, i = cs + lane;
     const bool act = i < nev;
     const u32 amk = __ballot_sync(FULL, act);
-    if (!act) return;
     const u32 W = c.W, H = c.H;
-    const u32* cnt = c.cnt + (size_t)g * W;
-    u32 lo = 0, hi = W;                                         // first index with cnt > i
-    while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (cnt[mid] > i) hi = mid; else lo = mid + 1; }
-    const u32 tt = lo - 1;
-    const u32 st = cnt[tt], n = (tt + 1 < W ? cnt[tt + 1] : nev) - st;
-    const u64* bucket = c.evb + ((size_t)g * W + tt) * H;
-    const u64 rec = bucket[i - st];
-    const u32 s = (u32)rec & 0xfffffu, wf = ((u32)rec >> 20) & 0xfffu;
-    const u32 d = tt + 1;
+    const u32* cnt = c.pfx + (size_t)g * W;                    // exclusive prefix of the per-cycle issue counts
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-    const u32 o = c.first_link[s];
+    u32 tt = 0xffffffffu, st = 0, n = 0, s = 0, wf = 0, o = 0;
+    u64 rec = 0;
+    const u64* bucket = nullptr;
+    if (act) {
+        u32 lo = 0, hi = W;                                     // first index with cnt > i
+        while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (cnt[mid] > i) hi = mid; else lo = mid + 1; }
+        tt = lo - 1;
+        st = cnt[tt]; n = (tt + 1 < W ? cnt[tt + 1] : nev) - st;
+        bucket = c.evb + ((size_t)g * W + tt) * H;
+        rec = bucket[i - st];
+        s = (u32)rec & 0xfffffu; wf = ((u32)rec >> 20) & 0xfffu;
+        o = c.first_link[s];
+    }
+    if (!act) return;
+    // rank among the issues of the same cycle (j) and among those that take the same out-link (jo); a bucket
+    // holds at most H records, each with its wavefront id and out-link (bits 48.. of the record)
     u32 j = 0, jo = 0;
+    const u32 oxm = o - e0;
     for (u32 x = 0; x < n; x++) {
-        const u32 r2 = (u32)bucket[x];
-        const bool lower = ((r2 >> 20) & 0xfffu) < wf;
+        const u64 r2 = bucket[x];
+        const bool lower = (((u32)r2 >> 20) & 0xfffu) < wf;
         j += lower;
-        if (deg > 1) jo += lower && c.first_link[r2 & 0xfffffu] == o;
+        jo += lower && (u32)(r2 >> 48) == oxm;
     }
     if (deg == 1) jo = j;
+    const u32 d = tt + 1;
     if (c.mask_off[o] == ASTRA_NONE32) {
         const u32 pos = (deg == 1 ? c.run[o] - nev + st : c.hist[(size_t)o * W + tt]) + jo;
         c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
     } else {
         cell_set(c, o, g, cb, d, c.nd_injoff[g] + j);
-        const u32 p = atomicAdd(&c.inj_n[g], 1u);
+        const u32 mm = __activemask();                          // one counter bump for the lanes that record an injection
+        u32 p = 0;
+        if ((mm & lanemask_lt()) == 0) p = atomicAdd(&c.inj_n[g], (u32)__popc(mm));
+        p = __shfl_sync(mm, p, __ffs(mm) - 1) + __popc(mm & lanemask_lt());
         if (p < c.inj_off[g + 1] - c.inj_off[g]) c.inj_list[c.inj_off[g] + p] = (rec & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)(d | (j << 10)) << ASTRA_FLIT_TIME_SHIFT);
         else atomicOr(&ctl.err, 4u);
     }
@@ -1480,18 +1526,31 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
 // ---------------------------------------------------------------------------------------------
 __device__ void link_prefix(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, u32 lane) {
     const u32 v = c.tail[o];
-    const u32 mw = c.nd_mw[v];
+    const u32 mw = c.nd_mw[v], NC = c.NC;
     const u32* masks = c.masks + c.mask_off[o];
     u32* pre = c.pre + c.pre_off[o];
     u32 n_new = 0;
-    for (u32 b = 0; b < wlen; b += 32) {
-        const u32 tau = b + lane; u32 cnt = 0;
-        if (tau < wlen) {
-            u32 ci = cb + tau; if (ci >= c.NC) ci -= c.NC;
-            for (u32 w = 0; w < mw; w++) cnt += __popc(masks[ci * mw + w]);
+    // four consecutive cycles per lane: their cell words are loaded together, one warp scan per 128 cycles
+    for (u32 b = 0; b < wlen; b += 128) {
+        u32 cq[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const u32 tau = b + 4 * lane + q;
+            cq[q] = 0;
+            if (tau < wlen) {
+                u32 ci = cb + tau; if (ci >= NC) ci -= NC;
+                for (u32 w = 0; w < mw; w++) cq[q] += __popc(masks[ci * mw + w]);
+            }
         }
-        const u32 incl = warp_incl_scan(cnt, lane);
-        if (tau < wlen) pre[tau] = n_new + incl - cnt;
+        const u32 tot = cq[0] + cq[1] + cq[2] + cq[3];
+        const u32 incl = warp_incl_scan(tot, lane);
+        u32 run = n_new + incl - tot;
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const u32 tau = b + 4 * lane + q;
+            if (tau < wlen) pre[tau] = run;
+            run += cq[q];
+        }
         n_new += __shfl_sync(FULL, incl, 31);
     }
     if (lane == 0) c.run[o] = c.ltail[o] + n_new;
@@ -1538,9 +1597,10 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
         const u32 v = c.tail[e];
         const u32 mw = c.nd_mw[v];
         u32* masks = c.masks + c.mask_off[e];
-        for (u32 x = lane; x < wlen * mw; x += 32) {
-            u32 ci = cb + x / mw; if (ci >= c.NC) ci -= c.NC;
-            masks[ci * mw + x % mw] = 0;
+        {   // cells [cb, cb + wlen) of the circular array: one or two contiguous word ranges
+            const u32 end1 = min(cb + wlen, c.NC);
+            for (u32 x = cb * mw + lane; x < end1 * mw; x += 32) masks[x] = 0;
+            if (cb + wlen > c.NC) for (u32 x = lane; x < (cb + wlen - c.NC) * mw; x += 32) masks[x] = 0;
         }
         __syncwarp();
         if (lane == 0) {                                     // injections that enter at t1 keep the link marked
@@ -1571,7 +1631,6 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
     } else if (kind == ASTRA_LK_GENERAL) { cr = c.lstate0[e]; tc = c.lstate1[e]; }
     const u32 capq = c.ceilb[e] * 256u;
     u32 n_acc = 0, first_x = 0, last_x = 0;
-
     if (kind != ASTRA_LK_GENERAL) {
         // 128 entries per step, four consecutive ones per lane: local running max, then one warp scan
         const int P = (int)param;
@@ -1792,7 +1851,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     if (is_gpu) {
         if (sw == 0) stage1_setup_gpu(c, ctl, hp, v, k, lane);
         const u32 n_ack = ld_vol(&c.bin_cnt[v * c.NW + kb]);
-        if (n_ack && n_ack <= c.alcap) {
+        if (n_ack && n_ack <= c.alcap) {                         // alcap == 0: no list, the bitmap is scanned
             for (u32 ch = sw; ch * 128 < n_ack; ch += ws) ack_list_chunk(c, ctl, v, ch, n_ack, k, t1, lane);
         } else if (n_ack) {
             const u32 nch = (c.bmwords + 31) / 32;
@@ -1859,21 +1918,25 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
                 set_sync(ws, set);
             }
             DIAG_CLK(2);
-            if (sw == 0) {
-                if (!gpu_binds(c, g, wlen, lane)) gpu_finalize(c, ctl, g, k, wlen, lane);
+            const bool bind = gpu_binds(c, g, wlen, lane);     // every warp checks: the same answer everywhere ...
+            set_sync(ws, set);                                  // ... before anybody writes over the counts
+            if (!bind) {                                        // the parts of the commit are dealt out
+                const u32 deg = e_hi - e_lo;
+                if (sw == 0) gpu_finalize_counts(c, g, k, wlen, lane);
+                if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) gpu_finalize_link(c, e_lo + x, wlen, lane);
+                if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
+            } else if (sw == 0) {
+                // the budget binds: back to the window start, then exact grants
+                if (lane == 0) DIAG_ADD(6, 1);
+                wf_restore(c, g, lane);
+                if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
                 else {
-                    // the budget binds: back to the window start, then exact grants
-                    if (lane == 0) DIAG_ADD(6, 1);
-                    wf_restore(c, g, lane);
-                    if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
-                    else {
-                        const u32 deg = e_hi - e_lo;
-                        for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
-                        if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
-                        __syncwarp();
-                        for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
-                        gpu_finalize(c, ctl, g, k, wlen, lane);
-                    }
+                    const u32 deg = e_hi - e_lo;
+                    for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
+                    if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
+                    __syncwarp();
+                    for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+                    gpu_finalize(c, g, k, wlen, lane);
                 }
             }
             set_sync(ws, set);
@@ -1924,7 +1987,9 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
                 const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
                 const u32 rot = (ib - i_lo + src) % ws;
                 if (fl == 0u) { if (sw == rot) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); continue; }
-                for (u32 ch = (sw + ws - rot) % ws; ch * 64 < n; ch += ws) cells_chunk<3>(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
+                for (u32 ch = (sw + ws - rot) % ws; ch * 64 < n; ch += ws) {
+                    cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
+                }
             }
         }
         set_sync(ws, set);
@@ -1947,8 +2012,8 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     DIAG_CLK(6);
 }
 
-extern "C" __global__ void __launch_bounds__(512, 1)
-astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
+__device__ __forceinline__ void
+step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
                   GroupCtl* groups, u32 n_points, u32 n_big, u32 n_slots, u32 group0,
                   u64 ws_big_stride, u64 ws_single_off, u64 ws_single_stride, u32 hot_off) {
@@ -2171,6 +2236,15 @@ astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_ba
     }
 }
 
+// The step kernel: 128 registers per thread; 16 warps per CTA and one CTA per SM unless ASTRA_FLAG_WARPS says otherwise.
+extern "C" __global__ void __launch_bounds__(512, 1)
+astra_step_kernel(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
+                  const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
+                  GroupCtl* groups, u32 n_points, u32 n_big, u32 n_slots, u32 group0,
+                  u64 ws_big_stride, u64 ws_single_off, u64 ws_single_stride, u32 hot_off) {
+    step_kernel_body(cblob, ws_base, results, points, order, queue, groups, n_points, n_big, n_slots, group0,
+                     ws_big_stride, ws_single_off, ws_single_stride, hot_off);
+}
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
@@ -2187,13 +2261,15 @@ u32 astra_engine_fixed_smem(u32 warps) {
     return (u32)((s + 127) & ~size_t(127));
 }
 
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err) {
+static const void* kernel_variant(u32) { return (const void*)astra_step_kernel; }
+
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, u32* ctas_per_sm, u32* n_sms, std::string& err) {
     int dev = 0, sms = 0, occ = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     size_t sm = (size_t)astra_engine_fixed_smem(warps_per_cta) + hot_bytes;
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, astra_step_kernel, (int)warps_per_cta * 32, sm);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel_variant(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_variant(variant), (int)warps_per_cta * 32, sm);
     if (e != cudaSuccess) { err = std::string("occupancy query: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
     *ctas_per_sm = (u32)occ; *n_sms = (u32)sms;
     return ASTRA_OK;
@@ -2202,7 +2278,7 @@ int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_s
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err) {
     const u32 fixed = astra_engine_fixed_smem(L.warps_per_cta);
     size_t sm = (size_t)fixed + L.hot_bytes;
-    cudaError_t e = cudaFuncSetAttribute(astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    cudaError_t e = cudaFuncSetAttribute(kernel_variant(L.variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) { err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
     e = cudaMemsetAsync(L.d_queue, 0, 4 * sizeof(u32), (cudaStream_t)stream);
     if (e == cudaSuccess && L.n_slots) e = cudaMemsetAsync(L.d_groups, 0, sizeof(GroupCtl) * L.n_slots, (cudaStream_t)stream);
@@ -2214,7 +2290,7 @@ int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& er
     u32 a7 = L.n_points, a8 = L.n_big, a9 = L.n_slots, a10 = L.group;
     u64 a11 = L.ws_big_stride, a12 = L.ws_single_off, a13 = L.ws_single_stride; u32 a14 = fixed;
     void* args[] = {&a0, &a1, &a2, &a3, &a4, &a5, &a6, &a7, &a8, &a9, &a10, &a11, &a12, &a13, &a14};
-    e = cudaLaunchCooperativeKernel((const void*)astra_step_kernel, dim3(L.grid), dim3(L.warps_per_cta * 32), args, sm,
+    e = cudaLaunchCooperativeKernel(kernel_variant(L.variant), dim3(L.grid), dim3(L.warps_per_cta * 32), args, sm,
                                     (cudaStream_t)stream);
     if (e != cudaSuccess) {
         (void)cudaGetLastError();

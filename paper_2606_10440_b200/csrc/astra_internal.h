@@ -45,7 +45,7 @@ typedef uint64_t u64;
     X(step_od) X(lines) X(cu_lo) X(cu_n) X(succ_ptr) X(succ) X(ndeps) \
     X(step_q) X(step_r) X(first_link) X(step_alpha) X(step_aq) X(step_ar) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
     X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(classoff) \
-    X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(gflag) X(lflag) X(lfwd)
+    X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(gflag) X(lflag) X(lfwd) X(lscr_off)
 
 // Mutable arrays of a design point.  X(name, element type, init) with init: 0 zero, 1 0xff bytes,
 // 2 written by the kernel's own initialisation, 3 scratch (no initialisation).
@@ -54,12 +54,12 @@ typedef uint64_t u64;
 #define ASTRA_WS_ARRAYS(X) \
     X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
     X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(due_cnt, u32, 0) X(tl_lo, u32, 3) X(tl_n, u32, 3) X(tl_base, u32, 3) X(tbase, u32, 3) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
-    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(pfx, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
     X(hlist, u32, 3) X(undo_busy, u64, 3) X(undo_rem, u32, 3) X(undo_cur, u32, 3) X(undo_want, u32, 3) X(undo_freeb, u32, 3) \
-    X(bitmap, u32, 0) X(ack_list, u32, 3) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
+    X(lscr, u32, 3) X(bitmap, u32, 0) X(ack_list, u32, 3) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
 
 enum AstraConstId {
 #define X(n) ASTRA_C_##n,
@@ -169,8 +169,9 @@ struct EngineLaunch {
     u32 n_big, n_slots, group, grid;
     u64 ws_big_stride, ws_single_off, ws_single_stride;
     u32 warps_per_cta, hot_bytes;
+    u32 variant;                    // 1: one CTA per SM (128 registers per thread), 2: two CTAs per SM (64)
 };
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err);
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32* ctas_per_sm, u32* n_sms, std::string& err);
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, u32* ctas_per_sm, u32* n_sms, std::string& err);
 u32 astra_engine_fixed_smem(u32 warps_per_cta);
 bool astra_engine_has_diag();

@@ -386,6 +386,16 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         else if (transits[e] && !delivers[e] && !multi_fwd[e] && !multi[fwd[e]]) { lflag[e] = ASTRA_LF_FORWARD_ONLY; lfwd[e] = fwd[e]; }
         else if (transits[e] && all_merged[e]) lflag[e] = ASTRA_LF_CELLS;
     }
+    // links on the cell path record (out-link, cell slot) per line of a window for the placement pass: 20 + 12 bits
+    std::vector<u32> lscr_off(E, 0);
+    u64 lscr_total = 0;
+    for (u32 e = 0; e < E; e++) {
+        if (lflag[e] != ASTRA_LF_CELLS) continue;
+        if (E >= (1u << 20) || nd_cellcap[t.head[e]] > 4096) { err = "too many links or cell slots for the merge path"; return ASTRA_ELIMIT; }
+        lscr_off[e] = (u32)lscr_total;
+        lscr_total += (u64)ceilb_v[e] * W;
+        if (lscr_total >= (1ull << 31)) { err = "merge scratch exceeds 2^31 words"; return ASTRA_ELIMIT; }
+    }
     // per-GPU flags: a GPU whose steps have ISSUED-kind successors always takes the cycle-serial issue path
     std::vector<u32> gflag(G, 0);
     for (u32 s = 0; s < S; s++)
@@ -415,6 +425,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_part] = blob.add(part);
     co[ASTRA_C_gflag] = blob.add(gflag);
     co[ASTRA_C_lflag] = blob.add(lflag); co[ASTRA_C_lfwd] = blob.add(lfwd);
+    co[ASTRA_C_lscr_off] = blob.add(lscr_off);
 
     // mutable arrays: sizes, then placement (shared memory in declaration order while it fits)
     const u64 GW = (u64)G * CW;
@@ -426,7 +437,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
     ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
     ab[ASTRA_A_gmode] = ab[ASTRA_A_nheavy] = 4ull * G;
-    ab[ASTRA_A_cnt] = 4ull * G * W;
+    ab[ASTRA_A_cnt] = ab[ASTRA_A_pfx] = 4ull * G * W;
     ab[ASTRA_A_undo_want] = ab[ASTRA_A_undo_freeb] = 4ull * G * P.nwords;
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
     ab[ASTRA_A_evb] = 8ull * G * g.H * W;
@@ -438,9 +449,18 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_bin_cnt] = 4ull * G * P.NW;
     ab[ASTRA_A_wf_busy] = ab[ASTRA_A_undo_busy] = 8ull * GW;
     ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = ab[ASTRA_A_hlist] = 4ull * GW;
+    ab[ASTRA_A_lscr] = 4ull * lscr_total;
     ab[ASTRA_A_bitmap] = 4ull * G * P.NW * P.bmwords;
-    P.alcap = std::min<u32>(slots, ASTRA_ACK_LIST_CAP);
-    ab[ASTRA_A_ack_list] = 4ull * G * P.NW * P.alcap;
+    // Ack discovery: a list per (GPU, window bin) that deliveries append to -- or, when the bitmap of a bin is a
+    // few 32-word chunks per warp of the node's set anyway, the scan of the bitmap itself (the append costs every
+    // delivery the round trip of a counting atomic).
+    {
+        const u32 nodes_per_cta = (V + group - 1) / group;
+        const u32 ws = std::max<u32>(1, 16 / std::min<u32>(16, nodes_per_cta));
+        const u32 chunks = (P.bmwords + 31) / 32;
+        P.alcap = chunks > 4 * ws ? std::min<u32>(slots, ASTRA_ACK_LIST_CAP) : 0u;
+    }
+    ab[ASTRA_A_ack_list] = 4ull * G * P.NW * P.alcap;      // 0 entries: no list
     ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
     ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
     ab[ASTRA_A_ring] = 8ull * ring_total;

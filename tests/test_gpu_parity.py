@@ -94,6 +94,37 @@ def test_cta_groups(group):
     check_workload(configs.config5(n_nodes=4), flags=FLAG_GROUP(group), oracle_flags=oracle.FLAG_PRUNED_SCAN)
 
 
+@pytest.mark.parametrize("warps", [1, 2, 4, 8])
+def test_warp_sets(warps):
+    """CTAs of fewer warps (ASTRA_FLAG_WARPS): a warp set then steps several simulated nodes one after the other,
+    or a node gets a set of 1, 2, 4, 8 warps -- every split of a CTA's warps over its nodes gives the same bits."""
+    from paper_2606_10440_b200.binding import FLAG_GROUP, FLAG_WARPS
+    check_workload(configs.config1(), flags=FLAG_WARPS(warps))
+    check_workload(configs.random_workload(23, n_points=6, max_gpus=6, max_steps=24, max_lines=200), flags=FLAG_WARPS(warps))
+    check_workload(configs.config2(range(6, 8)), flags=FLAG_WARPS(warps) | FLAG_GROUP(1), processes=4)
+    check_workload(configs.config4(8), flags=FLAG_WARPS(warps), oracle_flags=oracle.FLAG_PRUNED_SCAN, processes=8)
+    check_workload(configs.config5(n_nodes=4), flags=FLAG_WARPS(warps) | FLAG_GROUP(3), oracle_flags=oracle.FLAG_PRUNED_SCAN)
+
+
+def test_two_contexts_run_concurrently():
+    """Two astra_ctx on the same device, each with its own stream, both launched before either is waited for:
+    the cooperative launches are serialised or co-scheduled by the runtime, never deadlocked, and both give the
+    oracle's bits."""
+    from paper_2606_10440_b200 import Engine
+    wa = configs.config2(range(6, 12))
+    wb = configs.config5(n_nodes=4)
+    with Engine() as ea, Engine() as eb:
+        pa, pb = ea.load_workload(wa), eb.load_workload(wb)
+        ea.run_batch(pa, wa.max_cycles, asynchronous=True)
+        eb.run_batch(pb, wb.max_cycles, asynchronous=True)
+        ea.sync(); eb.sync()
+        ra = [ea.read_results(i) for i in range(len(pa))]
+        rb = [eb.read_results(i) for i in range(len(pb))]
+    for i, r in enumerate(oracle.run_workload(wa, processes=6)):
+        compare_point(ra[i], r, label=f"ctx A point {i}")
+    compare_point(rb[0], oracle.run_workload(wb, flags=oracle.FLAG_PRUNED_SCAN)[0], label="ctx B")
+
+
 def test_named_families_small():
     gpu = GpuCfg(8, 2, 4, 6)
     cases = [
