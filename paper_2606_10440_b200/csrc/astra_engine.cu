@@ -547,7 +547,7 @@ __device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, 
     const u32 od = c.step_od[step];
     const u32 dstg = od & 0xffffu;
     const bool deliver = dstg == v;
-    if (PASS == 1) c.lscr[c.lscr_off[e] + rel] = ASTRA_NONE32;      // overwritten below for a line that goes on
+    if (PASS == 1 && deliver) c.lscr[c.lscr_off[e] + rel] = ASTRA_NONE32;      // nothing to place for a line that ends here
     if (!deliver) {
         const u32 o = c.next_link[(size_t)v * c.G + dstg];
         if (PASS == 1) {
@@ -1407,18 +1407,17 @@ __device__ bool gpu_binds(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 lane) 
 
 // The run stands (no cycle exceeded H, or the exact grants were computed): three independent parts that
 // different warps of the set take -- (a) exclusive prefix of the per-cycle issue counts = item enumeration
-// of the window (written to pfx: cnt stays readable for the budget check of the other warps), (b) per
+// of the window (in place: every warp has finished its budget check by then, see node_window), (b) per
 // out-link the absolute FIFO position of each cycle's first line, (c) the window's ack bits are consumed.
 __device__ void gpu_finalize_counts(const Ctx& __restrict__ c, u32 g, u32 k, u32 wlen, u32 lane) {
     const u32 W = c.W;
-    const u32* cnt = c.cnt + (size_t)g * W;
-    u32* pfx = c.pfx + (size_t)g * W;
+    u32* cnt = c.cnt + (size_t)g * W;
     u32 carry = 0;
     for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
         const u32 v = (i < wlen) ? cnt[i] : 0;
         const u32 incl = warp_incl_scan(v, lane);
-        if (i < W) pfx[i] = carry + incl - v;
+        if (i < W) cnt[i] = carry + incl - v;
         carry += __shfl_sync(FULL, incl, 31);
     }
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
@@ -1474,7 +1473,7 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
     const bool act = i < nev;
     const u32 amk = __ballot_sync(FULL, act);
     const u32 W = c.W, H = c.H;
-    const u32* cnt = c.pfx + (size_t)g * W;                    // exclusive prefix of the per-cycle issue counts
+    const u32* cnt = c.cnt + (size_t)g * W;                    // by now the exclusive prefix of the per-cycle issue counts
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
     u32 tt = 0xffffffffu, st = 0, n = 0, s = 0, wf = 0, o = 0;
     u64 rec = 0;
@@ -1784,12 +1783,17 @@ __device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8
 #define X(n) c.n = (const u32*)(cb + P.c_off[ASTRA_C_##n]);
     ASTRA_CONST_TABLES(X)
 #undef X
-#define X(n, t, i) c.n = (t*)(((P.a_off[ASTRA_A_##n] & ASTRA_PLACE_SMEM) ? hot : ws) + (P.a_off[ASTRA_A_##n] & ~ASTRA_PLACE_SMEM));
+#define X(n, t, i) c.n = (t*)(((P.a_off[ASTRA_A_##n] & ASTRA_PLACE_SMEM) ? hot : ws) + (P.a_off[ASTRA_A_##n] & ~(ASTRA_PLACE_SMEM | ASTRA_PLACE_LOCAL)));
     ASTRA_WS_ARRAYS(X)
 #undef X
     // node range of this CTA (the whole graph when the point runs on one CTA)
     c.v_lo = c.part[rank]; c.v_hi = c.part[rank + 1];
     c.g_lo = min(c.v_lo, c.G); c.g_hi = min(c.v_hi, c.G);
+    // arrays that hold only this CTA's GPUs are indexed by absolute GPU id through a pointer moved back by g_lo strides
+#define X(n, per_gpu, eb) if (P.a_off[ASTRA_A_##n] & ASTRA_PLACE_LOCAL) c.n -= (size_t)c.g_lo * (per_gpu);
+    ASTRA_GPU_ARRAYS(X)
+#undef X
+    if (P.a_off[ASTRA_A_hist] & ASTRA_PLACE_LOCAL) c.hist -= (size_t)c.row_ptr[c.g_lo] * P.Wcyc;
     c.e_lo = c.row_ptr[c.v_lo]; c.e_hi = c.row_ptr[c.v_hi];
     c.i_lo = c.in_ptr[c.v_lo]; c.i_hi = c.in_ptr[c.v_hi];
     c.r_step_ts = (u64*)(rs + P.r_step_ts);
@@ -1847,15 +1851,21 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     const u32 kb = k & c.NWmask;
 
     // ---- stage 1: ack discovery (A3) and arrivals (A1) as chunk tasks over the set's warps ----
+    // Task t of the stage (all its chunks numbered through) is taken by warp t mod ws: tmod is the running
+    // task count mod ws, the same in every warp, and `(sw + ws - tmod) % ws` the first chunk of the next group
+    // that falls to this warp.
     bool any_fwd = false;
+    u32 tmod = 0;
     if (is_gpu) {
-        if (sw == 0) stage1_setup_gpu(c, ctl, hp, v, k, lane);
+        if (sw == ws - 1) stage1_setup_gpu(c, ctl, hp, v, k, lane);
         const u32 n_ack = ld_vol(&c.bin_cnt[v * c.NW + kb]);
         if (n_ack && n_ack <= c.alcap) {                         // alcap == 0: no list, the bitmap is scanned
             for (u32 ch = sw; ch * 128 < n_ack; ch += ws) ack_list_chunk(c, ctl, v, ch, n_ack, k, t1, lane);
+            tmod = ((n_ack + 127) / 128) % ws;
         } else if (n_ack) {
             const u32 nch = (c.bmwords + 31) / 32;
             for (u32 ch = sw; ch < nch; ch += ws) ack_chunk(c, ctl, v, ch, k, t1, scr, lane);
+            tmod = nch % ws;
         }
     }
     // the node's in-links, one per lane: id, lines due this window (counted by the link's service when it
@@ -1877,9 +1887,8 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             const u32 src = __ffs(nm) - 1; nm &= nm - 1;
             const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
             const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
-            const u32 rot = (ib - i_lo + src) % ws;
-            if (fl == 0u) { if (sw == rot) arrivals_link<1>(c, ctl, hp, ib + src, n, k, t0, wlen, cb, lane); continue; }
-            const u32 first = (sw + ws - rot) % ws;
+            const u32 first = (sw + ws - tmod) % ws;
+            if (fl == 0u) { if (first == 0u) arrivals_link<1>(c, ctl, hp, ib + src, n, k, t0, wlen, cb, lane); tmod = (tmod + 1) % ws; continue; }
             if (fl == ASTRA_LF_DELIVER_ONLY) {
                 for (u32 ch = first; ch * 32 < n; ch += ws) deliver_chunk(c, ctl, hp, e, lo, n, ch, k, t0, wlen, lane);
             } else if (fl == ASTRA_LF_FORWARD_ONLY) {
@@ -1889,6 +1898,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             } else {
                 for (u32 ch = first; ch * 64 < n; ch += ws) cells_chunk<1>(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
             }
+            tmod = (tmod + (fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32)) % ws;
         }
     }
     set_sync(ws, set);
@@ -1968,6 +1978,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
         set_sync(ws, set);
         if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
+        u32 tmod3 = 0;
         for (u32 ib = i_lo; ib < i_hi; ib += 32) {
             const u32 i = ib + lane;
             u32 e_b = e_l, n_b = n_l, lo_b = lo_l, fl_b = fl_l;
@@ -1985,11 +1996,10 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
                 const u32 src = __ffs(nm) - 1; nm &= nm - 1;
                 const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
                 const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
-                const u32 rot = (ib - i_lo + src) % ws;
-                if (fl == 0u) { if (sw == rot) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); continue; }
-                for (u32 ch = (sw + ws - rot) % ws; ch * 64 < n; ch += ws) {
-                    cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
-                }
+                const u32 first = (sw + ws - tmod3) % ws;
+                if (fl == 0u) { if (first == 0u) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); tmod3 = (tmod3 + 1) % ws; continue; }
+                for (u32 ch = first; ch * 64 < n; ch += ws) cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
+                tmod3 = (tmod3 + (n + 63) / 64) % ws;
             }
         }
         set_sync(ws, set);
@@ -2088,7 +2098,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             if (kind > 1) continue;
             const u64 off = P.a_off[a];
             const bool in_smem = (off & ASTRA_PLACE_SMEM) != 0;
-            uint8_t* base = (in_smem ? hot : ws) + (off & ~ASTRA_PLACE_SMEM);
+            uint8_t* base = (in_smem ? hot : ws) + (off & ~(ASTRA_PLACE_SMEM | ASTRA_PLACE_LOCAL));
             const u32 pat = kind ? ~0u : 0u;
             const u64 n16 = P.a_bytes[a] / 16;              // arrays are padded to 16 bytes
             uint4* p = reinterpret_cast<uint4*>(base);

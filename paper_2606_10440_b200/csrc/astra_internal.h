@@ -54,7 +54,7 @@ typedef uint64_t u64;
 #define ASTRA_WS_ARRAYS(X) \
     X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
     X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(due_cnt, u32, 0) X(tl_lo, u32, 3) X(tl_n, u32, 3) X(tl_base, u32, 3) X(tbase, u32, 3) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
-    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(pfx, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
@@ -76,6 +76,13 @@ enum AstraArrId {
 
 #define ASTRA_DIAG_WORDS 144                // u64 per CTA: 16 common + 16 warp sets x 8 stage clocks (ASTRA_DIAG builds)
 #define ASTRA_PLACE_SMEM (1ull << 63)     // a_off flag: offset is into the CTA's shared-memory hot region
+#define ASTRA_PLACE_LOCAL (1ull << 62)    // a_off flag (CTA groups): the array holds only the CTA's own GPUs; indexed by absolute GPU id
+                                          // through a pointer moved back by g_lo strides (hist: by the first out-link of g_lo)
+// Arrays indexed by GPU (X(name, elements per GPU as an expression of P, bytes per element)): in a CTA group each CTA keeps only its GPUs' part.
+#define ASTRA_GPU_ARRAYS(X) \
+    X(want, P.nwords, 4) X(freeb, P.nwords, 4) X(amask, P.nwords, 4) X(undo_want, P.nwords, 4) X(undo_freeb, P.nwords, 4) \
+    X(cnt, P.Wcyc, 4) X(sel, P.H, 4) X(wf_busy, P.CW, 8) X(undo_busy, P.CW, 8) X(wf_rem, P.CW, 4) X(wf_cur, P.CW, 4) \
+    X(undo_rem, P.CW, 4) X(undo_cur, P.CW, 4) X(hlist, P.CW, 4)
 
 // Per design point descriptor.  c_off are byte offsets into the batch's constant blob, a_off byte
 // offsets into the hot region (flag set) or the workspace of the CTA group running the point,

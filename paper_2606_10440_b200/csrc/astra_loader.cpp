@@ -437,7 +437,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
     ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
     ab[ASTRA_A_gmode] = ab[ASTRA_A_nheavy] = 4ull * G;
-    ab[ASTRA_A_cnt] = ab[ASTRA_A_pfx] = 4ull * G * W;
+    ab[ASTRA_A_cnt] = 4ull * G * W;
     ab[ASTRA_A_undo_want] = ab[ASTRA_A_undo_freeb] = 4ull * G * P.nwords;
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
     ab[ASTRA_A_evb] = 8ull * G * g.H * W;
@@ -464,8 +464,26 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_inj_list] = 8ull * inj_off[G];
     ab[ASTRA_A_ack_rec] = ab[ASTRA_A_ack_tmp] = ab[ASTRA_A_ack_sorted] = 8ull * G * slots;
     ab[ASTRA_A_ring] = 8ull * ring_total;
+    // CTA groups: the arrays indexed by GPU (and hist, indexed by the GPUs' out-links) are kept per CTA for its own
+    // GPUs only when that part fits in shared memory -- the whole point's arrays would crowd everything else out
+    u32 maxG = 0, maxOut = 0;
+    for (u32 r = 0; r < group; r++) {
+        const u32 a0 = std::min(part[r], G), a1 = std::min(part[r + 1], G);
+        maxG = std::max(maxG, a1 - a0); maxOut = std::max(maxOut, t.row_ptr[a1] - t.row_ptr[a0]);
+    }
+    u64 local_bytes[ASTRA_A_COUNT] = {0};
+    if (group > 1) {
+#define X(n, per_gpu, eb) local_bytes[ASTRA_A_##n] = (u64)(eb) * (per_gpu) * std::max<u32>(1, maxG);
+        ASTRA_GPU_ARRAYS(X)
+#undef X
+        local_bytes[ASTRA_A_hist] = 4ull * ((u64)maxOut * W + 1);
+    }
     u64 hot = 0, ws = 0;
     for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
+        if (local_bytes[a]) {
+            const u64 lb = (std::max<u64>(local_bytes[a], 16) + 15) & ~15ull;
+            if (hot + lb <= opt.hot_budget) { ab[a] = lb; P.a_off[a] = hot | ASTRA_PLACE_SMEM | ASTRA_PLACE_LOCAL; hot += lb; continue; }
+        }
         ab[a] = (std::max<u64>(ab[a], 16) + 15) & ~15ull;
         // streamed arrays stay in global memory; so does, for a CTA group, what another CTA of the group
         // reads or writes: link cursors seen from both ends, ack records / bitmap / bin counts (written
