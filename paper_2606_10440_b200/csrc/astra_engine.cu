@@ -510,12 +510,43 @@ __device__ void deliver_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
 // A line's cell slot is (in-link's slot base + its rank among the lines this link delivers in the
 // same cycle); lines of one cycle are consecutive in the stream, so the rank is a look at the
 // neighbours -- inside the chunk, and at most ceil(B)-1 entries back across its start.
-// PASS 1 delivers and marks cells; PASS 3 (after the cell prefix sums) writes the FIFO entries.
-template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 rel, u32 lane);
+// Pass 1 (here) delivers, marks cells and records (out-link, slot) per line; the placement pass
+// (cells_place_chunk, after the cell prefix sums) writes the FIFO entries.
 
-// A task is 64 entries: both halves' ring loads (and the look-back) are in flight before the first use.
-template <int PASS>
+// the lines of one half-chunk that end at the link's head GPU v: ack record, ack bin, delivery count (R6, R7 A1)
+__device__ __forceinline__ void cells_deliver(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u64 flit, u32 d, u32 od,
+                                              bool deliver, u32 vmask) {
+    const u32 dmask = __ballot_sync(vmask, deliver);
+    if (!deliver) return;
+    const u32 step = (u32)flit & 0xfffffu;
+    const u32 owner = od >> 16;
+    const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
+    const u32 ta = t0 + d + c.step_alpha[step];                       // R6
+    const u32 bit = wf * c.K + slot;
+    c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
+    const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
+    atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
+    const u32 mb = __match_any_sync(dmask, bin);
+    u32 lpos = 0;                                        // discovery list of the bin: position from the count
+    if ((mb & lanemask_lt()) == 0) { if (c.alcap) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); else atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); }
+    const u32 m = __match_any_sync(dmask, step);
+    const u32 dmax = __reduce_max_sync(m, d);
+    if ((m & lanemask_lt()) == 0) {
+        atomicMax(&c.t_deliv[step], t0 + dmax);
+        const u32 cntm = __popc(m);
+        const u32 old = atomicAdd(&c.deliv_cnt[step], cntm);
+        if (old + cntm == c.lines[step]) {
+            const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
+            c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
+        }
+    }
+    const u32 hint = __reduce_min_sync(dmask, ta);
+    if ((dmask & lanemask_lt()) == 0) atomicMin(hp, hint);
+    if (c.alcap) { lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt()); if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit; }
+}
+
+// A task is 64 entries, handled as two halves in lock step: the ring loads (and the look-back), then the step
+// lookups, then the route lookups of both halves are in flight together.
 __device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 lo, u32 n, u32 chunk, u32 k, u32 t0, u32 wlen, u32 cb, u32 lane) {
     const u32 i0 = lo + chunk * 64;
     const u64* ring = c.ring + c.ring_off[e];
@@ -526,68 +557,30 @@ __device__ void cells_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e,
     const u64 fa = in0 ? __ldcg(&ring[(i0 + lane) & rmask]) : 0ull;
     const u64 fb = in1 ? __ldcg(&ring[(i0 + 32 + lane) & rmask]) : 0ull;
     const u64 fz = inb ? __ldcg(&ring[(i0 - 1 - lane) & rmask]) : 0ull;
+    const u32 v = c.head[e], coff = c.classoff[e], G = c.G;
     const u32 da = in0 ? (((u32)(fa >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xffffffffu;
     const u32 db = in1 ? (((u32)(fb >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xfffffffeu;
     const u32 dz = inb ? (((u32)(fz >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26) : 0xfffffffdu;
     const u32 da0 = __shfl_sync(FULL, da, 0), db0 = __shfl_sync(FULL, db, 0);
     const u32 back_a = __popc(__ballot_sync(FULL, dz == da0));          // same-cycle lines before the task
     const u32 back_b = __popc(__ballot_sync(FULL, da == db0));          // ... before its second half
-    cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fa, da, in0 && da < wlen, da0, back_a, chunk * 64 + lane, lane);   // d >= wlen: watchdog cut inside the window
-    if (__any_sync(FULL, in1)) cells_half<PASS>(c, ctl, hp, e, k, t0, cb, fb, db, in1 && db < wlen, db0, back_b, chunk * 64 + 32 + lane, lane);
-}
-
-template <int PASS>
-__device__ void cells_half(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 cb, u64 flit, u32 d, bool valid, u32 d0, u32 back, u32 rel, u32 lane) {
-    const u32 vmask = __ballot_sync(FULL, valid);
-    if (!valid) return;
-    const u32 grp = __match_any_sync(vmask, d);
-    const u32 r = __popc(grp & lanemask_lt()) + (d == d0 ? back : 0u);
-    const u32 v = c.head[e];
-    const u32 step = (u32)flit & 0xfffffu;
-    const u32 od = c.step_od[step];
-    const u32 dstg = od & 0xffffu;
-    const bool deliver = dstg == v;
-    if (PASS == 1 && deliver) c.lscr[c.lscr_off[e] + rel] = ASTRA_NONE32;      // nothing to place for a line that ends here
-    if (!deliver) {
-        const u32 o = c.next_link[(size_t)v * c.G + dstg];
-        if (PASS == 1) {
-            const u32 slot = c.classoff[e] + r;
-            cell_set(c, o, v, cb, d, slot); c.tl_base[e] = 1u;
-            c.lscr[c.lscr_off[e] + rel] = (o << 12) | slot;           // the placement pass reads this instead of routing again
-        } else {
-            const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, c.classoff[e] + r);
-            c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
-        }
-    }
-    if (PASS == 1) {
-        const u32 dmask = __ballot_sync(vmask, deliver);
-        if (deliver) {
-            const u32 owner = od >> 16;
-            const u32 wf = ((u32)flit >> 20) & 0xfffu, slot = (u32)(flit >> 32) & 63u;
-            const u32 ta = t0 + d + c.step_alpha[step];                       // R6
-            const u32 bit = wf * c.K + slot;
-            c.ack_rec[(size_t)owner * c.slots + bit] = ((u64)step << 32) | ta;
-            const u32 bin = owner * c.NW + ((k + c.step_aq[step] + (d + c.step_ar[step] >= c.W ? 1u : 0u)) & c.NWmask);
-            atomicOr(&c.bitmap[(size_t)bin * c.bmwords + (bit >> 5)], 1u << (bit & 31));
-            const u32 mb = __match_any_sync(dmask, bin);
-            u32 lpos = 0;                                        // discovery list of the bin: position from the count
-            if ((mb & lanemask_lt()) == 0) { if (c.alcap) lpos = atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); else atomicAdd(&c.bin_cnt[bin], (u32)__popc(mb)); }
-            const u32 m = __match_any_sync(dmask, step);
-            const u32 dmax = __reduce_max_sync(m, d);
-            if ((m & lanemask_lt()) == 0) {
-                atomicMax(&c.t_deliv[step], t0 + dmax);
-                const u32 cntm = __popc(m);
-                const u32 old = atomicAdd(&c.deliv_cnt[step], cntm);
-                if (old + cntm == c.lines[step]) {
-                    const u32 pos = atomicAdd(&c.ev_cnt[v], 1u);
-                    c.ev_list[c.ev_off[v] + pos] = step | ((u32)ASTRA_DEP_DELIVERED << 30);
-                }
-            }
-            const u32 hint = __reduce_min_sync(dmask, ta);
-            if ((dmask & lanemask_lt()) == 0) atomicMin(hp, hint);
-            if (c.alcap) { lpos = __shfl_sync(mb, lpos, __ffs(mb) - 1) + __popc(mb & lanemask_lt()); if (lpos < c.alcap) c.ack_list[(size_t)bin * c.alcap + lpos] = bit; }
-        }
-    }
+    const bool va = in0 && da < wlen, vb = in1 && db < wlen;            // d >= wlen: watchdog cut inside the window
+    const u32 vma = __ballot_sync(FULL, va), vmb = __ballot_sync(FULL, vb);
+    const u32 oda = va ? c.step_od[(u32)fa & 0xfffffu] : 0u;
+    const u32 odb = vb ? c.step_od[(u32)fb & 0xfffffu] : 0u;
+    u32 ra = 0, rb = 0;
+    if (va) ra = __popc(__match_any_sync(vma, da) & lanemask_lt()) + (da == da0 ? back_a : 0u);
+    if (vb) rb = __popc(__match_any_sync(vmb, db) & lanemask_lt()) + (db == db0 ? back_b : 0u);
+    const bool dla = va && (oda & 0xffffu) == v, dlb = vb && (odb & 0xffffu) == v;
+    const bool tra = va && !dla, trb = vb && !dlb;
+    const u32 oa = tra ? c.next_link[(size_t)v * G + (oda & 0xffffu)] : 0u;
+    const u32 ob = trb ? c.next_link[(size_t)v * G + (odb & 0xffffu)] : 0u;
+    u32* scr = c.lscr + c.lscr_off[e] + chunk * 64 + lane;
+    if (va) { if (tra) { cell_set(c, oa, v, cb, da, coff + ra); scr[0] = (oa << 12) | (coff + ra); } else scr[0] = ASTRA_NONE32; }
+    if (vb) { if (trb) { cell_set(c, ob, v, cb, db, coff + rb); scr[32] = (ob << 12) | (coff + rb); } else scr[32] = ASTRA_NONE32; }
+    if (__any_sync(FULL, tra || trb) && lane == 0) c.tl_base[e] = 1u;   // the placement pass has work on this link
+    if (__any_sync(FULL, dla)) { if (va) cells_deliver(c, ctl, hp, v, k, t0, fa, da, oda, dla, vma); }
+    if (__any_sync(FULL, dlb)) { if (vb) cells_deliver(c, ctl, hp, v, k, t0, fb, db, odb, dlb, vmb); }
 }
 
 // Placement pass of such a link (after the cell prefix sums): the lines that go on are written to their
@@ -596,21 +589,36 @@ __device__ void cells_place_chunk(const Ctx& __restrict__ c, u32 e, u32 lo, u32 
     const u64* ring = c.ring + c.ring_off[e];
     const u32 rmask = c.ring_mask[e];
     const u32* scr = c.lscr + c.lscr_off[e];
-    const u32 v = c.head[e];
-    const u32 r0 = chunk * 64 + lane, r1 = r0 + 32;
-    const u64 fa = r0 < n ? __ldcg(&ring[(lo + r0) & rmask]) : 0ull;
-    const u64 fb = r1 < n ? __ldcg(&ring[(lo + r1) & rmask]) : 0ull;
-    const u32 sa = r0 < n ? scr[r0] : ASTRA_NONE32;
-    const u32 sb = r1 < n ? scr[r1] : ASTRA_NONE32;
+    const u32 v = c.head[e], mw = c.nd_mw[v], NC = c.NC;
+    u64 fl[2]; u32 sc[2], d[2], o[2], pb[2], tl[2], moff[2]; bool ok[2];
+    // both halves in lock step: flit + record, then cursors and prefix, then the cell words
 #pragma unroll
     for (int h = 0; h < 2; h++) {
-        const u64 flit = h ? fb : fa;
-        const u32 sc = h ? sb : sa;
-        const u32 d = ((u32)(flit >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
-        if ((h ? r1 : r0) >= n || d >= wlen || sc == ASTRA_NONE32) continue;     // d >= wlen: watchdog cut inside the window
-        const u32 o = sc >> 12;
-        const u32 pos = c.ltail[o] + cell_pos(c, o, v, cb, d, sc & 0xfffu);
-        c.ring[c.ring_off[o] + (pos & c.ring_mask[o])] = (flit & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d << ASTRA_FLIT_TIME_SHIFT);
+        const u32 r = chunk * 64 + h * 32 + lane;
+        fl[h] = r < n ? __ldcg(&ring[(lo + r) & rmask]) : 0ull;
+        sc[h] = r < n ? scr[r] : ASTRA_NONE32;
+    }
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        d[h] = ((u32)(fl[h] >> ASTRA_FLIT_TIME_SHIFT) - t0) & ASTRA_TMASK26;
+        ok[h] = chunk * 64 + h * 32 + lane < n && d[h] < wlen && sc[h] != ASTRA_NONE32;      // d >= wlen: watchdog cut inside the window
+        o[h] = ok[h] ? sc[h] >> 12 : 0u;
+        pb[h] = ok[h] ? c.pre[c.pre_off[o[h]] + d[h]] : 0u;
+        tl[h] = ok[h] ? c.ltail[o[h]] : 0u;
+        moff[h] = ok[h] ? c.mask_off[o[h]] : 0u;
+    }
+#pragma unroll
+    for (int h = 0; h < 2; h++) {
+        if (!ok[h]) continue;
+        const u32 slot = sc[h] & 0xfffu;
+        u32 ci = cb + d[h]; if (ci >= NC) ci -= NC;
+        const u32* words = c.masks + moff[h] + ci * mw;
+        u32 r = pb[h];
+        const u32 swd = slot >> 5;
+        for (u32 w = 0; w < swd; w++) r += __popc(words[w]);
+        r += __popc(words[swd] & ((1u << (slot & 31)) - 1u));
+        const u32 pos = tl[h] + r;
+        c.ring[c.ring_off[o[h]] + (pos & c.ring_mask[o[h]])] = (fl[h] & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)d[h] << ASTRA_FLIT_TIME_SHIFT);
     }
 }
 
@@ -1896,7 +1904,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
                 for (u32 ch = first; ch * 32 < n; ch += ws) forward_chunk(c, e, lo, n, base, ch, t0, wlen, lane);
                 any_fwd = true;
             } else {
-                for (u32 ch = first; ch * 64 < n; ch += ws) cells_chunk<1>(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
+                for (u32 ch = first; ch * 64 < n; ch += ws) cells_chunk(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
             }
             tmod = (tmod + (fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32)) % ws;
         }
