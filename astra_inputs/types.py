@@ -136,14 +136,19 @@ class CollectiveBuilder:
         )
 
 
+GPU_ISSUE_PER_CU = 1    # a CU dispatches at most one line per cycle (lowest ready wavefront)
+GPU_CAP_PER_CU = 2      # max_outstanding bounds the CU's wavefronts together
+
+
 @dataclass
 class GpuCfg:
     """astra_set_gpu parameters (PAPER.md:L189 CUs, L165 wavefronts, L209/L297 outstanding cap,
     L221 memory channels -> HBM rate)."""
     cus: int
     wavefronts_per_cu: int
-    max_outstanding: int          # per wavefront (SURVEY Q2)
+    max_outstanding: int          # per wavefront (SURVEY Q2) -- per CU when mode & GPU_CAP_PER_CU
     hbm_lines_per_cycle: int
+    mode: int = 0                 # GPU_ISSUE_PER_CU | GPU_CAP_PER_CU: the paper's per-CU readings (PAPER.md:L209, L297)
 
 
 @dataclass

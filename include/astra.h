@@ -148,6 +148,20 @@ int32_t astra_load_collective(astra_ctx* ctx, uint32_t n_gpus, uint32_t n_steps,
 int32_t astra_set_gpu(astra_ctx* ctx, uint32_t cus, uint32_t wavefronts_per_cu,
                       uint32_t max_outstanding, uint32_t hbm_lines_per_cycle, uint32_t* out_gpu_id);
 
+/* The same GPU model with the paper's per-CU readings of two rules switched on by `mode` bits (DESIGN.md
+ * section 3, R12' and R2'; astra_set_gpu is mode 0, the per-wavefront reading the BASELINE configs use):
+ *   ASTRA_GPU_ISSUE_PER_CU  a CU dispatches at most one line per cycle, from its lowest-id ready wavefront
+ *                           ("it can dispatch one cache-line-sized Wavefront Request in each
+ *                           cycle", L191 "chooses a wavefront that is ready")
+ *   ASTRA_GPU_CAP_PER_CU    max_outstanding bounds the un-acked lines of all wavefronts of a CU together
+ *                           ("maximum number of outstanding requests per CU")
+ * Such GPUs are stepped on the engine's cycle-serial issue path.  ELIMIT when wavefronts_per_cu > 32. */
+#define ASTRA_GPU_ISSUE_PER_CU 1u
+#define ASTRA_GPU_CAP_PER_CU   2u
+int32_t astra_set_gpu_ex(astra_ctx* ctx, uint32_t cus, uint32_t wavefronts_per_cu,
+                         uint32_t max_outstanding, uint32_t hbm_lines_per_cycle, uint32_t mode,
+                         uint32_t* out_gpu_id);
+
 /* Simulate n_points independent design points, each from t = 0 with empty queues (R1), until
  * every step is acked (R14) or cycle max_cycles (clamped to ASTRA_MAX_CYCLES) is reached.  Synchronous: returns when the
  * results are ready on the device.  EINVAL when a point's collective and topology disagree on

@@ -29,6 +29,15 @@
  *     or they issued).  Every visited wavefront runs the same full check.  The default (flag
  *     clear) is the plain scan over all wavefronts; tests assert both give identical output.
  *
+ * Round 2 adds the paper's own per-CU readings of two rules as OPTIONS (both off by default, so nothing above
+ * changes, R12' and R2'):
+ *   ORACLE_FLAG_ISSUE_PER_CU  a CU dispatches at most one line per cycle ("it can dispatch one
+ *                             cache-line-sized Wavefront Request in each cycle", L203), choosing its lowest-id ready
+ *                             wavefront (L191 "chooses a wavefront that is ready");
+ *   ORACLE_FLAG_CAP_PER_CU    max_outstanding bounds the un-acked lines of all wavefronts of a CU together
+ *                             ("maximum number of outstanding requests per CU").
+ * Pinned by hand traces H1-H3 (tests/golden/pins_survey_8c.json).
+ *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): hand traces P1-P3, closed forms CF1/CF2,
  * config 1 in full (P4: completion 38,623), alpha-beta convergence P5, config 2 ring/direct
  * formulas P6/P7, invariants I1-I9, and agreement with an independently structured tiny
@@ -46,6 +55,8 @@
 #define ORACLE_EINTERNAL    -100
 
 #define ORACLE_FLAG_PRUNED_SCAN 1u
+#define ORACLE_FLAG_ISSUE_PER_CU 2u
+#define ORACLE_FLAG_CAP_PER_CU   4u
 
 #define DEP_DELIVERED 0
 #define DEP_ACKED     1
@@ -255,6 +266,8 @@ int oracle_run(uint32_t n_gpus, uint32_t n_switches, const uint32_t *node_latenc
     uint32_t *wf_cur = (uint32_t *)calloc((size_t)G * WF, sizeof(uint32_t));   /* index into its CU list */
     uint32_t *wf_rem = (uint32_t *)calloc((size_t)G * WF, sizeof(uint32_t));   /* quota left; UINT32_MAX = not loaded */
     uint32_t *wf_out = (uint32_t *)calloc((size_t)G * WF, sizeof(uint32_t));
+    uint32_t *cu_out = (uint32_t *)calloc((size_t)G * cus, sizeof(uint32_t));      /* un-acked lines per CU (R2') */
+    uint64_t *cu_issued = (uint64_t *)calloc((size_t)G * cus, sizeof(uint64_t));   /* t + 1 of the CU's last issue (R12') */
     uint8_t *wf_maybe = (uint8_t *)malloc((size_t)G * WF);                     /* pruned scan only */
     uint32_t *gpu_unfinished = (uint32_t *)calloc(G, sizeof(uint32_t));        /* wavefronts with list not exhausted */
     uint32_t *gpu_maybe_cnt = (uint32_t *)calloc(G, sizeof(uint32_t));         /* pruned scan only: #wf_maybe set */
@@ -262,7 +275,7 @@ int oracle_run(uint32_t n_gpus, uint32_t n_switches, const uint32_t *node_latenc
     tokv_t *acks = NULL;  uint64_t Tcal = 0;
 
     if (!tail || !leff || !dist || !next_link || !in_ptr || !in_link || !fifo || !pipe || !credit || !cap ||
-        !issued_cnt || !deliv_cnt || !ack_cnt || !cul_ptr || !wf_cur || !wf_rem || !wf_out || !wf_maybe ||
+        !issued_cnt || !deliv_cnt || !ack_cnt || !cul_ptr || !wf_cur || !wf_rem || !wf_out || !cu_out || !cu_issued || !wf_maybe ||
         !gpu_unfinished || !gpu_maybe_cnt || !pending) { ret = ORACLE_ENOMEM; goto done; }
 
     for (uint32_t v = 0; v < V; v++)
@@ -374,7 +387,11 @@ int oracle_run(uint32_t n_gpus, uint32_t n_switches, const uint32_t *node_latenc
                 size_t w = (size_t)g * WF + tk.wf;
                 if (wf_out[w] == 0) { ret = ORACLE_EINTERNAL; goto done; }
                 wf_out[w]--;
+                cu_out[(size_t)g * cus + tk.wf / wpc]--;
                 if (!wf_maybe[w]) { wf_maybe[w] = 1; gpu_maybe_cnt[g]++; }
+                if (flags & ORACLE_FLAG_CAP_PER_CU)            /* the slot returns to the CU's pool: any of its wavefronts may use it */
+                    for (uint32_t x = (tk.wf / wpc) * wpc; x < (tk.wf / wpc + 1) * wpc; x++)
+                        if (!wf_maybe[(size_t)g * WF + x]) { wf_maybe[(size_t)g * WF + x] = 1; gpu_maybe_cnt[g]++; }
                 in_flight--;
                 ack_cnt[s]++;
                 TRACE(TR_ACK, s, (uint64_t)g * 65536 + tk.wf, 0);
@@ -433,9 +450,10 @@ int oracle_run(uint32_t n_gpus, uint32_t n_switches, const uint32_t *node_latenc
             for (uint32_t wf = 0; wf < WF && budget; wf++) {
                 size_t w = (size_t)g * WF + wf;
                 if ((flags & ORACLE_FLAG_PRUNED_SCAN) && !wf_maybe[w]) continue;
-                st_visits++;
                 uint32_t cu = wf / wpc, lane = wf % wpc;
                 size_t ck = (size_t)g * cus + cu;
+                if ((flags & ORACLE_FLAG_ISSUE_PER_CU) && cu_issued[ck] == t + 1) continue;   /* R12': the CU has dispatched this cycle */
+                st_visits++;
                 uint32_t len = cul_ptr[ck + 1] - cul_ptr[ck];
                 int can = 0; uint32_t s = 0;
                 while (wf_cur[w] < len) {                      /* in-order list, lazy advance (R11) */
@@ -453,8 +471,8 @@ int oracle_run(uint32_t n_gpus, uint32_t n_switches, const uint32_t *node_latenc
                     }
                     can = 1; break;
                 }
-                if (can && wf_out[w] < K) {
-                    wf_out[w]++; wf_rem[w]--; in_flight++;
+                if (can && ((flags & ORACLE_FLAG_CAP_PER_CU) ? cu_out[ck] < K : wf_out[w] < K)) {      /* R2 / R2' */
+                    wf_out[w]++; cu_out[ck]++; cu_issued[ck] = t + 1; wf_rem[w]--; in_flight++;
                     if (wf_out[w] > st_max_out) st_max_out = wf_out[w];
                     issued_cnt[s]++;
                     TRACE(TR_ISSUE, s, (uint64_t)g * 65536 + wf, 0);
@@ -500,7 +518,7 @@ done:
     free(tail); free(leff); free(dist); free(next_link); free(in_ptr); free(in_link);
     free(fifo); free(pipe); free(credit); free(cap);
     free(issued_cnt); free(deliv_cnt); free(ack_cnt);
-    free(cul_ptr); free(cul); free(wf_cur); free(wf_rem); free(wf_out); free(wf_maybe);
+    free(cul_ptr); free(cul); free(wf_cur); free(wf_rem); free(wf_out); free(cu_out); free(cu_issued); free(wf_maybe);
     free(gpu_unfinished); free(gpu_maybe_cnt); free(pending); free(acks);
     return ret;
 }

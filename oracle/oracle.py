@@ -18,6 +18,8 @@ _SRC = os.path.join(_HERE, "astra_oracle.c")
 _LIB = os.path.join(_HERE, "libastra_oracle.so")
 
 FLAG_PRUNED_SCAN = 1
+FLAG_ISSUE_PER_CU = 2      # R12': one line per CU per cycle
+FLAG_CAP_PER_CU = 4        # R2': max_outstanding per CU
 TS_NONE = np.uint64(0xFFFFFFFFFFFFFFFF)
 
 TR_ISSUE, TR_ACCEPT, TR_DELIVER, TR_ACK, TR_RELEASE = range(5)
@@ -75,6 +77,7 @@ def route(topo):
 def run_point(topo, coll, gpu, max_cycles: int = 1 << 40, flags: int = 0,
               trace_cap: int = 0, check: bool = True) -> OracleResult:
     lib = _load()
+    flags |= 2 * (getattr(gpu, "mode", 0) & 3)          # GpuCfg.mode bit 0: issue per CU, bit 1: cap per CU
     S, E = coll.n_steps, topo.n_links
     step_ts = np.zeros(max(1, 4 * S), dtype=np.uint64)
     link_lines = np.zeros(max(1, E), dtype=np.uint64)

@@ -16,7 +16,7 @@ _LIBPATH = os.path.join(_HERE, "libastra_b200_diag.so" if os.environ.get("ASTRA_
 
 EXPORTED_SYMBOLS = [
     "astra_create", "astra_destroy", "astra_last_error", "astra_set_stream",
-    "astra_load_infragraph", "astra_load_collective", "astra_set_gpu",
+    "astra_load_infragraph", "astra_load_collective", "astra_set_gpu", "astra_set_gpu_ex",
     "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
     "astra_last_run_info", "astra_last_transfer_bytes", "astra_read_diag", "astra_point_group",
 ]
@@ -93,6 +93,7 @@ def load_library(path: Optional[str] = None):
     lib.astra_load_infragraph.argtypes = [vp, u32, u32, vp, vp, vp, vp, vp, ctypes.POINTER(u32)]
     lib.astra_load_collective.argtypes = [vp, u32, u32, vp, vp, vp, vp, vp, vp, vp, vp, ctypes.POINTER(u32)]
     lib.astra_set_gpu.argtypes = [vp, u32, u32, u32, u32, ctypes.POINTER(u32)]
+    lib.astra_set_gpu_ex.argtypes = [vp, u32, u32, u32, u32, u32, ctypes.POINTER(u32)]
     lib.astra_run_batch.argtypes = [vp, u32, vp, u64]
     lib.astra_run_batch_async.argtypes = [vp, u32, vp, u64]
     lib.astra_sync.argtypes = [vp]
@@ -175,6 +176,12 @@ class Engine:
                                             hbm_lines_per_cycle, ctypes.byref(out)))
         return out.value
 
+    def set_gpu_ex(self, cus, wavefronts_per_cu, max_outstanding, hbm_lines_per_cycle, mode) -> int:
+        out = ctypes.c_uint32()
+        self._check(self._lib.astra_set_gpu_ex(self._ctx, cus, wavefronts_per_cu, max_outstanding,
+                                               hbm_lines_per_cycle, mode, ctypes.byref(out)))
+        return out.value
+
     def _marshal_points(self, points: Sequence[Tuple[int, int, int]]):
         arr = (_Point * max(1, len(points)))()
         for i, (t, c, g) in enumerate(points):
@@ -231,7 +238,9 @@ class Engine:
                 for t in w.topologies]
         cids = [self.load_collective(c.n_gpus, c.owner, c.dst, c.lines, c.cu_lo, c.cu_n, c.dep_ptr, c.dep_step,
                                      c.dep_kind) for c in w.collectives]
-        gids = [self.set_gpu(g.cus, g.wavefronts_per_cu, g.max_outstanding, g.hbm_lines_per_cycle) for g in w.gpus]
+        gids = [self.set_gpu_ex(g.cus, g.wavefronts_per_cu, g.max_outstanding, g.hbm_lines_per_cycle, getattr(g, "mode", 0))
+                if getattr(g, "mode", 0) else self.set_gpu(g.cus, g.wavefronts_per_cu, g.max_outstanding, g.hbm_lines_per_cycle)
+                for g in w.gpus]
         return [(tids[t], cids[c], gids[g]) for (t, c, g) in w.points]
 
 

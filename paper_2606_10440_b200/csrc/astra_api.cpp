@@ -142,14 +142,22 @@ extern "C" int32_t astra_load_collective(astra_ctx* c, uint32_t n_gpus, uint32_t
       catch (...) { return fail(c, ASTRA_EINVAL, "unexpected error"); }
 }
 
+extern "C" int32_t astra_set_gpu_ex(astra_ctx* c, uint32_t cus, uint32_t wpc, uint32_t k, uint32_t h, uint32_t mode, uint32_t* out_id);
+
 extern "C" int32_t astra_set_gpu(astra_ctx* c, uint32_t cus, uint32_t wpc, uint32_t k, uint32_t h, uint32_t* out_id) {
+    return astra_set_gpu_ex(c, cus, wpc, k, h, 0u, out_id);
+}
+
+extern "C" int32_t astra_set_gpu_ex(astra_ctx* c, uint32_t cus, uint32_t wpc, uint32_t k, uint32_t h, uint32_t mode, uint32_t* out_id) {
     if (!c) return ASTRA_EINVAL;
+    if (mode & ~(uint32_t)(ASTRA_GPU_ISSUE_PER_CU | ASTRA_GPU_CAP_PER_CU)) return fail(c, ASTRA_EINVAL, "unknown GPU mode bits");
+    if (mode && wpc > 32) return fail(c, ASTRA_ELIMIT, "the per-CU modes need wavefronts_per_cu <= 32");
     if (!out_id) return fail(c, ASTRA_EINVAL, "null argument");
     if (!cus || !wpc || !k || !h) return fail(c, ASTRA_EINVAL, "GPU parameters must be >= 1");
     if ((u64)cus * wpc > ASTRA_MAX_WAVEFRONTS) return fail(c, ASTRA_ELIMIT, "cus * wavefronts_per_cu above ASTRA_MAX_WAVEFRONTS");
     if (k > ASTRA_MAX_OUTSTANDING) return fail(c, ASTRA_ELIMIT, "max_outstanding above ASTRA_MAX_OUTSTANDING");
     if (h > ASTRA_MAX_HBM_LINES) return fail(c, ASTRA_ELIMIT, "hbm_lines_per_cycle above ASTRA_MAX_HBM_LINES");
-    HostGpu g; g.C = cus; g.Wv = wpc; g.K = k; g.H = h;
+    HostGpu g; g.C = cus; g.Wv = wpc; g.K = k; g.H = h; g.mode = mode;
     c->gpus.push_back(g);
     *out_id = (u32)c->gpus.size() - 1;
     return ASTRA_OK;

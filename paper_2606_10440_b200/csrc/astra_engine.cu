@@ -39,10 +39,15 @@
 #include <cuda_runtime.h>
 
 #define FULL 0xffffffffu
+#ifdef ASTRA_X_COLD
+#define ASTRA_COLD __noinline__
+#else
+#define ASTRA_COLD
+#endif
 #define SCR_WORDS 1088u   // per-warp scratch words: 32 lanes x 64 16-bit ack keys (wf_sim, wf_priority_word), 513 counters (ack_sort), 512 (ack_chunk)
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
-    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, W, NC, NWmask, NW, kmagic, tmax, flags, alcap;
+    u32 G, V, E, S, C, Wv, K, H, CW, nwords, slots, bmwords, W, NC, NWmask, NW, kmagic, tmax, flags, alcap, pcu;
     u32 group, rank, v_lo, v_hi, g_lo, g_hi, e_lo, e_hi, i_lo, i_hi;
     u64 fullmask;
 #define X(n) const u32* n;
@@ -237,7 +242,7 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
 // ---------------------------------------------------------------------------------------------
 // Cycle-serial path only: consume the window's ack bits of GPU g into ack_sorted, counting-sorted
 // by cycle (low word: cycle << 18 | wavefront << 6 | slot).
-__device__ void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
+__device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 k, u32 t0, u32 wlen, u32* scnt, u32 lane) {
     const u32 bin = k & c.NWmask;
     const u32 n = c.ack_n[g];
     if (n == 0) return;
@@ -385,7 +390,7 @@ __device__ void ack_list_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 c
 // 32 bitmap words of GPU g's ack bin: per-step ack counts, t_ack, ACKED events, amask (R6, A3).
 // The set bits are first compacted into the warp's scratch so that every lane handles the same
 // number of acks whatever their spread over the words, four record loads in flight per lane.
-__device__ void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32* scr, u32 lane) {
+__device__ ASTRA_COLD void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, u32 k, u32 t1, u32* scr, u32 lane) {
     const u32 CAP = 512;
     const u32 bin = k & c.NWmask;
     const u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
@@ -682,11 +687,21 @@ __device__ __forceinline__ bool wf_advance(const Ctx& __restrict__ c, u32 g, u32
     return false;
 }
 
+// Per-CU cap (R2'): the "has a free slot" bits of the W wavefronts of CU `cu` follow the CU's pool together.
+__device__ __forceinline__ void cu_set_free(u32* freeb, u32 cu, u32 Wv, bool free_now) {
+    const u32 lo = cu * Wv, hi = lo + Wv;                       // Wv <= 32: at most two words
+    const u32 w0 = lo >> 5, w1 = (hi - 1) >> 5;
+    const u32 m0 = (w0 == w1 ? ((Wv == 32 ? ~0u : ((1u << Wv) - 1u)) << (lo & 31)) : (~0u << (lo & 31)));
+    if (free_now) atomicOr(&freeb[w0], m0); else atomicAnd(&freeb[w0], ~m0);
+    if (w1 != w0) { const u32 m1 = (1u << (hi & 31)) - 1u; if (free_now) atomicOr(&freeb[w1], m1); else atomicAnd(&freeb[w1], ~m1); }
+}
+
 // ---------------------------------------------------------------------------------------------
 // stage 2: release + issue of GPU g over [t0, t1)   (R10 - R13, slot return of R7 A3)
 // ---------------------------------------------------------------------------------------------
-__device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
+__device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 t0, u32 t1, u32 cb, u32 lane) {
     const u32 ack_n = c.ack_n[g];
+    const u32 pcu = c.pcu;                                      // bit 0: one line per CU per cycle (R12'), bit 1: cap per CU (R2')
     const u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32* plist = c.plist + c.rel_off[g];
     u32* want = c.want + (size_t)g * c.nwords;
@@ -735,12 +750,19 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g
                         busy &= ~(((u64)bhi << 32) | blo);
                         c.wf_busy[(size_t)g * c.CW + wf] = busy;
                     }
-                    const u32 wi = wf >> 5;
-                    const u32 mi = __match_any_sync(nm, wi);
-                    const u32 bits = __reduce_or_sync(mi, 1u << (wf & 31));
-                    if ((mi & lanemask_lt()) == 0) freeb[wi] |= bits;
+                    if (pcu & 2u) {                                  // R2': the slots return to the CU's pool
+                        const u32 cu = wf / c.Wv;
+                        const u32 mc = __match_any_sync(nm, cu);
+                        if ((mc & lanemask_lt()) == 0) { c.cu_out[(size_t)g * c.C + cu] -= (u32)__popc(mc); cu_set_free(freeb, cu, c.Wv, true); }
+                    } else {
+                        const u32 wi = wf >> 5;
+                        const u32 mi = __match_any_sync(nm, wi);
+                        const u32 bits = __reduce_or_sync(mi, 1u << (wf & 31));
+                        if ((mi & lanemask_lt()) == 0) freeb[wi] |= bits;
+                    }
                 }
                 ack_pos += __popc(nm);
+                __syncwarp();                                        // the pool counts of one round are seen by the next
                 if (ack_pos - abase < 32 || ack_pos >= ack_n) break;
                 abase = ack_pos;                                     // register window exhausted: refill
                 abuf = (abase + lane < ack_n) ? (u32)srt[abase + lane] : 0xffffffffu;
@@ -798,6 +820,43 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g
         // ---- phase D: issue (R11 - R13) ----
         u32 budget = c.H, nsel = 0;
         bool left_over = false;
+        if (pcu) {
+            // per-CU readings: one CU per lane.  Of its ready wavefronts a CU may dispatch the lowest one (R12') or as
+            // many as its pool has room for (R2'); then the first H of all of them in ascending wavefront id (R12).
+            const u32 Wv = c.Wv;
+            for (u32 cb0 = 0; cb0 < c.C; cb0 += 32) {
+                const u32 cu = cb0 + lane;
+                u32 keep = 0, lo = 0;
+                bool more_ready = false;
+                if (cu < c.C) {
+                    lo = cu * Wv;
+                    const u32 w0 = lo >> 5, sh = lo & 31;
+                    u64 r2 = (u64)(want[w0] & freeb[w0]);
+                    if (w0 + 1 < c.nwords) r2 |= (u64)(want[w0 + 1] & freeb[w0 + 1]) << 32;
+                    u32 bits = (u32)(r2 >> sh) & (Wv == 32 ? ~0u : ((1u << Wv) - 1u));
+                    u32 room = Wv;
+                    if (pcu & 1u) room = 1u;
+                    if (pcu & 2u) room = min(room, c.K - c.cu_out[(size_t)g * c.C + cu]);
+                    for (u32 q = 0; q < room && bits; q++) { const u32 low = bits & (0u - bits); keep |= low; bits ^= low; }
+                    more_ready = bits != 0u;
+                }
+                const u32 cntc = __popc(keep);
+                const u32 incl = warp_incl_scan(cntc, lane);
+                const u32 tot = __shfl_sync(FULL, incl, 31);
+                if (__any_sync(FULL, more_ready)) left_over = true;
+                if (tot == 0) continue;
+                if (budget == 0) { left_over = true; break; }
+                const u32 excl = incl - cntc;
+                const u32 take = excl >= budget ? 0 : min(cntc, budget - excl);
+                for (u32 i = 0; i < take; i++) {
+                    const u32 b = __ffs(keep) - 1; keep &= keep - 1;
+                    sel[nsel + excl + i] = lo + b;
+                }
+                const u32 got = min(tot, budget);
+                if (tot > got) left_over = true;
+                nsel += got; budget -= got;
+            }
+        } else
         for (u32 wb = 0; wb < c.nwords; wb += 32) {
             const u32 wi = wb + lane;
             u32 r = (wi < c.nwords) ? (want[wi] & freeb[wi]) : 0;
@@ -874,11 +933,20 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g
                 }
                 const u32 wi = wf >> 5;
                 const u32 mi = __match_any_sync(amask, wi);
-                const u32 clrf = __reduce_or_sync(mi, full ? (1u << (wf & 31)) : 0u);
+                const u32 clrf = __reduce_or_sync(mi, (full && !(pcu & 2u)) ? (1u << (wf & 31)) : 0u);
                 const u32 clrw = __reduce_or_sync(mi, keepw ? 0u : (1u << (wf & 31)));
                 if ((mi & lanemask_lt()) == 0) {
-                    if (clrf) freeb[wi] &= ~clrf;
+                    if (clrf) atomicAnd(&freeb[wi], ~clrf);
                     if (clrw) want[wi] &= ~clrw;
+                }
+                if (pcu & 2u) {                                  // R2': the CU's pool fills
+                    const u32 cu = wf / c.Wv;
+                    const u32 mc = __match_any_sync(amask, cu);
+                    if ((mc & lanemask_lt()) == 0) {
+                        const u32 nout = c.cu_out[(size_t)g * c.C + cu] + (u32)__popc(mc);
+                        c.cu_out[(size_t)g * c.C + cu] = nout;
+                        if (nout >= c.K) cu_set_free(freeb, cu, c.Wv, false);
+                    }
                 }
             }
             u32 cm = __ballot_sync(FULL, completed);
@@ -888,6 +956,7 @@ __device__ void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g
                 on_event(c, g, p, ASTRA_DEP_ISSUED, t + 1, lane);      // visible to phase C of t + 1 (R10)
                 t_rel_next = ASTRA_T_INF;                               // recomputed below
             }
+            __syncwarp();                                               // counters of one batch of 32 are seen by the next
         }
         __syncwarp();
         if (nsel) more = true;            // an issuing wavefront may issue again at t + 1
@@ -961,7 +1030,7 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
     }
     const bool active = __ballot_sync(FULL, any != 0) != 0;
     u32 mode = 0;
-    if (active) mode = ((c.gflag[g] & ASTRA_GF_ISSUED_DEPS) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE)) ? 2u : 1u;
+    if (active) mode = ((c.gflag[g] & (ASTRA_GF_ISSUED_DEPS | ASTRA_GF_SERIAL)) || (c.flags & (u32)ASTRA_FLAG_SERIAL_ISSUE)) ? 2u : 1u;
     if (mode == 1) {
         const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
         u32* cnt = c.cnt + (size_t)g * c.W;
@@ -1254,7 +1323,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
 }
 
 // The budget bound: put the wavefronts of GPU g back to their state at the window start.
-__device__ void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
+__device__ ASTRA_COLD void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
     for (u32 wi = 0; wi < c.nwords; wi++) {
         const u32 am = c.amask[(size_t)g * c.nwords + wi];
         if (am == 0) continue;
@@ -1275,7 +1344,7 @@ __device__ void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
 // lower id are granted at t; occ[t] (the cnt array) holds the grants of all lower words, so the 32
 // wavefronts of a word step together through the cycles where one of them is ready and occ[t] < H,
 // a ballot giving the rank inside the word.  That rank is the bucket position of the issue.
-__device__ void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+__device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am = c.amask[(size_t)g * nwords + wi];
     if (am == 0) return;
@@ -1785,7 +1854,7 @@ __device__ void resolve_ctx(Ctx& c, const PointDesc& P, const uint8_t* cb, uint8
     c.G = P.G; c.V = P.V; c.E = P.E; c.S = P.S; c.C = P.C; c.Wv = P.Wv; c.K = P.K; c.H = P.H;
     c.CW = P.CW; c.nwords = P.nwords; c.slots = P.slots; c.bmwords = P.bmwords;
     c.W = P.Wcyc; c.NC = P.NC; c.NW = P.NW; c.NWmask = P.NW - 1; c.kmagic = P.kdiv_magic;
-    c.tmax = (u32)P.max_cycles; c.flags = P.flags; c.alcap = P.alcap;
+    c.tmax = (u32)P.max_cycles; c.flags = P.flags; c.alcap = P.alcap; c.pcu = P.pcu;
     c.fullmask = P.K >= 64 ? ~0ull : ((1ull << P.K) - 1);
     c.group = P.group; c.rank = rank;
 #define X(n) c.n = (const u32*)(cb + P.c_off[ASTRA_C_##n]);

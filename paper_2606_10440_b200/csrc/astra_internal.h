@@ -33,6 +33,7 @@ typedef uint64_t u64;
 #define ASTRA_LF_FORWARD_ONLY 2u           // lflag: every line over the link goes on to the single-feeder link lfwd[e]
 #define ASTRA_LF_CELLS 3u                  // lflag: lines terminate at the head or go on to multi-feeder links only (cells)
 #define ASTRA_GF_ISSUED_DEPS 1u            // gflag: some step of the GPU has an ISSUED-kind successor
+#define ASTRA_GF_SERIAL 2u                 // gflag: the GPU model couples the wavefronts of a CU: cycle-serial issue path
 
 // Link service kinds (R9): how the acceptance times of a FIFO are computed for a whole window.
 #define ASTRA_LK_INT     0u               // bw = B*256: B lines every cycle, no carried credit
@@ -57,7 +58,7 @@ typedef uint64_t u64;
     X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
-    X(bin_cnt, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
+    X(bin_cnt, u32, 0) X(cu_out, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \
     X(hlist, u32, 3) X(undo_busy, u64, 3) X(undo_rem, u32, 3) X(undo_cur, u32, 3) X(undo_want, u32, 3) X(undo_freeb, u32, 3) \
     X(lscr, u32, 3) X(bitmap, u32, 0) X(ack_list, u32, 3) X(inj_list, u64, 3) X(ack_rec, u64, 3) X(ack_tmp, u64, 3) X(ack_sorted, u64, 3) X(evb, u64, 3) X(ring, u64, 3)
 
@@ -93,6 +94,7 @@ struct PointDesc {
     u32 CW, nwords, slots, bmwords;
     u32 Wcyc, NW, kdiv_magic, NC;              // Wcyc lookahead window in cycles; NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
     u32 flags, group;                          // group: CTAs cooperating on this point
+    u32 pcu, pad1;                             // pcu: ASTRA_GPU_ISSUE_PER_CU | ASTRA_GPU_CAP_PER_CU of the point's GPU model
     u32 hot_bytes, alcap;                      // alcap: entries per (GPU, window bin) ack discovery list
     u64 max_cycles;
     u64 total_lines;
@@ -140,7 +142,7 @@ struct HostColl {
     u64 total_lines = 0;
 };
 
-struct HostGpu { u32 C = 0, Wv = 0, K = 0, H = 0; };
+struct HostGpu { u32 C = 0, Wv = 0, K = 0, H = 0, mode = 0; };
 
 struct Blob {                       // append-only byte buffer with 16-byte aligned sections
     std::vector<uint8_t> bytes;

@@ -194,6 +194,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     P.total_lines = c.total_lines;
     P.flags = (u32)opt.flags;
     P.group = group;
+    P.pcu = g.mode & 3u;
     u64 tmax = std::min<u64>(opt.max_cycles, ASTRA_MAX_CYCLES);       // documented clamp (include/astra.h)
     P.max_cycles = tmax;
 
@@ -401,6 +402,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     for (u32 s = 0; s < S; s++)
         for (u32 i = c.succ_ptr[s]; i < c.succ_ptr[s + 1]; i++)
             if ((c.succ[i] >> 30) == ASTRA_DEP_ISSUED) gflag[c.owner[s]] |= ASTRA_GF_ISSUED_DEPS;
+    if (g.mode & 3u) for (u32 q = 0; q < G; q++) gflag[q] |= ASTRA_GF_SERIAL;      // per-CU readings (R12', R2')
 
     // constant tables
     u64* co = P.c_off;
@@ -447,6 +449,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
                   ASTRA_A_ack_cnt, ASTRA_A_t_ack, ASTRA_A_ndep_left, ASTRA_A_rel_time, ASTRA_A_plist}) ab[a] = 4ull * S;
     ab[ASTRA_A_ev_list] = 4ull * ev_off[G];
     ab[ASTRA_A_bin_cnt] = 4ull * G * P.NW;
+    ab[ASTRA_A_cu_out] = (g.mode & 3u) ? 4ull * G * g.C : 0;
     ab[ASTRA_A_wf_busy] = ab[ASTRA_A_undo_busy] = 8ull * GW;
     ab[ASTRA_A_wf_rem] = ab[ASTRA_A_wf_cur] = ab[ASTRA_A_undo_rem] = ab[ASTRA_A_undo_cur] = ab[ASTRA_A_hlist] = 4ull * GW;
     ab[ASTRA_A_lscr] = 4ull * lscr_total;

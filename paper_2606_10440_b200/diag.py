@@ -13,9 +13,7 @@ from __future__ import annotations
 import os
 import sys
 
-os.environ["ASTRA_DIAG"] = "1"            # must be set before the binding picks its library
-
-import numpy as np  # noqa: E402
+import numpy as np
 
 STAGES = ["arrivals+acks", "release", "wavefront runs", "check/commit", "placement", "merge", "link service", "barrier wait"]
 
@@ -39,8 +37,10 @@ def describe(d) -> str:
 
 def run(name: str, top: int):
     from astra_inputs import configs
-    from . import build
+    from . import binding, build
     from .binding import Engine
+    if binding._LIBPATH != build.LIB_DIAG:              # this process uses the instrumented library
+        binding._LIBPATH, binding._lib = build.LIB_DIAG, None
     build.build(diag=True)
     w = configs.by_name(name)
     with Engine(0, 0) as e:

@@ -9,6 +9,7 @@ from astra_inputs.types import CollectiveBuilder
 GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "pins_survey_8c.json")))
 ROUND2 = ["G1_grant_order_H2", "G1_grant_order_H1", "G1_grant_order_K1", "G2_credit_096", "G2_credit_384",
           "G3_dep_issued", "G3_dep_acked"]
+PER_CU = ["H1_issue_per_cu", "H2_cap_per_cu", "H3_issue_and_cap_per_cu"]
 
 
 def build(key):
@@ -21,4 +22,4 @@ def build(key):
         coll = b.build()
     else:
         coll = C.single_transfer(2, 0, 1, s["lines"], 0, s["cus"])
-    return topo, coll, GpuCfg(s["cus"], s["wpc"], s["k"], s["h"])
+    return topo, coll, GpuCfg(s["cus"], s["wpc"], s["k"], s["h"], s.get("mode", 0))

@@ -49,6 +49,41 @@ def test_round2_hand_traces(key):
     assert res[0][1].tolist() == want
 
 
+@pytest.mark.parametrize("key", __import__("tests.pin_cases", fromlist=["PER_CU"]).PER_CU)
+def test_per_cu_hand_traces(key):
+    """The paper's per-CU readings (astra_set_gpu_ex: one line per CU per cycle, outstanding cap per CU):
+    engine == oracle == the hand-derived values."""
+    from tests import pin_cases
+    topo, coll, gpu = pin_cases.build(key)
+    res, _ = check_workload(_single(topo, coll, gpu, name=key))
+    assert res[0][1].tolist() == [pin_cases.GOLD[key]["step_ts"]]
+
+
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_per_cu_modes_random_and_families(mode):
+    """Per-CU modes on random workloads (all dep kinds, 1-cycle windows), on config 1 and on small instances of
+    the collective families, one CTA and CTA groups."""
+    import dataclasses
+    from paper_2606_10440_b200.binding import FLAG_GROUP
+    for seed in (41, 42, 43, 44):
+        w = configs.random_workload(seed, n_points=6, max_gpus=6, max_steps=24, max_lines=200)
+        w.gpus = [dataclasses.replace(g, mode=mode) for g in w.gpus]
+        check_workload(w)
+        check_workload(w, flags=FLAG_GROUP(3))
+    w = configs.config1()
+    w.gpus = [dataclasses.replace(g, mode=mode) for g in w.gpus]
+    check_workload(w)
+    gpu = GpuCfg(8, 4, 6, 5, mode)
+    for topo, coll in [(T.ring(8, 256, 9), C.ring_allreduce(8, 403, 8)[0]),
+                       (T.torus2d(2, 4, 128, 7), C.direct_allreduce(8, 370, 8)),
+                       (T.single_switch(4, 512, 6, 3), C.direct_allreduce(4, 320, 8)),
+                       (T.rail_optimized(2, 8, 512, 5, 2, 256, 9, 0), C.all_to_all(16, lambda g, d: 1 + (g * 7 + d * 3) % 19, 8))]:
+        check_workload(_single(topo, coll, gpu))
+    w = configs.config2(range(6, 8))
+    w.gpus = [dataclasses.replace(g, mode=mode) for g in w.gpus]
+    check_workload(w, processes=4)
+
+
 def test_config1_bit_exact_and_pin():
     gpu, _ = check_workload(configs.config1())
     assert gpu[0][0].completion_cycle == 38623          # SURVEY 8(c) P4

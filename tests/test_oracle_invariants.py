@@ -100,6 +100,26 @@ def test_bruteforce_agreement_random(seed):
         assert a.link_lines.astype(np.int64).tolist() == b["link_lines"]
 
 
+@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("seed", range(12))
+def test_bruteforce_agreement_per_cu_modes(seed, mode):
+    """The per-CU readings (R12' one line per CU per cycle, R2' outstanding cap per CU): oracle == tiny_sim on
+    random cases, plain and pruned scan alike, and never faster to issue than the per-wavefront reading allows."""
+    import dataclasses
+    w = configs.random_workload(300 + seed, n_points=2, max_lines=40)
+    for i in range(w.n_points):
+        topo, coll, gpu0 = w.point(i)
+        gpu = dataclasses.replace(gpu0, mode=mode)
+        a = oracle.run_point(topo, coll, gpu)
+        a2 = oracle.run_point(topo, coll, gpu, flags=oracle.FLAG_PRUNED_SCAN)
+        b = tiny_sim.simulate(topo, coll, gpu)
+        assert a.status == b["status"] == 0
+        assert a.step_ts.astype(np.int64).tolist() == b["step_ts"]
+        assert a.link_lines.astype(np.int64).tolist() == b["link_lines"]
+        assert (a.step_ts == a2.step_ts).all() and (a.link_lines == a2.link_lines).all()
+        assert (a.link_lines == oracle.run_point(topo, coll, gpu0).link_lines).all()      # same routes, same counts
+
+
 def _small_named_cases():
     cases = []
     gpu = GpuCfg(8, 2, 4, 6)

@@ -210,7 +210,7 @@ def test_routing_fat_tree_d_mod_k():
 from tests import pin_cases
 
 
-@pytest.mark.parametrize("key", pin_cases.ROUND2)
+@pytest.mark.parametrize("key", pin_cases.ROUND2 + pin_cases.PER_CU)
 def test_round2_hand_traces(key):
     """R12 grant order when H binds (lowest ready wavefront id first), R9 saturating
     credit at bandwidths that are neither integer nor 1/P, R10 release timing of ISSUED- and

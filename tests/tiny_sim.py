@@ -66,6 +66,7 @@ def simulate(topo, coll, gpu, max_cycles=1 << 22):
     deps = [[(int(coll.dep_step[i]), int(coll.dep_kind[i]))
              for i in range(int(coll.dep_ptr[s]), int(coll.dep_ptr[s + 1]))] for s in range(S)]
     C, W, K, H = gpu.cus, gpu.wavefronts_per_cu, gpu.max_outstanding, gpu.hbm_lines_per_cycle
+    per_cu_issue, per_cu_cap = bool(getattr(gpu, "mode", 0) & 1), bool(getattr(gpu, "mode", 0) & 2)     # R12', R2'
 
     # quota[(s, wf)]: deal the lines of step s round-robin over its wavefronts
     quota = {}
@@ -83,7 +84,7 @@ def simulate(topo, coll, gpu, max_cycles=1 << 22):
             cu = wf // W
             work[(g, wf)] = [[s, quota[(s, wf)]] for s in range(S)
                              if owner[s] == g and cu_lo[s] <= cu < cu_lo[s] + cu_n[s]]
-    outstanding = defaultdict(int)
+    outstanding = defaultdict(int)          # keyed (gpu, wavefront), or (gpu, 'cu', cu) for the per-CU pool
 
     ts = [[None] * 4 for _ in range(S)]   # release, issued, delivered, acked
     cnt_issued = [0] * S
@@ -119,7 +120,7 @@ def simulate(topo, coll, gpu, max_cycles=1 << 22):
             injected_prev[g] = []
         # A3
         for ln in ack_cal.pop(t, []):
-            outstanding[(ln.gpu, ln.wf)] -= 1
+            outstanding[(ln.gpu, "cu", ln.wf // W) if per_cu_cap else (ln.gpu, ln.wf)] -= 1
             cnt_ack[ln.step] += 1
             if cnt_ack[ln.step] == lines[ln.step]:
                 ts[ln.step][3] = t
@@ -145,19 +146,24 @@ def simulate(topo, coll, gpu, max_cycles=1 << 22):
         # D
         for g in range(G):
             budget = H
+            dispatched = set()                          # CUs that have issued this cycle
             for wf in range(C * W):
                 if budget == 0:
                     break
+                if per_cu_issue and wf // W in dispatched:
+                    continue
                 lst = work[(g, wf)]
                 while lst and ts[lst[0][0]][0] is not None and lst[0][1] == 0:
                     lst.pop(0)
                 if not lst or ts[lst[0][0]][0] is None:
                     continue
-                if outstanding[(g, wf)] >= K:
+                slot_key = (g, "cu", wf // W) if per_cu_cap else (g, wf)
+                if outstanding[slot_key] >= K:
                     continue
                 s = lst[0][0]
                 lst[0][1] -= 1
-                outstanding[(g, wf)] += 1
+                outstanding[slot_key] += 1
+                dispatched.add(wf // W)
                 cnt_issued[s] += 1
                 if cnt_issued[s] == lines[s]:
                     ts[s][1] = t
