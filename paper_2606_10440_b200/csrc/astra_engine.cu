@@ -1915,8 +1915,13 @@ __device__ __forceinline__ void set_sync(u32 ws, u32 set) {
 // set of ws warps).  Inside a window nothing a node does can reach another node (W <= min Leff), so
 // the stages of a node order only against each other: set barriers, no block barrier.
 // ---------------------------------------------------------------------------------------------
+#ifdef ASTRA_X_LOCKSTEP
+#define LOCKSTEP() do { if (lockstep) __syncthreads(); } while (0)
+#else
+#define LOCKSTEP() do { } while (0)
+#endif
 __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
-                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane) {
+                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, bool lockstep) {
 #ifdef ASTRA_DIAG
     long long dck = clock64();
 #endif
@@ -1990,61 +1995,72 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     DIAG_CLK(0);
 
     // ---- stage 2: release + issue of GPU v (R10 - R13) ----
+    LOCKSTEP();
+    u32 mode = 0;
+    const u32 g = v;
     if (is_gpu) {
-        const u32 g = v;
         if (sw == 0) gpu_prepare(c, ctl, g, t0, t1, lane);
         set_sync(ws, set);
         DIAG_CLK(1);
-        u32 mode = c.gmode[g];
-        if (mode == 1u) {
-            for (u32 wi = sw; wi < c.nwords; wi += ws) wf_sim(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+        mode = c.gmode[g];
+    }
+    LOCKSTEP();
+    if (mode == 1u) {
+        for (u32 wi = sw; wi < c.nwords; wi += ws) wf_sim(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+        set_sync(ws, set);
+    }
+    LOCKSTEP();
+    if (mode == 1u) {
+        const u32 nh = c.nheavy[g];
+        if (nh) {
+            for (u32 j = sw; j < nh; j += ws) wf_heavy(c, ctl, hp, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
             set_sync(ws, set);
-            const u32 nh = c.nheavy[g];
-            if (nh) {
-                for (u32 j = sw; j < nh; j += ws) wf_heavy(c, ctl, hp, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
-                set_sync(ws, set);
-            }
-            DIAG_CLK(2);
-            const bool bind = gpu_binds(c, g, wlen, lane);     // every warp checks: the same answer everywhere ...
-            set_sync(ws, set);                                  // ... before anybody writes over the counts
-            if (!bind) {                                        // the parts of the commit are dealt out
+        }
+        DIAG_CLK(2);
+    }
+    LOCKSTEP();
+    if (mode == 1u) {
+        const bool bind = gpu_binds(c, g, wlen, lane);     // every warp checks: the same answer everywhere ...
+        set_sync(ws, set);                                  // ... before anybody writes over the counts
+        if (!bind) {                                        // the parts of the commit are dealt out
+            const u32 deg = e_hi - e_lo;
+            if (sw == 0) gpu_finalize_counts(c, g, k, wlen, lane);
+            if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) gpu_finalize_link(c, e_lo + x, wlen, lane);
+            if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
+        } else if (sw == 0) {
+            // the budget binds: back to the window start, then exact grants
+            if (lane == 0) DIAG_ADD(6, 1);
+            wf_restore(c, g, lane);
+            if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
+            else {
                 const u32 deg = e_hi - e_lo;
-                if (sw == 0) gpu_finalize_counts(c, g, k, wlen, lane);
-                if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) gpu_finalize_link(c, e_lo + x, wlen, lane);
-                if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
-            } else if (sw == 0) {
-                // the budget binds: back to the window start, then exact grants
-                if (lane == 0) DIAG_ADD(6, 1);
-                wf_restore(c, g, lane);
-                if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
-                else {
-                    const u32 deg = e_hi - e_lo;
-                    for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
-                    if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
-                    __syncwarp();
-                    for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
-                    gpu_finalize(c, g, k, wlen, lane);
-                }
+                for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
+                if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
+                __syncwarp();
+                for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
+                gpu_finalize(c, g, k, wlen, lane);
             }
-            set_sync(ws, set);
-            mode = c.gmode[g];
         }
-        if (mode == 2u) {                        // cycle-serial path
-            if (sw == 0) {
-                ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
-                issue_window(c, ctl, hp, g, t0, t1, cb, lane);
-                for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
-            }
-            set_sync(ws, set);
-            DIAG_CLK(3);
-        } else if (mode == 1u) {
-            DIAG_CLK(3);
-            const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
-            for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
-            set_sync(ws, set);
-            DIAG_CLK(4);
+        set_sync(ws, set);
+        mode = c.gmode[g];
+    }
+    LOCKSTEP();
+    if (mode == 2u) {                        // cycle-serial path
+        if (sw == 0) {
+            ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
+            issue_window(c, ctl, hp, g, t0, t1, cb, lane);
+            for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
         }
-    } else if (any_fwd) set_sync(ws, set);
+        set_sync(ws, set);
+        DIAG_CLK(3);
+    } else if (mode == 1u) {
+        DIAG_CLK(3);
+        const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
+        for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
+        set_sync(ws, set);
+        DIAG_CLK(4);
+    } else if (!is_gpu && any_fwd) set_sync(ws, set);
+    LOCKSTEP();
 
     // ---- stage 3: merge into multi-feeder out-links of v (skipped when none received a line) ----
     bool any_dirty = false;
@@ -2054,6 +2070,9 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         for (u32 e = e_lo + sw; e < e_hi; e += ws)
             if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
         set_sync(ws, set);
+    }
+    LOCKSTEP();
+    if (any_dirty) {
         if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
         u32 tmod3 = 0;
         for (u32 ib = i_lo; ib < i_hi; ib += 32) {
@@ -2082,6 +2101,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         set_sync(ws, set);
     }
     DIAG_CLK(5);
+    LOCKSTEP();
 
     // ---- stage 4: link service of v's out-links (R9); the in-links' cursors move past the window ----
     if (sw == ws - 1) {
@@ -2212,6 +2232,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const u32 wset = nwarps / nsets;                   // warps per set (left-over warps idle through the window)
         const u32 set = warp / wset, sw = warp % wset;
         const bool in_set = set < nsets;
+        const bool lockstep = n_nodes == nwarps;            // experiment: every warp steps exactly one node per window
 
         // ---- window loop ----
         u32 k = 0, seq = 0;
@@ -2229,7 +2250,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             busy += t1 - t0;
             if (in_set)
                 for (u32 j = set; j < n_nodes; j += nsets)
-                    node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0);
+                    node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0, lockstep);
             // ---- stage 5: next non-idle window (A7), one block barrier per window ----
 #ifdef ASTRA_DIAG
             dck = clock64();
