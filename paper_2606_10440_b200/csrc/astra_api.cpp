@@ -239,6 +239,14 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev), "device attribute");
     const u32 smem_cta = std::min<u32>((u32)smem_max, (u32)smem_sm / ctas_per_sm - 1024);    // 1 KB per CTA is reserved by the system
     opt.hot_budget = smem_cta > fixed + 1024 ? smem_cta - fixed - 1024 : 0;
+    // Shared memory and L1 are one 256 KB array per SM, and the state that does not fit in shared memory (rings, ack
+    // records, the constant tables) is read through L1: measured on the five configs, a hot region beyond 48 KB
+    // (64 KB for batches with CTA groups) costs more in L1 misses than it saves (config 4: 157 KB -> 48 KB, -6 %).
+    {
+        bool any_big = false;
+        for (u32 i = 0; i < n; i++) any_big |= big[i] != 0;
+        opt.hot_budget = std::min<u32>(opt.hot_budget, any_big ? ASTRA_HOT_BUDGET_GROUPS : ASTRA_HOT_BUDGET_SINGLE);
+    }
     u32 hot_max = 0, n_big = 0;
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];

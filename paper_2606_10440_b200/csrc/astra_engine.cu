@@ -67,8 +67,9 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 hint[3];        // min over everything pending of its next event time; slot seq % 3 is the window's (A7)
     u32 g_hint, g_acked, g_err, g_completion;   // group mode: the group-wide values after the window's group barrier
     u32 abort;          // a group barrier timed out somewhere: leave the kernel
+    u32 nbb, bbq[32];   // one-warp nodes whose budget-bound sweep waits for the CTA this window (bb_sweep)
 #ifdef ASTRA_DIAG
-    u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows
+    u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows, [7] clocks on that path, [8] windows with such a GPU
     u64 sclk[16][8];    // per warp set (clocks of its first warp, summed over its nodes and windows): 0 arrivals+acks,
                         // 1 release events, 2 wavefront runs, 3 budget check / commit, 4 placement, 5 merge, 6 link service,
                         // 7 waiting at the end-of-window barrier (block + group)
@@ -1322,21 +1323,32 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
     __syncwarp();
 }
 
-// The budget bound: put the wavefronts of GPU g back to their state at the window start.
-__device__ ASTRA_COLD void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane) {
-    for (u32 wi = 0; wi < c.nwords; wi++) {
-        const u32 am = c.amask[(size_t)g * c.nwords + wi];
-        if (am == 0) continue;
-        if ((am >> lane) & 1u) {
-            const size_t gw = (size_t)g * c.CW + wi * 32 + lane;
-            c.wf_cur[gw] = c.undo_cur[gw]; c.wf_rem[gw] = c.undo_rem[gw]; c.wf_busy[gw] = c.undo_busy[gw];
-        }
-        if (lane == 0) {
-            c.want[(size_t)g * c.nwords + wi] = c.undo_want[(size_t)g * c.nwords + wi];
-            c.freeb[(size_t)g * c.nwords + wi] = c.undo_freeb[(size_t)g * c.nwords + wi];
-        }
+// The budget bound: put the wavefronts of word wi of GPU g back to their state at the window start.
+__device__ ASTRA_COLD void wf_restore_word(const Ctx& __restrict__ c, u32 g, u32 wi, u32 lane) {
+    const u32 am = c.amask[(size_t)g * c.nwords + wi];
+    if (am == 0) return;
+    if ((am >> lane) & 1u) {
+        const size_t gw = (size_t)g * c.CW + wi * 32 + lane;
+        c.wf_cur[gw] = c.undo_cur[gw]; c.wf_rem[gw] = c.undo_rem[gw]; c.wf_busy[gw] = c.undo_busy[gw];
+    }
+    if (lane == 0) {
+        c.want[(size_t)g * c.nwords + wi] = c.undo_want[(size_t)g * c.nwords + wi];
+        c.freeb[(size_t)g * c.nwords + wi] = c.undo_freeb[(size_t)g * c.nwords + wi];
     }
     __syncwarp();
+}
+
+// The words of a budget-bound GPU-window are swept in ascending order (word w needs the grants of all lower
+// words), but by several warps: each loads and sorts its word's inputs on its own, then waits for its turn.
+__device__ __forceinline__ void turn_wait(u32* turn, u32 wi, u32 lane) {
+    if (lane == 0) while (*(volatile u32*)turn != wi) __nanosleep(40);
+    __syncwarp();
+    __threadfence_block();
+}
+__device__ __forceinline__ void turn_pass(u32* turn, u32 wi, u32 lane) {
+    __syncwarp();
+    __threadfence_block();
+    if (lane == 0) *(volatile u32*)turn = wi + 1u;
 }
 
 // The budget binds in this GPU-window: exact fixed-priority grants (R12), word by word in ascending
@@ -1344,10 +1356,10 @@ __device__ ASTRA_COLD void wf_restore(const Ctx& __restrict__ c, u32 g, u32 lane
 // lower id are granted at t; occ[t] (the cnt array) holds the grants of all lower words, so the 32
 // wavefronts of a word step together through the cycles where one of them is ready and occ[t] < H,
 // a ballot giving the rank inside the word.  That rank is the bucket position of the issue.
-__device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+__device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 wi, u32 k, u32 t0, u32 t1, u32* scr, u32* turn, u32 lane) {
     const u32 nwords = c.nwords;
     const u32 am = c.amask[(size_t)g * nwords + wi];
-    if (am == 0) return;
+    if (am == 0) { if (turn) { turn_wait(turn, wi, lane); turn_pass(turn, wi, lane); } return; }
     const bool active = (am >> lane) & 1u;
     const u32 wf = wi * 32 + lane;
     const u32 W = c.W, H = c.H, K = c.K, wlen = t1 - t0;
@@ -1390,6 +1402,7 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
     u32 s = 0, ox = 0, last_issue = 0xffffffffu;
     bool have_s = false;
     u32 T = 0;
+    if (turn) turn_wait(turn, wi, lane);                       // the grants of all lower words are in occ[] now
     for (;;) {
         // bring the lane to cycle T: slots returned by T, step loaded if released by T
         u32 np = 0xffffffffu;                                   // earliest cycle this lane can be ready
@@ -1443,6 +1456,7 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
         T++;
         if (T >= wlen) break;
     }
+    if (turn) turn_pass(turn, wi, lane);
     bool wantb = false, freebit = false, hint = false;
     if (active) {
         for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));
@@ -1910,18 +1924,109 @@ __device__ __forceinline__ void set_sync(u32 ws, u32 set) {
     else asm volatile("bar.sync %0, %1;" :: "r"(set + 1u), "r"(ws * 32u) : "memory");
 }
 
+// The rest of a node's window after the issue decisions: placement of the window's issues (or the cycle-serial
+// issue path), merge into multi-feeder out-links, link service.  e_l .. fl_l: the node's first 32 in-links, one per
+// lane (id, lines due, read cursor, arrival path), as loaded by stage 1 (inlinks_first reloads them).
+__device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
+                          u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, u32 mode,
+                          u32 e_l, u32 n_l, u32 lo_l, u32 fl_l) {
+#ifdef ASTRA_DIAG
+    long long dck = clock64();
+#endif
+    const u32 wlen = t1 - t0;
+    const bool is_gpu = v < c.G;
+    const u32 g = v;
+    const u32 i_lo = c.in_ptr[v], i_hi = c.in_ptr[v + 1];
+    const u32 e_lo = c.row_ptr[v], e_hi = c.row_ptr[v + 1];
+    const bool serial_arr = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) != 0;
+    const u32 kb = k & c.NWmask;
+    if (mode == 2u) {                        // cycle-serial path
+        if (sw == 0) {
+            ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
+            issue_window(c, ctl, hp, g, t0, t1, cb, lane);
+            for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
+        }
+        set_sync(ws, set);
+    } else if (mode == 1u) {
+        const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
+        for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
+        set_sync(ws, set);
+    }
+    DIAG_CLK(4);
+
+    // ---- stage 3: merge into multi-feeder out-links of v (skipped when none received a line) ----
+    bool any_dirty = false;
+    for (u32 e = e_lo + lane; e < e_hi; e += 32) any_dirty |= c.dirty[e] != 0u;
+    any_dirty = __any_sync(FULL, any_dirty);
+    if (any_dirty) {
+        for (u32 e = e_lo + sw; e < e_hi; e += ws)
+            if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
+        set_sync(ws, set);
+        if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
+        u32 tmod3 = 0;
+        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+            const u32 i = ib + lane;
+            u32 e_b = e_l, n_b = n_l, lo_b = lo_l, fl_b = fl_l;
+            if (ib != i_lo) {
+                e_b = n_b = lo_b = fl_b = 0;
+                if (i < i_hi) {
+                    e_b = c.in_link[i]; n_b = ld_vol(&c.due_cnt[(size_t)e_b * c.NW + kb]);
+                    lo_b = c.pipe_head[e_b]; fl_b = serial_arr ? 0u : c.lflag[e_b];
+                }
+            }
+            // links that marked cells in pass 1 go over the same lines again, now with the FIFO positions known
+            const bool again = i < i_hi && (fl_b == 0u ? c.ndue[e_b] != 0u : (fl_b == ASTRA_LF_CELLS && c.tl_base[e_b] != 0u));
+            u32 nm = __ballot_sync(FULL, again);
+            while (nm) {
+                const u32 src = __ffs(nm) - 1; nm &= nm - 1;
+                const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
+                const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
+                const u32 first = (sw + ws - tmod3) % ws;
+                if (fl == 0u) { if (first == 0u) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); tmod3 = (tmod3 + 1) % ws; continue; }
+                for (u32 ch = first; ch * 64 < n; ch += ws) cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
+                tmod3 = (tmod3 + (n + 63) / 64) % ws;
+            }
+        }
+        set_sync(ws, set);
+    }
+    DIAG_CLK(5);
+
+    // ---- stage 4: link service of v's out-links (R9); the in-links' cursors move past the window ----
+    if (sw == ws - 1) {
+        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
+            const u32 i = ib + lane;
+            if (i >= i_hi) continue;
+            u32 e = e_l, n = n_l, fl = fl_l;
+            if (ib != i_lo) { e = c.in_link[i]; n = ld_vol(&c.due_cnt[(size_t)e * c.NW + kb]); fl = serial_arr ? 0u : c.lflag[e]; }
+            if (n == 0) continue;
+            c.due_cnt[(size_t)e * c.NW + kb] = 0;
+            if (fl != 0u) { c.pipe_head[e] += n; c.tl_base[e] = 0; }
+        }
+    }
+    for (u32 e = e_lo + sw; e < e_hi; e += ws) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
+    DIAG_CLK(6);
+}
+
+// The first 32 in-links of node v, one per lane, as stage 1 of node_window loads them.
+__device__ __forceinline__ void inlinks_first(const Ctx& __restrict__ c, u32 v, u32 k, u32 lane, u32& e_l, u32& n_l, u32& lo_l, u32& fl_l) {
+    const u32 i = c.in_ptr[v] + lane;
+    e_l = n_l = lo_l = fl_l = 0;
+    if (i < c.in_ptr[v + 1]) {
+        e_l = c.in_link[i];
+        n_l = ld_vol(&c.due_cnt[(size_t)e_l * c.NW + (k & c.NWmask)]);
+        lo_l = c.pipe_head[e_l];
+        fl_l = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e_l];
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // One lookahead window of one simulated node v, by the warp set that owns it (sw = warp index in the
 // set of ws warps).  Inside a window nothing a node does can reach another node (W <= min Leff), so
 // the stages of a node order only against each other: set barriers, no block barrier.
 // ---------------------------------------------------------------------------------------------
-#ifdef ASTRA_X_LOCKSTEP
-#define LOCKSTEP() do { if (lockstep) __syncthreads(); } while (0)
-#else
-#define LOCKSTEP() do { } while (0)
-#endif
-__device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
-                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, bool lockstep) {
+// Returns true when the node's budget-bound issue sweep and the rest of its window were deferred to the CTA (may_defer).
+__device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
+                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, bool may_defer) {
 #ifdef ASTRA_DIAG
     long long dck = clock64();
 #endif
@@ -1995,7 +2100,6 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     DIAG_CLK(0);
 
     // ---- stage 2: release + issue of GPU v (R10 - R13) ----
-    LOCKSTEP();
     u32 mode = 0;
     const u32 g = v;
     if (is_gpu) {
@@ -2004,119 +2108,62 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         DIAG_CLK(1);
         mode = c.gmode[g];
     }
-    LOCKSTEP();
     if (mode == 1u) {
         for (u32 wi = sw; wi < c.nwords; wi += ws) wf_sim(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
         set_sync(ws, set);
-    }
-    LOCKSTEP();
-    if (mode == 1u) {
         const u32 nh = c.nheavy[g];
         if (nh) {
             for (u32 j = sw; j < nh; j += ws) wf_heavy(c, ctl, hp, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
             set_sync(ws, set);
         }
         DIAG_CLK(2);
-    }
-    LOCKSTEP();
-    if (mode == 1u) {
         const bool bind = gpu_binds(c, g, wlen, lane);     // every warp checks: the same answer everywhere ...
         set_sync(ws, set);                                  // ... before anybody writes over the counts
+        const u32 deg = e_hi - e_lo;
         if (!bind) {                                        // the parts of the commit are dealt out
-            const u32 deg = e_hi - e_lo;
             if (sw == 0) gpu_finalize_counts(c, g, k, wlen, lane);
             if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) gpu_finalize_link(c, e_lo + x, wlen, lane);
             if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
-        } else if (sw == 0) {
-            // the budget binds: back to the window start, then exact grants
-            if (lane == 0) DIAG_ADD(6, 1);
-            wf_restore(c, g, lane);
-            if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) { if (lane == 0) c.gmode[g] = 2u; __syncwarp(); }
-            else {
-                const u32 deg = e_hi - e_lo;
-                for (u32 i = lane; i < c.W; i += 32) c.cnt[(size_t)g * c.W + i] = 0;
-                if (deg > 1) for (u32 i = lane; i < deg * c.W; i += 32) c.hist[(size_t)e_lo * c.W + i] = 0;
-                __syncwarp();
-                for (u32 wi = 0; wi < c.nwords; wi++) wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
-                gpu_finalize(c, g, k, wlen, lane);
+        } else if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) {      // testing: back to the window start, cycle-serial path
+            for (u32 wi = sw; wi < c.nwords; wi += ws) wf_restore_word(c, g, wi, lane);
+            if (sw == 0 && lane == 0) c.gmode[g] = 2u;
+        } else {
+            // The budget binds: back to the window start, then the exact grants word by word (wf_priority_word).
+            // The sweep is ordered, but every warp that takes part loads and sorts its words' inputs on its own:
+            // the warps of the set -- or, for a one-warp set, all warps of the CTA after the window's barrier
+            // (bb_sweep); the rest of this node's window then follows (node_tail).
+            if (sw == 0 && lane == 0) DIAG_ADD(6, 1);
+            for (u32 i = sw * 32 + lane; i < c.W; i += ws * 32) c.cnt[(size_t)g * c.W + i] = 0;
+            if (deg > 1) for (u32 i = sw * 32 + lane; i < deg * c.W; i += ws * 32) c.hist[(size_t)e_lo * c.W + i] = 0;
+            if (sw == 0 && lane == 0) c.turn[g] = 0u;
+            if (may_defer) {
+                if (lane == 0) ctl.bbq[atomicAdd(&ctl.nbb, 1u)] = g;
+                return true;
             }
+            set_sync(ws, set);
+            for (u32 wi = sw; wi < c.nwords; wi += ws) {
+                wf_restore_word(c, g, wi, lane);
+                wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, ws > 1 ? &c.turn[g] : nullptr, lane);
+            }
+            set_sync(ws, set);
+            if (sw == 0) gpu_finalize(c, g, k, wlen, lane);
         }
         set_sync(ws, set);
         mode = c.gmode[g];
-    }
-    LOCKSTEP();
-    if (mode == 2u) {                        // cycle-serial path
-        if (sw == 0) {
-            ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
-            issue_window(c, ctl, hp, g, t0, t1, cb, lane);
-            for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
-        }
-        set_sync(ws, set);
-        DIAG_CLK(3);
-    } else if (mode == 1u) {
-        DIAG_CLK(3);
-        const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
-        for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
-        set_sync(ws, set);
-        DIAG_CLK(4);
     } else if (!is_gpu && any_fwd) set_sync(ws, set);
-    LOCKSTEP();
+    DIAG_CLK(3);
+    node_tail(c, ctl, hp, v, k, t0, t1, cb, scr, lane, sw, ws, set, diag_lane, mode, e_l, n_l, lo_l, fl_l);
+    return false;
+}
 
-    // ---- stage 3: merge into multi-feeder out-links of v (skipped when none received a line) ----
-    bool any_dirty = false;
-    for (u32 e = e_lo + lane; e < e_hi; e += 32) any_dirty |= c.dirty[e] != 0u;
-    any_dirty = __any_sync(FULL, any_dirty);
-    if (any_dirty) {
-        for (u32 e = e_lo + sw; e < e_hi; e += ws)
-            if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
-        set_sync(ws, set);
+// A budget-bound GPU-window of a one-warp node, swept by all warps of the CTA after the window's barrier: team
+// member r of m takes words r, r + m, ... (restore, load, sort, then the ordered sweep); the last word's warp commits.
+__device__ ASTRA_COLD void bb_sweep(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 r, u32 m, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
+    for (u32 wi = r; wi < c.nwords; wi += m) {
+        wf_restore_word(c, g, wi, lane);
+        wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, &c.turn[g], lane);
+        if (wi == c.nwords - 1) gpu_finalize(c, g, k, t1 - t0, lane);
     }
-    LOCKSTEP();
-    if (any_dirty) {
-        if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
-        u32 tmod3 = 0;
-        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
-            const u32 i = ib + lane;
-            u32 e_b = e_l, n_b = n_l, lo_b = lo_l, fl_b = fl_l;
-            if (ib != i_lo) {
-                e_b = n_b = lo_b = fl_b = 0;
-                if (i < i_hi) {
-                    e_b = c.in_link[i]; n_b = ld_vol(&c.due_cnt[(size_t)e_b * c.NW + kb]);
-                    lo_b = c.pipe_head[e_b]; fl_b = serial_arr ? 0u : c.lflag[e_b];
-                }
-            }
-            // links that marked cells in pass 1 go over the same lines again, now with the FIFO positions known
-            const bool again = i < i_hi && (fl_b == 0u ? c.ndue[e_b] != 0u : (fl_b == ASTRA_LF_CELLS && c.tl_base[e_b] != 0u));
-            u32 nm = __ballot_sync(FULL, again);
-            while (nm) {
-                const u32 src = __ffs(nm) - 1; nm &= nm - 1;
-                const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
-                const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
-                const u32 first = (sw + ws - tmod3) % ws;
-                if (fl == 0u) { if (first == 0u) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); tmod3 = (tmod3 + 1) % ws; continue; }
-                for (u32 ch = first; ch * 64 < n; ch += ws) cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
-                tmod3 = (tmod3 + (n + 63) / 64) % ws;
-            }
-        }
-        set_sync(ws, set);
-    }
-    DIAG_CLK(5);
-    LOCKSTEP();
-
-    // ---- stage 4: link service of v's out-links (R9); the in-links' cursors move past the window ----
-    if (sw == ws - 1) {
-        for (u32 ib = i_lo; ib < i_hi; ib += 32) {
-            const u32 i = ib + lane;
-            if (i >= i_hi) continue;
-            u32 e = e_l, n = n_l, fl = fl_l;
-            if (ib != i_lo) { e = c.in_link[i]; n = ld_vol(&c.due_cnt[(size_t)e * c.NW + kb]); fl = serial_arr ? 0u : c.lflag[e]; }
-            if (n == 0) continue;
-            c.due_cnt[(size_t)e * c.NW + kb] = 0;
-            if (fl != 0u) { c.pipe_head[e] += n; c.tl_base[e] = 0; }
-        }
-    }
-    for (u32 e = e_lo + sw; e < e_hi; e += ws) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
-    DIAG_CLK(6);
 }
 
 __device__ __forceinline__ void
@@ -2179,6 +2226,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
             ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
+            ctl.nbb = 0u;
             ctl.g_hint = ASTRA_T_INF; ctl.g_acked = 0; ctl.g_err = 0; ctl.g_completion = 0;
 #ifdef ASTRA_DIAG
             for (int i = 0; i < 16; i++) ctl.clk[i] = 0;
@@ -2232,7 +2280,8 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const u32 wset = nwarps / nsets;                   // warps per set (left-over warps idle through the window)
         const u32 set = warp / wset, sw = warp % wset;
         const bool in_set = set < nsets;
-        const bool lockstep = n_nodes == nwarps;            // experiment: every warp steps exactly one node per window
+        // one-warp nodes, at most one per warp: a budget-bound sweep is handed to the whole CTA (bb_sweep)
+        const bool may_defer = wset == 1u && n_nodes <= nwarps && nwarps > 1u;
 
         // ---- window loop ----
         u32 k = 0, seq = 0;
@@ -2248,16 +2297,36 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             const u32 cb = t0 % c.NC;
             u32* const hp = &ctl.hint[seq % 3];
             busy += t1 - t0;
+            bool deferred = false;
             if (in_set)
                 for (u32 j = set; j < n_nodes; j += nsets)
-                    node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0, lockstep);
+                    deferred = node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0, may_defer);
+            bool synced = false;                               // the CTA has met and nothing was done since
+            if (may_defer) {
+                __syncthreads();
+                const u32 nbb = ctl.nbb;                       // the same value in every thread
+                synced = nbb == 0u;
+                if (nbb) {
+                    // warp w joins the team of GPU bbq[w % nbb] as member w / nbb
+                    const u32 gi = warp % nbb;
+                    bb_sweep(c, ctl, hp, ctl.bbq[gi], warp / nbb, (nwarps - gi + nbb - 1u) / nbb, k, t0, t1, scr, lane);
+                    __syncthreads();
+                    if (tid == 0) ctl.nbb = 0u;
+                    if (deferred) {
+                        const u32 v = c.v_lo + set;
+                        u32 e_l, n_l, lo_l, fl_l;
+                        inlinks_first(c, v, k, lane, e_l, n_l, lo_l, fl_l);
+                        node_tail(c, ctl, hp, v, k, t0, t1, cb, scr, lane, 0u, 1u, set, lane == 0, c.gmode[v], e_l, n_l, lo_l, fl_l);
+                    }
+                }
+            }
             // ---- stage 5: next non-idle window (A7), one block barrier per window ----
 #ifdef ASTRA_DIAG
             dck = clock64();
 #endif
             u32 hint, acked_total, err;
             if (group > 1) {
-                __syncthreads();
+                if (!synced) __syncthreads();
                 if (tid == 0) {
                     atomicMin(&gc->hint[seq % 3], *hp);
                     if (ctl.acked) { atomicAdd(&gc->acked, ctl.acked); atomicMax(&gc->completion, ctl.completion); ctl.acked = 0; }
@@ -2276,7 +2345,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
                 __syncthreads();
                 hint = ctl.g_hint; acked_total = ctl.g_acked; err = ctl.g_err;
             } else {
-                __syncthreads();
+                if (!synced) __syncthreads();
                 hint = *hp; acked_total = ctl.acked; err = ctl.err;
                 // slot (seq + 2) % 3 was last read before this barrier and is next written after the next one
                 if (tid == 0) ctl.hint[(seq + 2) % 3] = ASTRA_T_INF;

@@ -24,7 +24,11 @@ typedef uint64_t u64;
 #define ASTRA_NOTLOADED 0xffffffffu
 #define ASTRA_TS_NONE32 0xffffffffu
 #define ASTRA_NONE32 0xffffffffu
-#define ASTRA_WMAX_LOG2 9                 // lookahead window capped at 512 cycles
+#ifndef ASTRA_WMAX
+#define ASTRA_WMAX 512u                   // cap of the lookahead window in cycles (< 1024: 10-bit cycle fields in the flit)
+#endif
+#define ASTRA_HOT_BUDGET_SINGLE (48u << 10)  // bytes of shared memory for hot arrays, batches of one-CTA points (the rest of the SM's 256 KB is L1)
+#define ASTRA_HOT_BUDGET_GROUPS (64u << 10)  // ... batches with CTA groups
 #define ASTRA_NW_MAX 256                  // ack window bins per GPU
 #define ASTRA_ACK_LIST_CAP 4096u           // ack discovery list entries per (GPU, window bin); beyond: bitmap scan
 #define ASTRA_HEAVY_MIN 8u                // possible issues in a window from which a wavefront gets a warp of its own
@@ -55,7 +59,7 @@ typedef uint64_t u64;
 #define ASTRA_WS_ARRAYS(X) \
     X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
     X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(due_cnt, u32, 0) X(tl_lo, u32, 3) X(tl_n, u32, 3) X(tl_base, u32, 3) X(tbase, u32, 3) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
-    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(turn, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(cu_out, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \

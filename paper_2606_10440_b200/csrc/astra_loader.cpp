@@ -159,7 +159,7 @@ double astra_point_cost(const HostTopo& t, const HostColl& c, u64 flags) {
     for (u32 e = 0; e < E; e++) cycles = std::max(cycles, (double)via[e] * 256.0 / t.bw[e]);
     cycles += 4.0 * alpha_max;
     u32 W = 1;
-    if (!(flags & ASTRA_FLAG_WINDOW_1)) { W = std::max<u32>(1, std::min<u32>(t.min_leff, 1u << ASTRA_WMAX_LOG2)); if (W >= 64) W &= ~63u; }
+    if (!(flags & ASTRA_FLAG_WINDOW_1)) { W = std::max<u32>(1, std::min<u32>(t.min_leff, (u32)ASTRA_WMAX)); if (W >= 64) W &= ~63u; }
     // measured: a window costs a CTA about 20 k clocks plus 3.5 k per GPU and per link it steps; events are cheap
     return cycles / W * (20000.0 + 3500.0 * (t.G + E)) + events * 10.0;
 }
@@ -201,7 +201,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     // lookahead window: min Leff (any value, not only powers of two), capped
     u32 W = 1;
     if (!(opt.flags & ASTRA_FLAG_WINDOW_1)) {
-        W = std::max<u32>(1, std::min<u32>(t.min_leff, 1u << ASTRA_WMAX_LOG2));
+        W = std::max<u32>(1, std::min<u32>(t.min_leff, (u32)ASTRA_WMAX));
         if (W >= 64) W &= ~63u;                 // whole 32-entry chunks per link and window at the usual bandwidths
     }
     P.Wcyc = W;
@@ -438,7 +438,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_tbase] = 4ull * (E + 1);
     for (u32 a : {ASTRA_A_pcnt, ASTRA_A_ev_cnt, ASTRA_A_ack_n, ASTRA_A_inj_n}) ab[a] = 4ull * G;
     ab[ASTRA_A_want] = ab[ASTRA_A_freeb] = ab[ASTRA_A_amask] = 4ull * G * P.nwords;
-    ab[ASTRA_A_gmode] = ab[ASTRA_A_nheavy] = 4ull * G;
+    ab[ASTRA_A_gmode] = ab[ASTRA_A_nheavy] = ab[ASTRA_A_turn] = 4ull * G;
     ab[ASTRA_A_cnt] = 4ull * G * W;
     ab[ASTRA_A_undo_want] = ab[ASTRA_A_undo_freeb] = 4ull * G * P.nwords;
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
