@@ -1037,9 +1037,14 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
         u32* cnt = c.cnt + (size_t)g * c.W;
         for (u32 i = lane; i < c.W; i += 32) cnt[i] = 0;
         if (lane == 0) c.nheavy[g] = 0;
-        if (deg > 1) {
-            u32* h = c.hist + (size_t)e0 * c.W;
-            for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0;
+        if (deg > 1) {                                          // per-cycle issue counts of the direct out-links
+            u32 dm = deg > 32 ? 0u : c.gdirect[g];
+            if (deg > 32) { u32* h = c.hist + (size_t)e0 * c.W; for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0; }
+            while (dm) {
+                const u32 x = __ffs(dm) - 1; dm &= dm - 1;
+                u32* h = c.hist + (size_t)(e0 + x) * c.W;
+                for (u32 i = lane; i < c.W; i += 32) h[i] = 0;
+            }
         }
     }
     if (lane == 0) c.gmode[g] = mode;
@@ -1119,6 +1124,8 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
         u32 nq = na ? aq[0] : 0xffffffffu;                       // earliest ack not applied yet (packed)
         const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
         const u32 wlen = t1 - t0;
+        const u32 gdir = c.gdirect[g];                          // out-links that need their per-cycle issue counts
+        bool hx = false;
         u32 tt = 0, s = 0, ox = 0, last_issue = 0xffffffffu;    // tt: candidate cycle relative to t0
         u32 eq0 = 0, eq1 = 0, eq2 = 0, eq3 = 0, nb = 0;             // buffered issues: cycle << 6 | slot
         bool have_s = false;
@@ -1137,7 +1144,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
                 if (!got) break;
                 have_s = false;
             }
-            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; have_s = true; }
+            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; hx = deg > 1 && ((gdir >> (ox & 31u)) & 1u); have_s = true; }
             if (busy == fullmask) {                             // all K slots in flight: wait for the next ack
                 if (ai >= na) break;
                 tt = max(tt, nq >> 6);
@@ -1161,7 +1168,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
                 for (int q = 0; q < 4; q++) if ((u32)q < nb) {
                     const u32 t2 = bb[q] >> 6;
                     if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
-                    if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
+                    if (hx) atomicAdd(&h[ox * W + t2], 1u);
                 }
                 nb = 0;
             }
@@ -1175,7 +1182,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
             for (int q = 0; q < 4; q++) if ((u32)q < nb) {
                 const u32 t2 = bb[q] >> 6;
                 if (pp[q] < H) evb[(size_t)t2 * H + pp[q]] = (u64)s | ((u64)wf << 20) | ((u64)(bb[q] & 63u) << 32) | ((u64)(t2 + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
-                if (deg > 1) atomicAdd(&h[ox * W + t2], 1u);
+                if (hx) atomicAdd(&h[ox * W + t2], 1u);
             }
         }
         for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));   // acks later in the window than the last look
@@ -1283,6 +1290,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
         }
         const u32 s = cul[cur];
         const u32 ox = c.first_link[s] - e0;
+        const bool hx = deg > 1 && ((c.gdirect[g] >> (ox & 31u)) & 1u);
         while (rem > 0) {
             const u32 i = idx + lane;
             const u32 want_n = min(32u, rem);
@@ -1298,7 +1306,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
                 if (slot < 32) im_lo |= 1u << slot; else im_hi |= 1u << (slot - 32);
                 const u32 p = atomicAdd(&cnt[x], 1u);
                 if (p < H) evb[(size_t)x * H + p] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(x + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
-                if (deg > 1) atomicAdd(&h[ox * W + x], 1u);
+                if (hx) atomicAdd(&h[ox * W + x], 1u);
             }
             if (nv) {
                 last_issue = __shfl_sync(FULL, x, nv - 1);
@@ -1400,7 +1408,8 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
     }
     u32 nq = na ? aq[0] : 0xffffffffu;
     u32 s = 0, ox = 0, last_issue = 0xffffffffu;
-    bool have_s = false;
+    bool have_s = false, hx = false;
+    const u32 gdir = c.gdirect[g];
     u32 T = 0;
     if (turn) turn_wait(turn, wi, lane);                       // the grants of all lower words are in occ[] now
     for (;;) {
@@ -1442,11 +1451,11 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
         const u32 rank = o + __popc(rm & lanemask_lt());
         const bool granted = ready && rank < H;
         if (granted) {
-            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; have_s = true; }
+            if (!have_s) { s = cul[cur]; ox = c.first_link[s] - e0; hx = deg > 1 && ((gdir >> (ox & 31u)) & 1u); have_s = true; }
             const u32 slot = __ffsll((long long)~busy) - 1;
             busy |= 1ull << slot;
             evb[(size_t)T * H + rank] = (u64)s | ((u64)wf << 20) | ((u64)slot << 32) | ((u64)(T + 1) << ASTRA_FLIT_TIME_SHIFT) | ((u64)ox << 48);
-            if (deg > 1) atomicAdd(&h[ox * W + T], 1u);
+            if (hx) atomicAdd(&h[ox * W + T], 1u);
             last_issue = T;
             if (--rem == 0) { cur++; rem = ASTRA_NOTLOADED; }
         }
@@ -1549,7 +1558,7 @@ __device__ void gpu_finalize_acks(const Ctx& __restrict__ c, u32 g, u32 k, u32 l
 __device__ void gpu_finalize(const Ctx& __restrict__ c, u32 g, u32 k, u32 wlen, u32 lane) {   // all parts on one warp
     gpu_finalize_counts(c, g, k, wlen, lane);
     const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
-    if (deg > 1) for (u32 x = 0; x < deg; x++) gpu_finalize_link(c, e0 + x, wlen, lane);
+    if (deg > 1) for (u32 x = 0; x < deg; x++) if (deg > 32 || ((c.gdirect[g] >> x) & 1u)) gpu_finalize_link(c, e0 + x, wlen, lane);
     gpu_finalize_acks(c, g, k, lane);
     __syncwarp();
 }
@@ -2122,7 +2131,7 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         const u32 deg = e_hi - e_lo;
         if (!bind) {                                        // the parts of the commit are dealt out
             if (sw == 0) gpu_finalize_counts(c, g, k, wlen, lane);
-            if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) gpu_finalize_link(c, e_lo + x, wlen, lane);
+            if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) if (deg > 32 || ((c.gdirect[g] >> x) & 1u)) gpu_finalize_link(c, e_lo + x, wlen, lane);
             if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
         } else if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) {      // testing: back to the window start, cycle-serial path
             for (u32 wi = sw; wi < c.nwords; wi += ws) wf_restore_word(c, g, wi, lane);
@@ -2134,7 +2143,8 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             // (bb_sweep); the rest of this node's window then follows (node_tail).
             if (sw == 0 && lane == 0) DIAG_ADD(6, 1);
             for (u32 i = sw * 32 + lane; i < c.W; i += ws * 32) c.cnt[(size_t)g * c.W + i] = 0;
-            if (deg > 1) for (u32 i = sw * 32 + lane; i < deg * c.W; i += ws * 32) c.hist[(size_t)e_lo * c.W + i] = 0;
+            if (deg > 1) for (u32 x = 0; x < deg; x++)
+                if (deg > 32 || ((c.gdirect[g] >> x) & 1u)) for (u32 i = sw * 32 + lane; i < c.W; i += ws * 32) c.hist[(size_t)(e_lo + x) * c.W + i] = 0;
             if (sw == 0 && lane == 0) c.turn[g] = 0u;
             if (may_defer) {
                 if (lane == 0) ctl.bbq[atomicAdd(&ctl.nbb, 1u)] = g;

@@ -404,6 +404,15 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
             if ((c.succ[i] >> 30) == ASTRA_DEP_ISSUED) gflag[c.owner[s]] |= ASTRA_GF_ISSUED_DEPS;
     if (g.mode & 3u) for (u32 q = 0; q < G; q++) gflag[q] |= ASTRA_GF_SERIAL;      // per-CU readings (R12', R2')
 
+    // gdirect[g]: bit x set when out-link x of GPU g is single-feeder (the GPU appends its issues to it directly and
+    // needs the per-cycle issue counts of that link); all ones for a GPU with more than 32 out-links
+    std::vector<u32> gdirect(G, 0);
+    for (u32 q = 0; q < G; q++) {
+        const u32 e0 = t.row_ptr[q], deg = t.row_ptr[q + 1] - e0;
+        if (deg > 32) { gdirect[q] = ~0u; continue; }
+        for (u32 x = 0; x < deg; x++) if (!multi[e0 + x]) gdirect[q] |= 1u << x;
+    }
+
     // constant tables
     u64* co = P.c_off;
     co[ASTRA_C_in_ptr] = topo_off[0]; co[ASTRA_C_in_link] = topo_off[1]; co[ASTRA_C_head] = topo_off[2];
@@ -426,6 +435,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
     co[ASTRA_C_part] = blob.add(part);
     co[ASTRA_C_gflag] = blob.add(gflag);
+    co[ASTRA_C_gdirect] = blob.add(gdirect);
     co[ASTRA_C_lflag] = blob.add(lflag); co[ASTRA_C_lfwd] = blob.add(lfwd);
     co[ASTRA_C_lscr_off] = blob.add(lscr_off);
 
