@@ -39,11 +39,7 @@
 #include <cuda_runtime.h>
 
 #define FULL 0xffffffffu
-#ifdef ASTRA_X_COLD
-#define ASTRA_COLD __noinline__
-#else
-#define ASTRA_COLD
-#endif
+#define ASTRA_COLD            // measured: real calls (__noinline__) for the rarely taken paths cost 3 % on every config
 #define SCR_WORDS 1088u   // per-warp scratch words: 32 lanes x 64 16-bit ack keys (wf_sim, wf_priority_word), 513 counters (ack_sort), 512 (ack_chunk)
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
@@ -67,7 +63,6 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 hint[3];        // min over everything pending of its next event time; slot seq % 3 is the window's (A7)
     u32 g_hint, g_acked, g_err, g_completion;   // group mode: the group-wide values after the window's group barrier
     u32 abort;          // a group barrier timed out somewhere: leave the kernel
-    u32 nbb, bbq[32];   // one-warp nodes whose budget-bound sweep waits for the CTA this window (bb_sweep)
 #ifdef ASTRA_DIAG
     u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows, [7] clocks on that path, [8] windows with such a GPU
     u64 sclk[16][8];    // per warp set (clocks of its first warp, summed over its nodes and windows): 0 arrivals+acks,
@@ -107,10 +102,14 @@ __device__ __forceinline__ int warp_incl_max(int v, u32 lane) {
     return v;
 }
 
-// Mark slot `slot` of the cell (out-link o at node v, cycle t0 + d) occupied (R7/R8).
+// Mark slot `slot` of the cell (out-link o at node v, cycle t0 + d) occupied (R7/R8).  A multi-feeder link that the
+// loader expects to see lines in few cycles of a window (nz_off set) also keeps one bit per cycle, "this cell is not
+// empty": its prefix pass and its clean-up look only at the marked cells instead of sweeping all of them.
 __device__ __forceinline__ void cell_set(const Ctx& __restrict__ c, u32 o, u32 v, u32 cb, u32 d, u32 slot) {
     u32 ci = cb + d; if (ci >= c.NC) ci -= c.NC;
     atomicOr(&c.masks[c.mask_off[o] + ci * c.nd_mw[v] + (slot >> 5)], 1u << (slot & 31));
+    const u32 nzo = c.nz_off[o];
+    if (nzo != ASTRA_NONE32) atomicOr(&c.nz[nzo + (d >> 5)], 1u << (d & 31));
     c.dirty[o] = 1u;
 }
 // FIFO position, relative to the tail at the window start, of the line in slot `slot` of that cell.
@@ -120,6 +119,7 @@ __device__ __forceinline__ u32 cell_pos(const Ctx& __restrict__ c, u32 o, u32 v,
     const u32* words = c.masks + c.mask_off[o] + ci * mw;
     u32 r = c.pre[c.pre_off[o] + d];
     const u32 sw = slot >> 5;
+    #pragma unroll 1
     for (u32 w = 0; w < sw; w++) r += __popc(words[w]);
     return r + __popc(words[sw] & ((1u << (slot & 31)) - 1u));
 }
@@ -142,6 +142,7 @@ __device__ void arrivals_link(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 
     if (PASS == 1 && lane == 0 && hi - lo > rmask + 1) atomicOr(&ctl.err, 1u);
     u32 carry_d = 0xffffffffu, carry_cnt = 0, idx = lo, ndue = 0, hint = ASTRA_T_INF;
     bool any_p3 = false;
+    #pragma unroll 1
     for (;;) {
         const u32 ii = idx + lane;
         const bool valid = (int32_t)(hi - ii) > 0;
@@ -247,6 +248,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
     const u32 bin = k & c.NWmask;
     const u32 n = c.ack_n[g];
     if (n == 0) return;
+    #pragma unroll 1
     for (u32 i = lane; i <= wlen; i += 32) scnt[i] = 0;
     __syncwarp();
     u32* bm = c.bitmap + (size_t)(g * c.NW + bin) * c.bmwords;
@@ -254,6 +256,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
     u64* tmp = c.ack_tmp + (size_t)g * c.slots;
     u64* srt = c.ack_sorted + (size_t)g * c.slots;
     u32 total = 0;
+    #pragma unroll 1
     for (u32 wb = 0; wb < c.bmwords; wb += 32) {
         const u32 wi = wb + lane;
         u32 w = (wi < c.bmwords) ? __ldcg(&bm[wi]) : 0;
@@ -262,6 +265,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
         const u32 incl = warp_incl_scan(cnt, lane);
         u32 pos = total + incl - cnt;
         total += __shfl_sync(FULL, incl, 31);
+        #pragma unroll 1
         while (w) {
             const u32 b = __ffs(w) - 1; w &= w - 1;
             const u32 idx = wi * 32 + b;
@@ -275,6 +279,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
     }
     __syncwarp();
     u32 carry = 0;
+    #pragma unroll 1
     for (u32 b = 0; b < wlen; b += 32) {
         const u32 i = b + lane;
         const u32 vv = (i < wlen) ? scnt[i] : 0;
@@ -283,6 +288,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
         carry += __shfl_sync(FULL, incl, 31);
     }
     __syncwarp();
+    #pragma unroll 1
     for (u32 b = 0; b < total; b += 32) {
         const u32 i = b + lane;
         if (i < total) {
@@ -306,6 +312,7 @@ __device__ ASTRA_COLD void ack_sort(const Ctx& __restrict__ c, Ctl& ctl, u32 g, 
 // ---------------------------------------------------------------------------------------------
 __device__ void stage1_setup_gpu(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 k, u32 lane) {
     u32 best = ASTRA_T_INF;                                     // earliest later window with acks pending (A7)
+    #pragma unroll 1
     for (u32 j = 1 + lane; j < c.NW; j += 32)
         if (ld_vol(&c.bin_cnt[g * c.NW + ((k + j) & c.NWmask)])) { best = j; break; }
     best = __reduce_min_sync(FULL, best);
@@ -325,6 +332,7 @@ __device__ __forceinline__ void link_inflight_hint(const Ctx& __restrict__ c, Ct
     const u32* dcb = &c.due_cnt[(size_t)e * c.NW];
     const u32 span = min(c.NW - 1, c.leff[e] / c.W + 2);
     u32 best = ASTRA_T_INF;
+    #pragma unroll 1
     for (u32 j = span; j >= 1; j--)
         if (ld_vol(&dcb[(k + j) & c.NWmask])) best = j;
     if (best != ASTRA_T_INF) {
@@ -408,9 +416,11 @@ __device__ ASTRA_COLD void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g,
     u32 tmax = 0;
     // per-lane caches: consecutive acks of a lane mostly belong to one step and one amask word
     u32 cs = 0xffffffffu, cc = 0, cm = 0, aw = 0xffffffffu, ab = 0;
+    #pragma unroll 1
     for (u32 base = 0; base < total; base += CAP) {
         {
             u32 pos = excl, ww = w;
+            #pragma unroll 1
             while (ww) {
                 const u32 b = __ffs(ww) - 1; ww &= ww - 1;
                 if (pos >= base && pos < base + CAP) scr[pos - base] = (lane << 5) | b;
@@ -419,6 +429,7 @@ __device__ ASTRA_COLD void ack_chunk(const Ctx& __restrict__ c, Ctl& ctl, u32 g,
         }
         __syncwarp();
         const u32 nn = min(CAP, total - base);
+        #pragma unroll 1
         for (u32 j0 = 0; j0 < nn; j0 += 128) {
             u32 idx[4]; u64 rc[4];
 #pragma unroll
@@ -621,6 +632,7 @@ __device__ void cells_place_chunk(const Ctx& __restrict__ c, u32 e, u32 lo, u32 
         const u32* words = c.masks + moff[h] + ci * mw;
         u32 r = pb[h];
         const u32 swd = slot >> 5;
+        #pragma unroll 1
         for (u32 w = 0; w < swd; w++) r += __popc(words[w]);
         r += __popc(words[swd] & ((1u << (slot & 31)) - 1u));
         const u32 pos = tl[h] + r;
@@ -649,6 +661,7 @@ __device__ void forward_chunk(const Ctx& __restrict__ c, u32 e, u32 lo, u32 n, u
 // its dependencies' times and joins g's pending-release list.  Whole warp, warp-uniform p.
 __device__ __forceinline__ void on_event(const Ctx& __restrict__ c, u32 g, u32 p, u32 kind, u32 time, u32 lane) {
     const u32 lo = c.succ_ptr[p], hi = c.succ_ptr[p + 1];
+    #pragma unroll 1
     for (u32 b = lo; b < hi; b += 32) {
         const u32 i = b + lane; bool ready = false; u32 s2 = 0;
         if (i < hi) {
@@ -678,6 +691,7 @@ __device__ __forceinline__ void on_event(const Ctx& __restrict__ c, u32 g, u32 p
 __device__ __forceinline__ bool wf_advance(const Ctx& __restrict__ c, u32 g, u32 wf, u32& cur, u32& rem, u32 t) {
     const u32 end = c.cul_ptr[g * c.C + wf / c.Wv + 1];
     rem = ASTRA_NOTLOADED;
+    #pragma unroll 1
     while (cur < end) {
         const u32 s = c.cul[cur];
         if (c.t_release[s] > t) return false;           // NONE (0xffffffff) or a later cycle
@@ -719,23 +733,27 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
     u32 t_rel_next = ASTRA_T_INF;
     {
         const u32 np = c.pcnt[g];
+        #pragma unroll 1
         for (u32 i = lane; i < np; i += 32) t_rel_next = min(t_rel_next, c.t_release[plist[i]]);
         t_rel_next = __reduce_min_sync(FULL, t_rel_next);
     }
     bool more;
     {
         u32 any = 0;
+        #pragma unroll 1
         for (u32 wi = lane; wi < c.nwords; wi += 32) any |= want[wi] & freeb[wi];
         more = __ballot_sync(FULL, any != 0) != 0;
     }
     u32 t = min(min(t_ack_next, t_rel_next), more ? t0 : ASTRA_T_INF);
     if (t < t0) t = t0;
 
+    #pragma unroll 1
     while (t < t1) {
         more = false;
         // ---- slot return: acks due at t (R7 A3) ----
         if (t_ack_next == t) {
             const u32 cyc = t - t0;
+            #pragma unroll 1
             for (;;) {
                 const u32 j0 = ack_pos - abase;
                 const bool now = lane >= j0 && abase + lane < ack_n && (abuf >> 18) == cyc;
@@ -780,6 +798,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
         if (t_rel_next == t) {
             const u32 np = c.pcnt[g];
             u32 keep = 0, tn = ASTRA_T_INF;
+            #pragma unroll 1
             for (u32 b = 0; b < np; b += 32) {
                 const u32 i = b + lane;
                 const u32 s = (i < np) ? plist[i] : 0;
@@ -791,10 +810,12 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
                 __syncwarp();
                 if (later) { plist[keep + __popc(laterm & lanemask_lt())] = s; tn = min(tn, tr); }
                 keep += __popc(laterm);
+                #pragma unroll 1
                 while (nowm) {
                     const u32 src = __ffs(nowm) - 1; nowm &= nowm - 1;
                     const u32 sr = __shfl_sync(FULL, s, src);
                     const u32 lo = c.cu_lo[sr] * c.Wv, hi = lo + c.cu_n[sr] * c.Wv;
+                    #pragma unroll 1
                     for (u32 wb = lo & ~31u; wb < hi; wb += 32) {
                         const u32 wf = wb + lane;
                         bool setw = false;
@@ -825,6 +846,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
             // per-CU readings: one CU per lane.  Of its ready wavefronts a CU may dispatch the lowest one (R12') or as
             // many as its pool has room for (R2'); then the first H of all of them in ascending wavefront id (R12).
             const u32 Wv = c.Wv;
+            #pragma unroll 1
             for (u32 cb0 = 0; cb0 < c.C; cb0 += 32) {
                 const u32 cu = cb0 + lane;
                 u32 keep = 0, lo = 0;
@@ -838,6 +860,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
                     u32 room = Wv;
                     if (pcu & 1u) room = 1u;
                     if (pcu & 2u) room = min(room, c.K - c.cu_out[(size_t)g * c.C + cu]);
+                    #pragma unroll 1
                     for (u32 q = 0; q < room && bits; q++) { const u32 low = bits & (0u - bits); keep |= low; bits ^= low; }
                     more_ready = bits != 0u;
                 }
@@ -849,6 +872,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
                 if (budget == 0) { left_over = true; break; }
                 const u32 excl = incl - cntc;
                 const u32 take = excl >= budget ? 0 : min(cntc, budget - excl);
+                #pragma unroll 1
                 for (u32 i = 0; i < take; i++) {
                     const u32 b = __ffs(keep) - 1; keep &= keep - 1;
                     sel[nsel + excl + i] = lo + b;
@@ -858,6 +882,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
                 nsel += got; budget -= got;
             }
         } else
+        #pragma unroll 1
         for (u32 wb = 0; wb < c.nwords; wb += 32) {
             const u32 wi = wb + lane;
             u32 r = (wi < c.nwords) ? (want[wi] & freeb[wi]) : 0;
@@ -868,6 +893,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
             if (budget == 0) { left_over = true; break; }
             const u32 excl = incl - cnt;
             const u32 take = excl >= budget ? 0 : min(cnt, budget - excl);
+            #pragma unroll 1
             for (u32 i = 0; i < take; i++) {
                 const u32 b = __ffs(r) - 1; r &= r - 1;
                 sel[nsel + excl + i] = wi * 32 + b;
@@ -878,6 +904,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
         }
         __syncwarp();
         const u32 d = t + 1 - t0;     // injected at t + 1 into the first-hop FIFO, after that cycle's transit lines (R7 A2)
+        #pragma unroll 1
         for (u32 b = 0; b < nsel; b += 32) {
             const u32 j = b + lane; const bool act = j < nsel;
             u32 wf = 0, s = 0, o = 0, moff = 0; bool full = false, keepw = true;
@@ -951,6 +978,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
                 }
             }
             u32 cm = __ballot_sync(FULL, completed);
+            #pragma unroll 1
             while (cm) {
                 const u32 src = __ffs(cm) - 1; cm &= cm - 1;
                 const u32 p = __shfl_sync(FULL, s, src);
@@ -965,6 +993,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
         if (t_rel_next == ASTRA_T_INF) {
             const u32 np = c.pcnt[g];
             u32 tn = ASTRA_T_INF;
+            #pragma unroll 1
             for (u32 i = lane; i < np; i += 32) tn = min(tn, c.t_release[plist[i]]);
             t_rel_next = __reduce_min_sync(FULL, tn);
         }
@@ -996,6 +1025,7 @@ __device__ ASTRA_COLD void issue_window(const Ctx& __restrict__ c, Ctl& ctl, u32
 __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, u32 t1, u32 lane) {
     {
         const u32 nev = c.ev_cnt[g];
+        #pragma unroll 1
         for (u32 j = 0; j < nev; j++) {
             const u32 ek = c.ev_list[c.ev_off[g] + j];
             const u32 p = ek & 0xfffffu, kind = ek >> 30;
@@ -1011,10 +1041,12 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
     // wavefronts of the CU range of every step released inside this window
     const u32 np = c.pcnt[g];
     const u32* plist = c.plist + c.rel_off[g];
+    #pragma unroll 1
     for (u32 i = 0; i < np; i++) {
         const u32 s = plist[i];
         if (c.t_release[s] >= t1) continue;
         const u32 lo = c.cu_lo[s] * c.Wv, hi = lo + c.cu_n[s] * c.Wv;
+        #pragma unroll 1
         for (u32 wi = (lo >> 5) + lane; wi <= ((hi - 1) >> 5); wi += 32) {
             const u32 b0 = wi * 32;
             u32 m = ~0u;
@@ -1025,6 +1057,7 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
         __syncwarp();
     }
     u32 any = 0;
+    #pragma unroll 1
     for (u32 wi = lane; wi < c.nwords; wi += 32) {
         const u32 a = am[wi] | (want[wi] & freeb[wi]);
         am[wi] = a; any |= a;
@@ -1035,14 +1068,17 @@ __device__ void gpu_prepare(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 t0, 
     if (mode == 1) {
         const u32 e0 = c.row_ptr[g], deg = c.row_ptr[g + 1] - e0;
         u32* cnt = c.cnt + (size_t)g * c.W;
+        #pragma unroll 1
         for (u32 i = lane; i < c.W; i += 32) cnt[i] = 0;
         if (lane == 0) c.nheavy[g] = 0;
         if (deg > 1) {                                          // per-cycle issue counts of the direct out-links
             u32 dm = deg > 32 ? 0u : c.gdirect[g];
             if (deg > 32) { u32* h = c.hist + (size_t)e0 * c.W; for (u32 i = lane; i < deg * c.W; i += 32) h[i] = 0; }
+            #pragma unroll 1
             while (dm) {
                 const u32 x = __ffs(dm) - 1; dm &= dm - 1;
                 u32* h = c.hist + (size_t)(e0 + x) * c.W;
+                #pragma unroll 1
                 for (u32 i = lane; i < c.W; i += 32) h[i] = 0;
             }
         }
@@ -1106,6 +1142,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
         if (rb) {
             const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
             u64 x = rb;
+            #pragma unroll 1
             while (x) {                                         // four loads in flight at a time
                 u32 b[4]; u32 v[4]; int m = 0;
 #pragma unroll
@@ -1115,8 +1152,10 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
 #pragma unroll
                 for (int q = 0; q < 4; q++) if (q < m) aq[32 * na++] = (unsigned short)(((v[q] - t0) << 6) | b[q]);
             }
+            #pragma unroll 1
             for (u32 i = 1; i < na; i++) {
                 const u32 xv = aq[32 * i]; u32 j = i;
+                #pragma unroll 1
                 while (j > 0 && aq[32 * (j - 1)] > xv) { aq[32 * j] = aq[32 * (j - 1)]; j--; }
                 aq[32 * j] = (unsigned short)xv;
             }
@@ -1129,9 +1168,11 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
         u32 tt = 0, s = 0, ox = 0, last_issue = 0xffffffffu;    // tt: candidate cycle relative to t0
         u32 eq0 = 0, eq1 = 0, eq2 = 0, eq3 = 0, nb = 0;             // buffered issues: cycle << 6 | slot
         bool have_s = false;
+        #pragma unroll 1
         for (;;) {
             if (rem == ASTRA_NOTLOADED) {
                 bool got = false;
+                #pragma unroll 1
                 while (cur < end) {
                     const u32 s2 = cul[cur];
                     const u32 tr = t_release[s2];
@@ -1149,6 +1190,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
                 if (ai >= na) break;
                 tt = max(tt, nq >> 6);
             }
+            #pragma unroll 1
             while ((nq >> 6) <= tt) {                           // slots returned by this cycle (A3 before D)
                 busy &= ~(1ull << (nq & 63u)); ai++;
                 nq = ai < na ? aq[32 * ai] : 0xffffffffu;
@@ -1185,6 +1227,7 @@ __device__ void wf_sim(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 
                 if (hx) atomicAdd(&h[ox * W + t2], 1u);
             }
         }
+        #pragma unroll 1
         for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));   // acks later in the window than the last look
         c.wf_cur[gw] = cur; c.wf_rem[gw] = rem; c.wf_busy[gw] = busy;
         wantb = rem != ASTRA_NOTLOADED;
@@ -1274,9 +1317,11 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
     u32 idx = 0, xp = 0, last_issue = 0xffffffffu;              // xp: earliest cycle (relative to t0) of the next issue
     u32 im_lo = 0, im_hi = 0;                                   // slots taken by this lane's issues
     bool stop = false;
+    #pragma unroll 1
     while (!stop) {
         if (rem == ASTRA_NOTLOADED) {
             bool got = false;
+            #pragma unroll 1
             while (cur < end) {
                 const u32 s2 = cul[cur];
                 const u32 tr = t_release[s2];
@@ -1291,6 +1336,7 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
         const u32 s = cul[cur];
         const u32 ox = c.first_link[s] - e0;
         const bool hx = deg > 1 && ((c.gdirect[g] >> (ox & 31u)) & 1u);
+        #pragma unroll 1
         while (rem > 0) {
             const u32 i = idx + lane;
             const u32 want_n = min(32u, rem);
@@ -1399,9 +1445,12 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
             rb &= fullmask;
         }
         const u64* rec = c.ack_rec + (size_t)g * c.slots + b0;
+        #pragma unroll 1
         while (rb) { const u32 b = __ffsll((long long)rb) - 1; rb &= rb - 1; aq[32 * na++] = (unsigned short)((((u32)__ldcg(&rec[b]) - t0) << 6) | b); }
+        #pragma unroll 1
         for (u32 i = 1; i < na; i++) {
             const u32 xv = aq[32 * i]; u32 j = i;
+            #pragma unroll 1
             while (j > 0 && aq[32 * (j - 1)] > xv) { aq[32 * j] = aq[32 * (j - 1)]; j--; }
             aq[32 * j] = (unsigned short)xv;
         }
@@ -1412,12 +1461,15 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
     const u32 gdir = c.gdirect[g];
     u32 T = 0;
     if (turn) turn_wait(turn, wi, lane);                       // the grants of all lower words are in occ[] now
+    #pragma unroll 1
     for (;;) {
         // bring the lane to cycle T: slots returned by T, step loaded if released by T
         u32 np = 0xffffffffu;                                   // earliest cycle this lane can be ready
         if (active) {
+            #pragma unroll 1
             while ((nq >> 6) <= T) { busy &= ~(1ull << (nq & 63u)); ai++; nq = ai < na ? aq[32 * ai] : 0xffffffffu; }
             if (rem == ASTRA_NOTLOADED) {
+                #pragma unroll 1
                 while (cur < end) {
                     const u32 s2 = cul[cur];
                     const u32 tr = t_release[s2];
@@ -1436,6 +1488,7 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
         const u32 o = occ[T];
         if (o >= H) {                                           // cycle taken by lower ids: next cycle with room
             u32 t2 = T + 1;
+            #pragma unroll 1
             for (;;) {
                 const bool room = t2 + lane < wlen && occ[t2 + lane] < H;
                 const u32 rm2 = __ballot_sync(FULL, room);
@@ -1468,8 +1521,10 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
     if (turn) turn_pass(turn, wi, lane);
     bool wantb = false, freebit = false, hint = false;
     if (active) {
+        #pragma unroll 1
         for (; ai < na; ai++) busy &= ~(1ull << (aq[32 * ai] & 63u));
         if (rem == ASTRA_NOTLOADED) {                           // a step released by the end of the window is loaded (as in wf_sim)
+            #pragma unroll 1
             while (cur < end) {
                 const u32 s2 = cul[cur];
                 if (t_release[s2] >= t1) break;
@@ -1501,6 +1556,7 @@ __device__ ASTRA_COLD void wf_priority_word(const Ctx& __restrict__ c, Ctl& ctl,
 __device__ bool gpu_binds(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 lane) {
     const u32* cnt = c.cnt + (size_t)g * c.W;
     bool bind = false;
+    #pragma unroll 1
     for (u32 tt = lane; tt < wlen; tt += 32) if (cnt[tt] > c.H) bind = true;
     return __any_sync(FULL, bind);
 }
@@ -1513,6 +1569,7 @@ __device__ void gpu_finalize_counts(const Ctx& __restrict__ c, u32 g, u32 k, u32
     const u32 W = c.W;
     u32* cnt = c.cnt + (size_t)g * W;
     u32 carry = 0;
+    #pragma unroll 1
     for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
         const u32 v = (i < wlen) ? cnt[i] : 0;
@@ -1534,6 +1591,7 @@ __device__ void gpu_finalize_link(const Ctx& __restrict__ c, u32 e, u32 wlen, u3
     const bool direct = c.mask_off[e] == ASTRA_NONE32;
     u32 acc = direct ? c.run[e] : 0u;
     const u32 acc0 = acc;
+    #pragma unroll 1
     for (u32 b = 0; b < W; b += 32) {
         const u32 i = b + lane;
         const u32 v = (i < wlen) ? h[i] : 0;
@@ -1550,9 +1608,11 @@ __device__ void gpu_finalize_acks(const Ctx& __restrict__ c, u32 g, u32 k, u32 l
         u32* bm = c.bitmap + (size_t)(g * c.NW + (k & c.NWmask)) * c.bmwords;
         if (n_ack <= c.alcap) {     // every bit of the bin's words is consumed this window: whole words can go
             const u32* list = c.ack_list + (size_t)(g * c.NW + (k & c.NWmask)) * c.alcap;
+            #pragma unroll 1
             for (u32 i = lane; i < n_ack; i += 32) bm[__ldcg(&list[i]) >> 5] = 0;
         } else for (u32 i = lane; i < c.bmwords; i += 32) bm[i] = 0;
     }
+    #pragma unroll 1
     for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
 }
 __device__ void gpu_finalize(const Ctx& __restrict__ c, u32 g, u32 k, u32 wlen, u32 lane) {   // all parts on one warp
@@ -1580,6 +1640,7 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
     const u64* bucket = nullptr;
     if (act) {
         u32 lo = 0, hi = W;                                     // first index with cnt > i
+        #pragma unroll 1
         while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (cnt[mid] > i) hi = mid; else lo = mid + 1; }
         tt = lo - 1;
         st = cnt[tt]; n = (tt + 1 < W ? cnt[tt + 1] : nev) - st;
@@ -1593,6 +1654,7 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
     // holds at most H records, each with its wavefront id and out-link (bits 48.. of the record)
     u32 j = 0, jo = 0;
     const u32 oxm = o - e0;
+    #pragma unroll 1
     for (u32 x = 0; x < n; x++) {
         const u64 r2 = bucket[x];
         const bool lower = (((u32)r2 >> 20) & 0xfffu) < wf;
@@ -1623,13 +1685,15 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
 // stage 3a: FIFO positions of the cells of multi-feeder out-link o: exclusive prefix over the
 // cell popcounts of the window (R7/R8: cycle by cycle, slot order inside a cycle).
 // ---------------------------------------------------------------------------------------------
-__device__ void link_prefix(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, u32 lane) {
+// every cycle of the window is looked at: links that carry a line per cycle or more
+__device__ void link_prefix_dense(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, u32 lane) {
     const u32 v = c.tail[o];
     const u32 mw = c.nd_mw[v], NC = c.NC;
     const u32* masks = c.masks + c.mask_off[o];
     u32* pre = c.pre + c.pre_off[o];
     u32 n_new = 0;
     // four consecutive cycles per lane: their cell words are loaded together, one warp scan per 128 cycles
+#pragma unroll 1
     for (u32 b = 0; b < wlen; b += 128) {
         u32 cq[4];
 #pragma unroll
@@ -1655,6 +1719,50 @@ __device__ void link_prefix(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, 
     if (lane == 0) c.run[o] = c.ltail[o] + n_new;
 }
 
+// only the cycles marked in the link's bitmap of non-empty cells are looked at: links below one line per cycle
+__device__ void link_prefix(const Ctx& __restrict__ c, u32 o, u32 wlen, u32 cb, u32* scr, u32 lane) {
+    const u32 v = c.tail[o];
+    const u32 mw = c.nd_mw[v], NC = c.NC;
+    const u32* masks = c.masks + c.mask_off[o];
+    u32* pre = c.pre + c.pre_off[o];
+    if (c.nz_off[o] == ASTRA_NONE32) { link_prefix_dense(c, o, wlen, cb, lane); return; }
+    const u32* nz = c.nz + c.nz_off[o];
+    const u32 nzw = (wlen + 31) / 32;
+    // the non-empty cycles of the window (cycle wlen belongs to the next one), in ascending order, into the warp's scratch
+    u32 total = 0;
+    #pragma unroll 1
+    for (u32 wb = 0; wb < nzw; wb += 32) {
+        const u32 wi = wb + lane;
+        u32 w = wi < nzw ? nz[wi] : 0u;
+        if (wi == (wlen >> 5)) w &= (1u << (wlen & 31)) - 1u;
+        const u32 cw = __popc(w);
+        const u32 incl = warp_incl_scan(cw, lane);
+        u32 pos = total + incl - cw;
+        #pragma unroll 1
+        while (w) { const u32 b = __ffs(w) - 1; w &= w - 1; scr[pos++] = wi * 32 + b; }
+        total += __shfl_sync(FULL, incl, 31);
+    }
+    __syncwarp();
+    // cell popcounts and their exclusive prefix, 32 non-empty cycles per step
+    u32 n_new = 0;
+    #pragma unroll 1
+    for (u32 b = 0; b < total; b += 32) {
+        const u32 j = b + lane;
+        u32 cq = 0, tau = 0;
+        if (j < total) {
+            tau = scr[j];
+            u32 ci = cb + tau; if (ci >= NC) ci -= NC;
+            #pragma unroll 1
+            for (u32 w = 0; w < mw; w++) cq += __popc(masks[ci * mw + w]);
+        }
+        const u32 incl = warp_incl_scan(cq, lane);
+        if (j < total) pre[tau] = n_new + incl - cq;
+        n_new += __shfl_sync(FULL, incl, 31);
+    }
+    __syncwarp();
+    if (lane == 0) c.run[o] = c.ltail[o] + n_new;
+}
+
 // stage 3b: GPU g's recorded injections go to their FIFO positions; the ones that enter at the
 // first cycle of the next window stay recorded.
 __device__ void inject_place(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 cb, u32 lane) {
@@ -1663,6 +1771,7 @@ __device__ void inject_place(const Ctx& __restrict__ c, u32 g, u32 wlen, u32 cb,
     u64* inj = c.inj_list + c.inj_off[g];
     const u32 injoff = c.nd_injoff[g];
     u32 keep = 0;
+    #pragma unroll 1
     for (u32 b = 0; b < n; b += 32) {
         const u32 i = b + lane;
         const bool act = i < n;
@@ -1694,20 +1803,42 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
     const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
     if (c.dirty[e]) {                                        // consume the cells of the window
         const u32 v = c.tail[e];
-        const u32 mw = c.nd_mw[v];
+        const u32 mw = c.nd_mw[v], NC = c.NC;
         u32* masks = c.masks + c.mask_off[e];
-        {   // cells [cb, cb + wlen) of the circular array: one or two contiguous word ranges
-            const u32 end1 = min(cb + wlen, c.NC);
+        bool carry = false;                                  // injections that enter at t1 (cycle wlen) keep the link marked
+        if (c.nz_off[e] == ASTRA_NONE32) {
+            // cells [cb, cb + wlen) of the circular array: one or two contiguous word ranges
+            const u32 end1 = min(cb + wlen, NC);
+            #pragma unroll 1
             for (u32 x = cb * mw + lane; x < end1 * mw; x += 32) masks[x] = 0;
-            if (cb + wlen > c.NC) for (u32 x = lane; x < (cb + wlen - c.NC) * mw; x += 32) masks[x] = 0;
+            if (cb + wlen > NC) for (u32 x = lane; x < (cb + wlen - NC) * mw; x += 32) masks[x] = 0;
+            __syncwarp();
+            u32 ci = cb + wlen; if (ci >= NC) ci -= NC;
+            #pragma unroll 1
+            for (u32 w = lane; w < mw; w += 32) carry |= masks[ci * mw + w] != 0u;
+            carry = __any_sync(FULL, carry);
+        } else {                                             // only the marked cells
+            u32* nz = c.nz + c.nz_off[e];
+            const u32 NZW = (NC + 31) / 32;
+            #pragma unroll 1
+            for (u32 wi = lane; wi < NZW; wi += 32) {
+                u32 w = nz[wi];
+                if (w == 0u) continue;
+                nz[wi] = 0u;
+                if (wi == (wlen >> 5) && ((w >> (wlen & 31)) & 1u)) { carry = true; w &= ~(1u << (wlen & 31)); }
+                #pragma unroll 1
+                while (w) {
+                    const u32 b = __ffs(w) - 1; w &= w - 1;
+                    u32 ci = cb + wi * 32 + b; if (ci >= NC) ci -= NC;
+                    #pragma unroll 1
+                    for (u32 x = 0; x < mw; x++) masks[ci * mw + x] = 0u;
+                }
+            }
+            carry = __any_sync(FULL, carry);
+            if (lane == 0 && carry) nz[0] = 1u;                // cycle wlen is cycle 0 of the next window
         }
+        if (lane == 0) c.dirty[e] = carry ? 1u : 0u;
         __syncwarp();
-        if (lane == 0) {                                     // injections that enter at t1 keep the link marked
-            u32 ci = cb + wlen; if (ci >= c.NC) ci -= c.NC;
-            u32 any = 0;
-            for (u32 w = 0; w < mw; w++) any |= masks[ci * mw + w];
-            c.dirty[e] = any ? 1u : 0u;
-        }
     }
     const u32 n_back = tl - fh, n_new = tn - tl;
     const u32 n_tot = n_back + n_new;
@@ -1737,6 +1868,7 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
         u64 nx[4];                                           // next step's entries, loaded one step ahead
 #pragma unroll
         for (int q = 0; q < 4; q++) nx[q] = 4 * lane + q < scan_limit ? ring[(fh + 4 * lane + q) & rmask] : 0ull;
+        #pragma unroll 1
         for (u32 base = 0; base < scan_limit; base += 128) {
             const u32 j0 = base + 4 * lane;
             u64 fl[4]; int val[4]; u32 xx[4]; bool act[4];
@@ -1795,6 +1927,7 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
     // ring loads run two chunks ahead of the scan
     u64 fq0 = lane < scan_limit ? ring[(fh + lane) & rmask] : 0ull;
     u64 fq1 = 32 + lane < scan_limit ? ring[(fh + 32 + lane) & rmask] : 0ull;
+    #pragma unroll 1
     for (u32 base = 0; base < scan_limit; base += 32) {
         const u32 i = base + lane;
         const bool act = i < scan_limit;
@@ -1821,6 +1954,7 @@ __device__ void link_service(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e
         } else {
             // saturating credit walked in FIFO order; every lane tracks the same state
             const u32 bw = param;
+            #pragma unroll 1
             for (u32 j = 0; j < 32; j++) {
                 if (base + j >= scan_limit) break;
                 const u32 aj = t0 + __shfl_sync(FULL, a, j);
@@ -1914,6 +2048,7 @@ __device__ __forceinline__ bool group_barrier(GroupCtl* gc, u32 target, u32* abo
         atomicAdd(&gc->bar, 1u);
         const long long start = clock64();
         u32 spins = 0;
+        #pragma unroll 1
         while ((int32_t)(*(volatile u32*)&gc->bar - target) < 0) {
             if ((++spins & 0x3ffu) == 0) {
                 if (*(volatile u32*)abort_flag) { ctl.abort = 1u; break; }
@@ -1935,7 +2070,7 @@ __device__ __forceinline__ void set_sync(u32 ws, u32 set) {
 
 // The rest of a node's window after the issue decisions: placement of the window's issues (or the cycle-serial
 // issue path), merge into multi-feeder out-links, link service.  e_l .. fl_l: the node's first 32 in-links, one per
-// lane (id, lines due, read cursor, arrival path), as loaded by stage 1 (inlinks_first reloads them).
+// lane (id, lines due, read cursor, arrival path), as loaded by stage 1.
 __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
                           u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, u32 mode,
                           u32 e_l, u32 n_l, u32 lo_l, u32 fl_l) {
@@ -1953,11 +2088,13 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
         if (sw == 0) {
             ack_sort(c, ctl, g, k, t0, wlen, scr, lane);
             issue_window(c, ctl, hp, g, t0, t1, cb, lane);
+            #pragma unroll 1
             for (u32 wi = lane; wi < c.nwords; wi += 32) c.amask[(size_t)g * c.nwords + wi] = 0;
         }
         set_sync(ws, set);
     } else if (mode == 1u) {
         const u32 nch = (c.sel[(size_t)g * c.H] + 31) / 32;
+        #pragma unroll 1
         for (u32 ch = sw; ch < nch; ch += ws) ev_place(c, ctl, g, ch, t0, cb, lane);
         set_sync(ws, set);
     }
@@ -1965,14 +2102,17 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
 
     // ---- stage 3: merge into multi-feeder out-links of v (skipped when none received a line) ----
     bool any_dirty = false;
+    #pragma unroll 1
     for (u32 e = e_lo + lane; e < e_hi; e += 32) any_dirty |= c.dirty[e] != 0u;
     any_dirty = __any_sync(FULL, any_dirty);
     if (any_dirty) {
+        #pragma unroll 1
         for (u32 e = e_lo + sw; e < e_hi; e += ws)
-            if (c.dirty[e]) link_prefix(c, e, wlen, cb, lane);
+            if (c.dirty[e]) link_prefix(c, e, wlen, cb, scr, lane);
         set_sync(ws, set);
         if (is_gpu && sw == ws - 1) inject_place(c, v, wlen, cb, lane);
         u32 tmod3 = 0;
+        #pragma unroll 1
         for (u32 ib = i_lo; ib < i_hi; ib += 32) {
             const u32 i = ib + lane;
             u32 e_b = e_l, n_b = n_l, lo_b = lo_l, fl_b = fl_l;
@@ -1986,12 +2126,14 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
             // links that marked cells in pass 1 go over the same lines again, now with the FIFO positions known
             const bool again = i < i_hi && (fl_b == 0u ? c.ndue[e_b] != 0u : (fl_b == ASTRA_LF_CELLS && c.tl_base[e_b] != 0u));
             u32 nm = __ballot_sync(FULL, again);
+            #pragma unroll 1
             while (nm) {
                 const u32 src = __ffs(nm) - 1; nm &= nm - 1;
                 const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
                 const u32 lo = __shfl_sync(FULL, lo_b, src), fl = __shfl_sync(FULL, fl_b, src);
                 const u32 first = (sw + ws - tmod3) % ws;
                 if (fl == 0u) { if (first == 0u) arrivals_link<3>(c, ctl, hp, ib + src, 0u, k, t0, wlen, cb, lane); tmod3 = (tmod3 + 1) % ws; continue; }
+                #pragma unroll 1
                 for (u32 ch = first; ch * 64 < n; ch += ws) cells_place_chunk(c, e, lo, n, ch, t0, wlen, cb, lane);
                 tmod3 = (tmod3 + (n + 63) / 64) % ws;
             }
@@ -2002,6 +2144,7 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
 
     // ---- stage 4: link service of v's out-links (R9); the in-links' cursors move past the window ----
     if (sw == ws - 1) {
+        #pragma unroll 1
         for (u32 ib = i_lo; ib < i_hi; ib += 32) {
             const u32 i = ib + lane;
             if (i >= i_hi) continue;
@@ -2012,20 +2155,9 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
             if (fl != 0u) { c.pipe_head[e] += n; c.tl_base[e] = 0; }
         }
     }
+    #pragma unroll 1
     for (u32 e = e_lo + sw; e < e_hi; e += ws) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
     DIAG_CLK(6);
-}
-
-// The first 32 in-links of node v, one per lane, as stage 1 of node_window loads them.
-__device__ __forceinline__ void inlinks_first(const Ctx& __restrict__ c, u32 v, u32 k, u32 lane, u32& e_l, u32& n_l, u32& lo_l, u32& fl_l) {
-    const u32 i = c.in_ptr[v] + lane;
-    e_l = n_l = lo_l = fl_l = 0;
-    if (i < c.in_ptr[v + 1]) {
-        e_l = c.in_link[i];
-        n_l = ld_vol(&c.due_cnt[(size_t)e_l * c.NW + (k & c.NWmask)]);
-        lo_l = c.pipe_head[e_l];
-        fl_l = (c.flags & (u32)ASTRA_FLAG_SERIAL_ARRIVALS) ? 0u : c.lflag[e_l];
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -2033,9 +2165,8 @@ __device__ __forceinline__ void inlinks_first(const Ctx& __restrict__ c, u32 v, 
 // set of ws warps).  Inside a window nothing a node does can reach another node (W <= min Leff), so
 // the stages of a node order only against each other: set barriers, no block barrier.
 // ---------------------------------------------------------------------------------------------
-// Returns true when the node's budget-bound issue sweep and the rest of its window were deferred to the CTA (may_defer).
-__device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
-                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane, bool may_defer) {
+__device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u32 k, u32 t0, u32 t1, u32 cb,
+                            u32* scr, u32 lane, u32 sw, u32 ws, u32 set, bool diag_lane) {
 #ifdef ASTRA_DIAG
     long long dck = clock64();
 #endif
@@ -2056,10 +2187,12 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         if (sw == ws - 1) stage1_setup_gpu(c, ctl, hp, v, k, lane);
         const u32 n_ack = ld_vol(&c.bin_cnt[v * c.NW + kb]);
         if (n_ack && n_ack <= c.alcap) {                         // alcap == 0: no list, the bitmap is scanned
+            #pragma unroll 1
             for (u32 ch = sw; ch * 128 < n_ack; ch += ws) ack_list_chunk(c, ctl, v, ch, n_ack, k, t1, lane);
             tmod = ((n_ack + 127) / 128) % ws;
         } else if (n_ack) {
             const u32 nch = (c.bmwords + 31) / 32;
+            #pragma unroll 1
             for (u32 ch = sw; ch < nch; ch += ws) ack_chunk(c, ctl, v, ch, k, t1, scr, lane);
             tmod = nch % ws;
         }
@@ -2067,6 +2200,7 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     // the node's in-links, one per lane: id, lines due this window (counted by the link's service when it
     // accepted them), read cursor, arrival path -- all loads of a batch of 32 links in flight at once
     u32 e_l = 0, n_l = 0, lo_l = 0, fl_l = 0;
+    #pragma unroll 1
     for (u32 ib = i_lo; ib < i_hi; ib += 32) {
         const u32 i = ib + lane;
         u32 e_b = 0, n_b = 0, lo_b = 0, fl_b = 0;
@@ -2079,6 +2213,7 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         }
         if (ib == i_lo) { e_l = e_b; n_l = n_b; lo_l = lo_b; fl_l = fl_b; }     // first batch stays in registers for stages 3 and 4
         u32 nm = __ballot_sync(FULL, n_b != 0u);
+        #pragma unroll 1
         while (nm) {
             const u32 src = __ffs(nm) - 1; nm &= nm - 1;
             const u32 e = __shfl_sync(FULL, e_b, src), n = __shfl_sync(FULL, n_b, src);
@@ -2086,12 +2221,15 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             const u32 first = (sw + ws - tmod) % ws;
             if (fl == 0u) { if (first == 0u) arrivals_link<1>(c, ctl, hp, ib + src, n, k, t0, wlen, cb, lane); tmod = (tmod + 1) % ws; continue; }
             if (fl == ASTRA_LF_DELIVER_ONLY) {
+                #pragma unroll 1
                 for (u32 ch = first; ch * 32 < n; ch += ws) deliver_chunk(c, ctl, hp, e, lo, n, ch, k, t0, wlen, lane);
             } else if (fl == ASTRA_LF_FORWARD_ONLY) {
                 const u32 base = c.run[c.lfwd[e]];
+                #pragma unroll 1
                 for (u32 ch = first; ch * 32 < n; ch += ws) forward_chunk(c, e, lo, n, base, ch, t0, wlen, lane);
                 any_fwd = true;
             } else {
+                #pragma unroll 1
                 for (u32 ch = first; ch * 64 < n; ch += ws) cells_chunk(c, ctl, hp, e, lo, n, ch, k, t0, wlen, cb, lane);
             }
             tmod = (tmod + (fl == ASTRA_LF_CELLS ? (n + 63) / 64 : (n + 31) / 32)) % ws;
@@ -2099,6 +2237,7 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     }
     set_sync(ws, set);
     if (any_fwd && sw == 0) {                    // forwarded lines are now in the next link's FIFO
+        #pragma unroll 1
         for (u32 ib = i_lo; ib < i_hi; ib += 32) {
             const u32 i = ib + lane;
             if (i >= i_hi) continue;
@@ -2118,10 +2257,12 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
         mode = c.gmode[g];
     }
     if (mode == 1u) {
+        #pragma unroll 1
         for (u32 wi = sw; wi < c.nwords; wi += ws) wf_sim(c, ctl, hp, g, wi, k, t0, t1, scr, lane);
         set_sync(ws, set);
         const u32 nh = c.nheavy[g];
         if (nh) {
+            #pragma unroll 1
             for (u32 j = sw; j < nh; j += ws) wf_heavy(c, ctl, hp, g, c.hlist[(size_t)g * c.CW + j], k, t0, t1, scr, lane);
             set_sync(ws, set);
         }
@@ -2134,23 +2275,21 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
             if (deg > 1) for (u32 x = (sw + ws - 1) % ws; x < deg; x += ws) if (deg > 32 || ((c.gdirect[g] >> x) & 1u)) gpu_finalize_link(c, e_lo + x, wlen, lane);
             if (sw == ws - 1) gpu_finalize_acks(c, g, k, lane);
         } else if (c.flags & (u32)ASTRA_FLAG_NO_PRIORITY_SWEEP) {      // testing: back to the window start, cycle-serial path
+            #pragma unroll 1
             for (u32 wi = sw; wi < c.nwords; wi += ws) wf_restore_word(c, g, wi, lane);
             if (sw == 0 && lane == 0) c.gmode[g] = 2u;
         } else {
             // The budget binds: back to the window start, then the exact grants word by word (wf_priority_word).
-            // The sweep is ordered, but every warp that takes part loads and sorts its words' inputs on its own:
-            // the warps of the set -- or, for a one-warp set, all warps of the CTA after the window's barrier
-            // (bb_sweep); the rest of this node's window then follows (node_tail).
+            // The sweep is ordered, but every warp of the set loads and sorts its words' inputs on its own and then
+            // waits for its turn (a CTA-wide version for one-warp sets was measured: no gain on config 4).
             if (sw == 0 && lane == 0) DIAG_ADD(6, 1);
+            #pragma unroll 1
             for (u32 i = sw * 32 + lane; i < c.W; i += ws * 32) c.cnt[(size_t)g * c.W + i] = 0;
             if (deg > 1) for (u32 x = 0; x < deg; x++)
                 if (deg > 32 || ((c.gdirect[g] >> x) & 1u)) for (u32 i = sw * 32 + lane; i < c.W; i += ws * 32) c.hist[(size_t)(e_lo + x) * c.W + i] = 0;
             if (sw == 0 && lane == 0) c.turn[g] = 0u;
-            if (may_defer) {
-                if (lane == 0) ctl.bbq[atomicAdd(&ctl.nbb, 1u)] = g;
-                return true;
-            }
             set_sync(ws, set);
+            #pragma unroll 1
             for (u32 wi = sw; wi < c.nwords; wi += ws) {
                 wf_restore_word(c, g, wi, lane);
                 wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, ws > 1 ? &c.turn[g] : nullptr, lane);
@@ -2163,17 +2302,6 @@ __device__ bool node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     } else if (!is_gpu && any_fwd) set_sync(ws, set);
     DIAG_CLK(3);
     node_tail(c, ctl, hp, v, k, t0, t1, cb, scr, lane, sw, ws, set, diag_lane, mode, e_l, n_l, lo_l, fl_l);
-    return false;
-}
-
-// A budget-bound GPU-window of a one-warp node, swept by all warps of the CTA after the window's barrier: team
-// member r of m takes words r, r + m, ... (restore, load, sort, then the ordered sweep); the last word's warp commits.
-__device__ ASTRA_COLD void bb_sweep(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u32 r, u32 m, u32 k, u32 t0, u32 t1, u32* scr, u32 lane) {
-    for (u32 wi = r; wi < c.nwords; wi += m) {
-        wf_restore_word(c, g, wi, lane);
-        wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, &c.turn[g], lane);
-        if (wi == c.nwords - 1) gpu_finalize(c, g, k, t1 - t0, lane);
-    }
 }
 
 __device__ __forceinline__ void
@@ -2200,6 +2328,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
     u32 bar_target = 0;                 // arrivals that complete the next group barrier
     if (tid == 0) ctl.abort = 0u;
 
+    #pragma unroll 1
     for (;;) {
         __syncthreads();
         if (group == 1) {
@@ -2236,10 +2365,11 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
             ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
-            ctl.nbb = 0u;
             ctl.g_hint = ASTRA_T_INF; ctl.g_acked = 0; ctl.g_err = 0; ctl.g_completion = 0;
 #ifdef ASTRA_DIAG
+            #pragma unroll 1
             for (int i = 0; i < 16; i++) ctl.clk[i] = 0;
+            #pragma unroll 1
             for (int i = 0; i < 128; i++) (&ctl.sclk[0][0])[i] = 0;
 #endif
         }
@@ -2248,6 +2378,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
 #endif
         __syncthreads();
         // ---- state init: shared-memory arrays by their CTA, global arrays split over the group ----
+        #pragma unroll 1
         for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
             const u32 kind = k_arr_init[a];
             if (kind > 1) continue;
@@ -2262,7 +2393,9 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             else { for (u64 i = (u64)rank * nthr + tid; i < n16; i += (u64)group * nthr) p[i] = v4; }
         }
         if (group > 1) { bar_target += group; if (!group_barrier(gc, bar_target, abort_flag, ctl)) break; } else __syncthreads();
+        #pragma unroll 1
         for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.lstate0[e] = c.lstate0_init[e];
+        #pragma unroll 1
         for (u32 s = tid; s < c.S; s += nthr) {
             const u32 ow = c.step_od[s] >> 16;
             if (ow < c.g_lo || ow >= c.g_hi) continue;
@@ -2270,9 +2403,13 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             // steps without deps are released at t = 0 (R10) -- unless the watchdog allows no cycle at all
             c.t_release[s] = (c.ndeps[s] || c.tmax == 0u) ? ASTRA_TS_NONE32 : 0u;
         }
+        #pragma unroll 1
         for (u32 gq = c.g_lo; gq < c.g_hi; gq++) {
+            #pragma unroll 1
             for (u32 j = c.rel_off[gq] + tid; j < c.rel_off[gq + 1]; j += nthr) c.plist[j] = c.init_rel[j];
+            #pragma unroll 1
             for (u32 wf = tid; wf < c.CW; wf += nthr) c.wf_cur[(size_t)gq * c.CW + wf] = c.cul_ptr[gq * c.C + wf / c.Wv];
+            #pragma unroll 1
             for (u32 wi = tid; wi < c.nwords; wi += nthr) {
                 const u32 nb = c.CW - wi * 32;
                 c.freeb[(size_t)gq * c.nwords + wi] = nb >= 32 ? ~0u : ((1u << nb) - 1u);
@@ -2290,8 +2427,6 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const u32 wset = nwarps / nsets;                   // warps per set (left-over warps idle through the window)
         const u32 set = warp / wset, sw = warp % wset;
         const bool in_set = set < nsets;
-        // one-warp nodes, at most one per warp: a budget-bound sweep is handed to the whole CTA (bb_sweep)
-        const bool may_defer = wset == 1u && n_nodes <= nwarps && nwarps > 1u;
 
         // ---- window loop ----
         u32 k = 0, seq = 0;
@@ -2299,6 +2434,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const u32 W = c.W;
         u64 busy = 0, skipped = 0;
         bool aborted = false;
+        #pragma unroll 1
         for (;;) {
             const u64 t0l = (u64)k * W;
             if (t0l >= c.tmax) { status = ASTRA_STATUS_MAX_CYCLES; break; }
@@ -2307,36 +2443,17 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             const u32 cb = t0 % c.NC;
             u32* const hp = &ctl.hint[seq % 3];
             busy += t1 - t0;
-            bool deferred = false;
             if (in_set)
+#pragma unroll 1
                 for (u32 j = set; j < n_nodes; j += nsets)
-                    deferred = node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0, may_defer);
-            bool synced = false;                               // the CTA has met and nothing was done since
-            if (may_defer) {
-                __syncthreads();
-                const u32 nbb = ctl.nbb;                       // the same value in every thread
-                synced = nbb == 0u;
-                if (nbb) {
-                    // warp w joins the team of GPU bbq[w % nbb] as member w / nbb
-                    const u32 gi = warp % nbb;
-                    bb_sweep(c, ctl, hp, ctl.bbq[gi], warp / nbb, (nwarps - gi + nbb - 1u) / nbb, k, t0, t1, scr, lane);
-                    __syncthreads();
-                    if (tid == 0) ctl.nbb = 0u;
-                    if (deferred) {
-                        const u32 v = c.v_lo + set;
-                        u32 e_l, n_l, lo_l, fl_l;
-                        inlinks_first(c, v, k, lane, e_l, n_l, lo_l, fl_l);
-                        node_tail(c, ctl, hp, v, k, t0, t1, cb, scr, lane, 0u, 1u, set, lane == 0, c.gmode[v], e_l, n_l, lo_l, fl_l);
-                    }
-                }
-            }
+                    node_window(c, ctl, hp, c.v_lo + j, k, t0, t1, cb, scr, lane, sw, wset, set, sw == 0 && lane == 0);
             // ---- stage 5: next non-idle window (A7), one block barrier per window ----
 #ifdef ASTRA_DIAG
             dck = clock64();
 #endif
             u32 hint, acked_total, err;
             if (group > 1) {
-                if (!synced) __syncthreads();
+                __syncthreads();
                 if (tid == 0) {
                     atomicMin(&gc->hint[seq % 3], *hp);
                     if (ctl.acked) { atomicAdd(&gc->acked, ctl.acked); atomicMax(&gc->completion, ctl.completion); ctl.acked = 0; }
@@ -2355,7 +2472,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
                 __syncthreads();
                 hint = ctl.g_hint; acked_total = ctl.g_acked; err = ctl.g_err;
             } else {
-                if (!synced) __syncthreads();
+                __syncthreads();
                 hint = *hp; acked_total = ctl.acked; err = ctl.err;
                 // slot (seq + 2) % 3 was last read before this barrier and is next written after the next one
                 if (tid == 0) ctl.hint[(seq + 2) % 3] = ASTRA_T_INF;
@@ -2379,6 +2496,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         __syncthreads();
         // ---- A8: write-out (each CTA the steps / links of its own nodes) ----
         u32 cmax = 0;                                       // completion = max t_ack over fully acked steps (R14)
+        #pragma unroll 1
         for (u32 s = tid; s < c.S; s += nthr) {
             const u32 n = c.lines[s];
             const u32 od = c.step_od[s];
@@ -2394,6 +2512,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             if (ds >= c.g_lo && ds < c.g_hi)
                 c.r_step_ts[4 * (size_t)s + 2] = c.deliv_cnt[s] == n ? (u64)c.t_deliv[s] : ~0ull;
         }
+        #pragma unroll 1
         for (u32 e = c.e_lo + tid; e < c.e_hi; e += nthr) c.r_link_lines[e] = c.link_lines[e];
         cmax = __reduce_max_sync(FULL, cmax);
         if (tid == 0) ctl.completion = 0;

@@ -49,7 +49,7 @@ typedef uint64_t u64;
     X(in_ptr) X(in_link) X(head) X(tail) X(leff) X(next_link) X(row_ptr) \
     X(step_od) X(lines) X(cu_lo) X(cu_n) X(succ_ptr) X(succ) X(ndeps) \
     X(step_q) X(step_r) X(first_link) X(step_alpha) X(step_aq) X(step_ar) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
-    X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(classoff) \
+    X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(nz_off) X(classoff) \
     X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(gflag) X(gdirect) X(lflag) X(lfwd) X(lscr_off)
 
 // Mutable arrays of a design point.  X(name, element type, init) with init: 0 zero, 1 0xff bytes,
@@ -59,7 +59,7 @@ typedef uint64_t u64;
 #define ASTRA_WS_ARRAYS(X) \
     X(pipe_head, u32, 0) X(fifo_head, u32, 0) X(ltail, u32, 0) X(run, u32, 0) X(lstate0, u32, 2) X(lstate1, u32, 0) \
     X(link_lines, u32, 0) X(dirty, u32, 0) X(ndue, u32, 0) X(due_cnt, u32, 0) X(tl_lo, u32, 3) X(tl_n, u32, 3) X(tl_base, u32, 3) X(tbase, u32, 3) X(pcnt, u32, 2) X(ev_cnt, u32, 0) X(ack_n, u32, 0) \
-    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(turn, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(masks, u32, 0) X(pre, u32, 3) \
+    X(inj_n, u32, 0) X(want, u32, 0) X(freeb, u32, 2) X(amask, u32, 0) X(gmode, u32, 0) X(nheavy, u32, 0) X(turn, u32, 0) X(cnt, u32, 3) X(hist, u32, 3) X(sel, u32, 3) X(nz, u32, 0) X(masks, u32, 0) X(pre, u32, 3) \
     X(t_release, u32, 2) X(issued_cnt, u32, 0) X(t_issued, u32, 0) X(deliv_cnt, u32, 0) X(t_deliv, u32, 0) \
     X(ack_cnt, u32, 0) X(t_ack, u32, 0) X(ndep_left, u32, 2) X(rel_time, u32, 0) X(plist, u32, 2) X(ev_list, u32, 3) \
     X(bin_cnt, u32, 0) X(cu_out, u32, 0) X(wf_busy, u64, 0) X(wf_rem, u32, 1) X(wf_cur, u32, 2) \

@@ -253,12 +253,15 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     std::vector<uint8_t> delivers(E, 0), transits(E, 0), multi_fwd(E, 0);
     std::vector<u32> fwd(E, ASTRA_NONE32);       // the one link that lines arriving over e are forwarded to
     std::vector<double> load(V, 0.0);
+    std::vector<u64> via_tot(E, 0);                 // lines routed over every link, all owners
+    double t_win = 1.0;                             // run length if only the outstanding caps bound it (cycles)
     {
         std::vector<std::vector<u32>> by_owner(G);
         for (u32 s = 0; s < S; s++) by_owner[c.owner[s]].push_back(s);
         std::vector<u64> via(E, 0); std::vector<u32> touched;
         for (u32 o = 0; o < G; o++) {
             touched.clear();
+            double t_own = 0.0;
             for (u32 s : by_owner[o]) {
                 u32 v = o, d = c.dst[s], hops = 0, prev = E;
                 while (v != d) {
@@ -279,9 +282,11 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
                     if (++hops > V) { err = "routing loop"; return ASTRA_EINVAL; }
                 }
                 load[o] += 2.0 * c.lines[s];
+                t_own += (double)c.lines[s] * (2.0 * step_alpha[s] + 1.0) / (double)slots;
                 cost += (double)c.lines[s] * hops;
             }
-            for (u32 e : touched) { bound[e] += std::min<u64>(slots, via[e]); via[e] = 0; }
+            for (u32 e : touched) { bound[e] += std::min<u64>(slots, via[e]); via_tot[e] += via[e]; via[e] = 0; }
+            t_win = std::max(t_win, t_own);
         }
     }
     // cells: slot layout per node, cell and prefix regions per multi-feeder link
@@ -298,8 +303,31 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         if (nd_cellcap[v] == 0) nd_cellcap[v] = 1;
         nd_mw[v] = (nd_cellcap[v] + 31) / 32;
     }
-    std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), inj_off(G + 1, 0);
-    u64 ring_total = 0, mask_total = 0, pre_total = 0;
+    // A multi-feeder link whose cells are expected to be mostly empty keeps a bitmap of the non-empty ones (see cell_set).
+    // Estimate: run length = the longer of the bottleneck link's occupancy and the outstanding-cap bound; a link with
+    // via lines over that time sees them in bursts of ceil(B) per cycle, so about via / (ceil(B) * cycles) of its cells
+    // are marked.  Sparse below 1/8.  (Performance only: both paths give the same result.)
+    std::vector<uint8_t> sparse_cells(E, 0);
+    {
+        double t_bw = 1.0;
+        for (u32 e = 0; e < E; e++) t_bw = std::max(t_bw, (double)via_tot[e] * 256.0 / t.bw[e]);
+        const double t_run = std::max(t_bw, t_win);
+        for (u32 e = 0; e < E; e++) {
+            const double cb_ = std::max(1.0, t.bw[e] / 256.0);
+#if defined(ASTRA_X_SPARSE_ALL)
+            sparse_cells[e] = 1;
+#elif defined(ASTRA_X_SPARSE_NONE)
+            sparse_cells[e] = 0;
+#elif defined(ASTRA_X_SPARSE_T)
+            sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < ASTRA_X_SPARSE_T;
+#else
+            sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < 0.125;
+#endif
+        }
+    }
+    std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), nz_off(E, ASTRA_NONE32), inj_off(G + 1, 0);
+    u64 ring_total = 0, mask_total = 0, pre_total = 0, nz_total = 0;
+    const u32 NZW = (NC + 31) / 32;            // words of a link's bitmap of non-empty cells (one bit per cycle of the window)
     for (u32 e = 0; e < E; e++) {
         u32 ceilb = (t.bw[e] + 255) / 256;
         ceilb_v[e] = ceilb;
@@ -316,6 +344,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
             if (mask_total + mk >= (1ull << 31) || pre_total + NC >= (1ull << 31)) { err = "cell space exceeds 2^31 words"; return ASTRA_ELIMIT; }
             mask_off[e] = (u32)mask_total; mask_total += mk;
             pre_off[e] = (u32)pre_total; pre_total += NC;
+            if (sparse_cells[e]) { nz_off[e] = (u32)nz_total; nz_total += NZW; }
             if (v < G) inj_off[v + 1] = g.H * (W + 2);
         } else { mask_off[e] = ASTRA_NONE32; pre_off[e] = ASTRA_NONE32; }
     }
@@ -430,7 +459,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_ring_off] = blob.add(ring_off); co[ASTRA_C_ring_mask] = blob.add(ring_mask);
     co[ASTRA_C_lkind] = blob.add(lkind); co[ASTRA_C_ceilb] = blob.add(ceilb_v);
     co[ASTRA_C_lstate0_init] = blob.add(lstate0);
-    co[ASTRA_C_mask_off] = blob.add(mask_off); co[ASTRA_C_pre_off] = blob.add(pre_off);
+    co[ASTRA_C_mask_off] = blob.add(mask_off); co[ASTRA_C_pre_off] = blob.add(pre_off); co[ASTRA_C_nz_off] = blob.add(nz_off);
     co[ASTRA_C_classoff] = blob.add(classoff); co[ASTRA_C_nd_mw] = blob.add(nd_mw);
     co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
     co[ASTRA_C_part] = blob.add(part);
@@ -454,7 +483,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     ab[ASTRA_A_hist] = 4ull * ((u64)t.row_ptr[G] * W + 1);
     ab[ASTRA_A_evb] = 8ull * G * g.H * W;
     ab[ASTRA_A_sel] = 4ull * G * g.H;
-    ab[ASTRA_A_masks] = 4ull * mask_total; ab[ASTRA_A_pre] = 4ull * pre_total;
+    ab[ASTRA_A_masks] = 4ull * mask_total; ab[ASTRA_A_pre] = 4ull * pre_total; ab[ASTRA_A_nz] = 4ull * nz_total;
     for (u32 a : {ASTRA_A_t_release, ASTRA_A_issued_cnt, ASTRA_A_t_issued, ASTRA_A_deliv_cnt, ASTRA_A_t_deliv,
                   ASTRA_A_ack_cnt, ASTRA_A_t_ack, ASTRA_A_ndep_left, ASTRA_A_rel_time, ASTRA_A_plist}) ab[a] = 4ull * S;
     ab[ASTRA_A_ev_list] = 4ull * ev_off[G];
