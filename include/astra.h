@@ -77,6 +77,10 @@ extern "C" {
 #define ASTRA_FLAG_SERIAL_ISSUE   4ull   /* always take the cycle-serial issue path (testing)  */
 #define ASTRA_FLAG_NO_HEAVY        16ull  /* no warp-per-wavefront issue path (testing)         */
 #define ASTRA_FLAG_NO_PRIORITY_SWEEP 32ull /* budget-bound windows take the cycle-serial path (testing) */
+#define ASTRA_FLAG_RUN_AHEAD     64ull  /* one-CTA points of up to 32 nodes: no block barrier per window, a node starts its next
+                                         * window as soon as the nodes it depends on have completed the current one.  Same
+                                         * results; measured slower on B200 (config 4 +11 %: the barrier keeps the warps of a
+                                         * CTA in the same stage and so in the same instruction-cache lines), hence opt-in */
 #define ASTRA_FLAG_SERIAL_ARRIVALS 8ull  /* one task per in-link, no chunking (testing)        */
 #define ASTRA_FLAG_WARPS(w) (((uint64_t)(w) & 0x3full) << 20) /* CTA shape: w in {1,2,4,8,16} warps per CTA, 16/w CTAs per SM
                                             (0 = engine's choice) */

@@ -27,6 +27,7 @@ FLAG_SERIAL_ISSUE = 4          # testing: cycle-serial issue path everywhere
 FLAG_SERIAL_ARRIVALS = 8       # testing: one task per in-link
 FLAG_NO_HEAVY = 16             # testing: no warp-per-wavefront path
 FLAG_NO_PRIORITY_SWEEP = 32    # testing: budget-bound windows on the cycle-serial path
+FLAG_RUN_AHEAD = 64            # one-CTA points: nodes run ahead of the nodes they do not depend on (no barrier per window)
 
 
 def FLAG_WARPS(w: int) -> int:

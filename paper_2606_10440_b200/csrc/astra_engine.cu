@@ -63,6 +63,11 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 hint[3];        // min over everything pending of its next event time; slot seq % 3 is the window's (A7)
     u32 g_hint, g_acked, g_err, g_completion;   // group mode: the group-wide values after the window's group barrier
     u32 abort;          // a group barrier timed out somewhere: leave the kernel
+    // run-ahead windows (one-CTA points of up to 32 nodes, one node per warp set): no block barrier per window
+    u32 prog[32];       // windows completed by node (set) i
+    u32 shint[32][2];   // next-event hint of node i's current window (slot: window ordinal & 1)
+    u32 hint8[8];       // the point's hint per window ordinal & 7
+    u32 stop;           // 1 + final status once a node has decided that the run ends
 #ifdef ASTRA_DIAG
     u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows, [7] clocks on that path, [8] windows with such a GPU
     u64 sclk[16][8];    // per warp set (clocks of its first warp, summed over its nodes and windows): 0 arrivals+acks,
@@ -1299,13 +1304,13 @@ __device__ void wf_heavy(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 g, u3
         if (lane + 32 < na) { const u32 b = scr[96 + lane]; key1 = (((u32)__ldcg(&rec[b]) - t0) << 6) | b; }
         u32 r0 = 0, r1 = 0;
         if (na > 32) {
-#pragma unroll
+#pragma unroll 2
             for (u32 j = 0; j < 32; j++) {
                 const u32 k0 = __shfl_sync(FULL, key0, j), k1 = __shfl_sync(FULL, key1, j);
                 r0 += (k0 < key0) + (k1 < key0); r1 += (k0 < key1) + (k1 < key1);
             }
         } else if (na > 1) {
-#pragma unroll
+#pragma unroll 4
             for (u32 j = 0; j < 32; j++) r0 += __shfl_sync(FULL, key0, j) < key0;
         }
         if (lane < na) scr[r0] = key0;
@@ -2304,6 +2309,26 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
     node_tail(c, ctl, hp, v, k, t0, t1, cb, scr, lane, sw, ws, set, diag_lane, mode, e_l, n_l, lo_l, fl_l);
 }
 
+// Run-ahead windows: wait until the nodes of `pm` have completed `need_pred` windows and all nodes `need_all`.
+// Returns 0, or 1 + final status when the run has ended meanwhile (or an internal error / a time-out ends it).
+__device__ u32 wait_prog(Ctl& ctl, u32 lane, u32 n_nodes, u32 pm, u32 need_pred, u32 allm, u32 need_all) {
+    const long long start = clock64();
+#pragma unroll 1
+    for (u32 spins = 0;; spins++) {
+        const u32 p = lane < n_nodes ? *(volatile u32*)&ctl.prog[lane] : 0xffffffffu;
+        const u32 okp = __ballot_sync(FULL, p >= need_pred), oka = __ballot_sync(FULL, p >= need_all);
+        const u32 stop = *(volatile u32*)&ctl.stop;
+        if (stop) return stop;
+        if (*(volatile u32*)&ctl.err || ((spins & 0xfffu) == 0xfffu && clock64() - start > ASTRA_SPIN_CLOCKS)) {
+            if (lane == 0) { atomicOr(&ctl.err, 16u); atomicCAS(&ctl.stop, 0u, 1u + (u32)ASTRA_STATUS_INTERNAL); }
+            __syncwarp();
+            return 1u + (u32)ASTRA_STATUS_INTERNAL;
+        }
+        if ((okp & pm) == pm && (oka & allm) == allm) { __threadfence_block(); return 0u; }
+        __nanosleep(64);
+    }
+}
+
 __device__ __forceinline__ void
 step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
@@ -2434,6 +2459,79 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const u32 W = c.W;
         u64 busy = 0, skipped = 0;
         bool aborted = false;
+        // Run-ahead windows (ASTRA_FLAG_RUN_AHEAD; off by default, see include/astra.h).  Inside a window a node depends on nothing; between windows only on the nodes that feed
+        // its in-links and that receive its lines (predmask).  So there is no barrier per window: a node whose own
+        // pending events fall into the next window knows that window is the next one for everybody and starts it as
+        // soon as its predecessors have completed the current one (and every node the one before: buffers are sized
+        // for a distance of two windows).  A node without such an event waits for all nodes and takes the point's
+        // hint, as the barrier version does.  All nodes step through the same sequence of windows.
+        const bool run_ahead = P.run_ahead != 0u && group == 1u && nsets == n_nodes && n_nodes > 1u && n_nodes <= 32u;
+        if (run_ahead) {
+            if (tid < 32) ctl.prog[tid] = 0u;
+            if (tid < 8) ctl.hint8[tid] = ASTRA_T_INF;
+            if (tid == 0) ctl.stop = 0u;
+            __syncthreads();
+            if (in_set) {
+                const u32 pm = c.predmask[c.v_lo + set];
+                const u32 allm = n_nodes == 32u ? ~0u : (1u << n_nodes) - 1u;
+                const bool leader = sw == 0 && lane == 0;
+                u32 n = 0;                                  // ordinal of the window in the sequence all nodes step through
+#pragma unroll 1
+                for (;;) {
+                    const u64 t0l = (u64)k * W;
+                    if (t0l >= c.tmax) { if (leader) atomicCAS(&ctl.stop, 0u, 1u + (u32)ASTRA_STATUS_MAX_CYCLES); break; }
+                    const u32 t0 = (u32)t0l;
+                    const u32 t1 = (u32)min((u64)c.tmax, t0l + W);
+                    const u32 cb = t0 % c.NC;
+                    u32* const hp = &ctl.shint[set][n & 1u];
+#ifdef ASTRA_DIAG
+                    dck = clock64();
+#endif
+                    if (n > 0 && wait_prog(ctl, lane, n_nodes, pm, n, allm, n - 1u)) break;
+#ifdef ASTRA_DIAG
+                    if (leader) ctl.sclk[set][7] += (u64)(clock64() - dck);
+#endif
+                    if (leader) *hp = ASTRA_T_INF;
+                    set_sync(wset, set);
+                    busy += t1 - t0;
+                    node_window(c, ctl, hp, c.v_lo + set, k, t0, t1, cb, scr, lane, sw, wset, set, leader);
+                    set_sync(wset, set);
+                    const u32 own = *(volatile u32*)hp;
+                    if (leader) {
+                        atomicMin(&ctl.hint8[n & 7u], own);
+                        ctl.hint8[(n + 4u) & 7u] = ASTRA_T_INF;  // last read before anybody started window n - 2, next written after n + 3
+                        __threadfence_block();
+                        *(volatile u32*)&ctl.prog[set] = n + 1u;
+#ifdef ASTRA_DIAG
+                        if (set == 0) ctl.clk[0]++;
+#endif
+                    }
+                    const bool last = (u64)(k + 1) * W >= c.tmax;
+                    if (!last && own / W <= k + 1u) { k++; n++; continue; }      // the next window is k + 1 for everybody
+                    // the point's decision after this window, from what all nodes have posted
+#ifdef ASTRA_DIAG
+                    dck = clock64();
+#endif
+                    if (wait_prog(ctl, lane, n_nodes, 0u, 0u, allm, n + 1u)) break;
+#ifdef ASTRA_DIAG
+                    if (leader) ctl.sclk[set][7] += (u64)(clock64() - dck);
+#endif
+                    const u32 hint = *(volatile u32*)&ctl.hint8[n & 7u];
+                    int32_t st = -1;
+                    if (*(volatile u32*)&ctl.acked == c.S) st = ASTRA_STATUS_DONE;
+                    else if (*(volatile u32*)&ctl.err) st = ASTRA_STATUS_INTERNAL;
+                    else if (last) st = ASTRA_STATUS_MAX_CYCLES;       // events past the watchdog cut are not looked at
+                    else if (hint == ASTRA_T_INF) st = ASTRA_STATUS_DEADLOCK;
+                    if (st >= 0) { if (leader) atomicCAS(&ctl.stop, 0u, 1u + (u32)st); break; }
+                    u32 nk = k + 1;
+                    if (!(c.flags & (u32)ASTRA_FLAG_NO_WINDOW_SKIP)) nk = max(nk, hint / W);
+                    skipped += (u64)(nk - k - 1) * W;
+                    k = nk; n++;
+                }
+            }
+            __syncthreads();
+            status = (int32_t)ctl.stop - 1;
+        } else
         #pragma unroll 1
         for (;;) {
             const u64 t0l = (u64)k * W;

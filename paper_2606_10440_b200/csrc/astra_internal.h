@@ -50,7 +50,7 @@ typedef uint64_t u64;
     X(step_od) X(lines) X(cu_lo) X(cu_n) X(succ_ptr) X(succ) X(ndeps) \
     X(step_q) X(step_r) X(first_link) X(step_alpha) X(step_aq) X(step_ar) X(cul_ptr) X(cul) X(rel_off) X(init_rel) X(init_rel_cnt) \
     X(ev_off) X(ring_off) X(ring_mask) X(lkind) X(ceilb) X(lstate0_init) X(mask_off) X(pre_off) X(nz_off) X(classoff) \
-    X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(gflag) X(gdirect) X(lflag) X(lfwd) X(lscr_off)
+    X(nd_mw) X(nd_injoff) X(inj_off) X(part) X(predmask) X(gflag) X(gdirect) X(lflag) X(lfwd) X(lscr_off)
 
 // Mutable arrays of a design point.  X(name, element type, init) with init: 0 zero, 1 0xff bytes,
 // 2 written by the kernel's own initialisation, 3 scratch (no initialisation).
@@ -98,7 +98,8 @@ struct PointDesc {
     u32 CW, nwords, slots, bmwords;
     u32 Wcyc, NW, kdiv_magic, NC;              // Wcyc lookahead window in cycles; NW power of two; kdiv_magic = ceil(2^32 / K); NC = W + 1
     u32 flags, group;                          // group: CTAs cooperating on this point
-    u32 pcu, pad1;                             // pcu: ASTRA_GPU_ISSUE_PER_CU | ASTRA_GPU_CAP_PER_CU of the point's GPU model
+    u32 pcu, run_ahead;                        // pcu: ASTRA_GPU_ISSUE_PER_CU | ASTRA_GPU_CAP_PER_CU of the point's GPU model;
+                                               // run_ahead: buffers are sized for nodes two windows apart (one CTA, <= 32 nodes)
     u32 hot_bytes, alcap;                      // alcap: entries per (GPU, window bin) ack discovery list
     u64 max_cycles;
     u64 total_lines;

@@ -219,7 +219,13 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         u32 m = c.cu_n[s] * g.Wv;
         step_q[s] = c.lines[s] / m; step_r[s] = c.lines[s] % m;
     }
-    u64 nw64 = pow2ceil((u64)(alpha_max + W - 1) / W + 2);
+    // ASTRA_FLAG_RUN_AHEAD: one-CTA points of up to 32 nodes let a node run ahead of the nodes it does not depend on, at
+    // most two windows apart (step_kernel_body): one more window bin, 2 W ceil(B) more ring entries per link for the
+    // lagging reader.
+    bool run_ahead = group == 1 && V <= 32 && (opt.flags & ASTRA_FLAG_RUN_AHEAD);
+    if (run_ahead && pow2ceil((u64)(alpha_max + W - 1) / W + 3) > ASTRA_NW_MAX) run_ahead = false;     // no room for the extra bin
+    P.run_ahead = run_ahead ? 1u : 0u;
+    u64 nw64 = pow2ceil((u64)(alpha_max + W - 1) / W + (run_ahead ? 3 : 2));
     if (nw64 > ASTRA_NW_MAX) { err = "route latency / lookahead window ratio above the engine limit"; return ASTRA_ELIMIT; }
     P.NW = (u32)nw64;
 
@@ -335,7 +341,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         else if (256 % t.bw[e] == 0) { lkind[e] = ASTRA_LK_PERIOD | ((256 / t.bw[e]) << 2); lstate0[e] = 0; }   // next accept not before cycle 0
         else { lkind[e] = ASTRA_LK_GENERAL | (t.bw[e] << 2); lstate0[e] = ceilb * 256; }
         // a group's writer checks the ring against a reader cursor that may lag one window: 2x
-        u32 rc = std::max<u32>(32, pow2ceil(bound[e] * (group > 1 ? 2 : 1)));
+        u32 rc = std::max<u32>(32, pow2ceil(run_ahead ? bound[e] + 2ull * W * ceilb : bound[e] * (group > 1 ? 2 : 1)));
         if (ring_total + rc >= (1ull << 32)) { err = "ring space exceeds 2^32 entries"; return ASTRA_ELIMIT; }
         ring_off[e] = (u32)ring_total; ring_mask[e] = rc - 1; ring_total += rc;
         u32 v = t.tail[e];
@@ -442,6 +448,16 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         for (u32 x = 0; x < deg; x++) if (!multi[e0 + x]) gdirect[q] |= 1u << x;
     }
 
+    // predmask[v] (points of up to 32 nodes): the nodes whose window k - 1 must be complete before v starts window k --
+    // the tails of v's in-links (lines, due counts) and the destinations of the steps v owns (their arrival stage
+    // writes v's ack records and bins)
+    std::vector<u32> predmask(V, 0);
+    if (V <= 32) {
+        for (u32 e = 0; e < E; e++) predmask[t.head[e]] |= 1u << t.tail[e];
+        for (u32 s = 0; s < S; s++) predmask[c.owner[s]] |= 1u << c.dst[s];
+        for (u32 v = 0; v < V; v++) predmask[v] &= ~(1u << v);
+    }
+
     // constant tables
     u64* co = P.c_off;
     co[ASTRA_C_in_ptr] = topo_off[0]; co[ASTRA_C_in_link] = topo_off[1]; co[ASTRA_C_head] = topo_off[2];
@@ -463,6 +479,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
     co[ASTRA_C_classoff] = blob.add(classoff); co[ASTRA_C_nd_mw] = blob.add(nd_mw);
     co[ASTRA_C_nd_injoff] = blob.add(nd_injoff); co[ASTRA_C_inj_off] = blob.add(inj_off);
     co[ASTRA_C_part] = blob.add(part);
+    co[ASTRA_C_predmask] = blob.add(predmask);
     co[ASTRA_C_gflag] = blob.add(gflag);
     co[ASTRA_C_gdirect] = blob.add(gdirect);
     co[ASTRA_C_lflag] = blob.add(lflag); co[ASTRA_C_lfwd] = blob.add(lfwd);

@@ -12,6 +12,7 @@ from tests.parity import check_workload, compare_point
 pytestmark = pytest.mark.gpu
 
 FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_NO_HEAVY, FLAG_NO_PRIORITY_SWEEP = 1, 2, 4, 8, 16, 32
+FLAG_RUN_AHEAD = 64
 
 
 def _single(topo, coll, gpu, name="case", max_cycles=1 << 22):
@@ -100,7 +101,8 @@ def test_random_small_workloads(seed):
     check_workload(configs.random_workload(seed, n_points=4, max_gpus=6, max_steps=24, max_lines=200))
 
 
-@pytest.mark.parametrize("flags", [FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_NO_WINDOW_SKIP | FLAG_WINDOW_1])
+@pytest.mark.parametrize("flags", [FLAG_NO_WINDOW_SKIP, FLAG_WINDOW_1, FLAG_NO_WINDOW_SKIP | FLAG_WINDOW_1,
+                                   FLAG_RUN_AHEAD | FLAG_WINDOW_1 | 0x100, FLAG_RUN_AHEAD | FLAG_NO_WINDOW_SKIP | FLAG_WINDOW_1 | 0x100])
 def test_i8_skip_equivalence(flags):
     """I8: outputs with idle-cycle / window skipping == without, and with a 1-cycle window."""
     w = configs.random_workload(77, n_points=6, max_gpus=6, max_steps=24, max_lines=200)
@@ -108,10 +110,12 @@ def test_i8_skip_equivalence(flags):
     check_workload(configs.config1(), flags=flags)
 
 
-@pytest.mark.parametrize("flags", [FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_NO_HEAVY, FLAG_NO_PRIORITY_SWEEP, FLAG_SERIAL_ISSUE | FLAG_SERIAL_ARRIVALS | 0x100])
+@pytest.mark.parametrize("flags", [FLAG_SERIAL_ISSUE, FLAG_SERIAL_ARRIVALS, FLAG_NO_HEAVY, FLAG_NO_PRIORITY_SWEEP, FLAG_SERIAL_ISSUE | FLAG_SERIAL_ARRIVALS | 0x100,
+                                   FLAG_RUN_AHEAD, FLAG_RUN_AHEAD | 0x100, FLAG_RUN_AHEAD | FLAG_NO_WINDOW_SKIP | 0x100])
 def test_engine_paths_agree(flags):
     """The wavefront-parallel issue stage and the chunked arrival stage (defaults) and the cycle-serial /
-    one-task-per-link paths they fall back to give the same bits; 0x100 = one CTA per point."""
+    one-task-per-link paths they fall back to give the same bits; 0x100 = one CTA per point; RUN_AHEAD = no block
+    barrier per window, nodes run ahead of the nodes they do not depend on."""
     check_workload(configs.random_workload(91, n_points=6, max_gpus=6, max_steps=24, max_lines=200), flags=flags)
     check_workload(configs.config1(), flags=flags)
     check_workload(configs.config2(range(6, 8)), flags=flags, processes=4)
@@ -217,6 +221,21 @@ def test_i6_batch_independence():
         assert a[i][0].completion_cycle == b[j][0].completion_cycle
         assert (a[i][1] == b[j][1]).all() and (a[i][2] == b[j][2]).all()
     assert (a[5][1] == c[0][1]).all()
+
+
+@pytest.mark.parametrize("flags", [0, 0x100, FLAG_RUN_AHEAD | 0x100])
+def test_watchdog_cuts(flags):
+    """Runs cut by max_cycles at many points of the run (inside a window, at a window edge, at the completion cycle
+    and one before): status and every timestamp stamped before the cut equal the oracle's, with nodes running ahead
+    (one CTA per point, 0x100) and with the barrier per window."""
+    topo, coll, gpu = configs.config1().point(0)
+    for mc in (0, 1, 191, 192, 193, 5000, 38400, 38592, 38622, 38623, 38624, 38700):
+        check_workload(_single(topo, coll, gpu, max_cycles=mc), flags=flags)
+    w = configs.random_workload(12, n_points=1, max_gpus=6, max_steps=24, max_lines=200)
+    t2, c2, g2 = w.point(0)
+    full = check_workload(w, flags=flags)[0][0][0].completion_cycle
+    for mc in (full - 1, full, full + 1, full // 2, 7):
+        check_workload(_single(t2, c2, g2, max_cycles=max(0, mc)), flags=flags)
 
 
 def test_watchdog_and_edge_cases():
