@@ -68,6 +68,9 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 shint[32][2];   // next-event hint of node i's current window (slot: window ordinal & 1)
     u32 hint8[8];       // the point's hint per window ordinal & 7
     u32 stop;           // 1 + final status once a node has decided that the run ends
+    // link service by all warps of a set (link_service_set)
+    int ls_max[32];     // per warp: maximum of its block
+    u32 ls_acc[32], ls_last[32];   // per set: lines accepted, last acceptance cycle
 #ifdef ASTRA_DIAG
     u64 clk[16];        // [0] windows, [5] init clocks, [6] budget-bound GPU-windows, [7] clocks on that path, [8] windows with such a GPU
     u64 sclk[16][8];    // per warp set (clocks of its first warp, summed over its nodes and windows): 0 arrivals+acks,
@@ -337,9 +340,17 @@ __device__ __forceinline__ void link_inflight_hint(const Ctx& __restrict__ c, Ct
     const u32* dcb = &c.due_cnt[(size_t)e * c.NW];
     const u32 span = min(c.NW - 1, c.leff[e] / c.W + 2);
     u32 best = ASTRA_T_INF;
-    #pragma unroll 1
-    for (u32 j = span; j >= 1; j--)
-        if (ld_vol(&dcb[(k + j) & c.NWmask])) best = j;
+    {   // the first eight bins in flight together (the counts are other CTAs' writes in a group: volatile loads)
+        u32 dv[8];
+#pragma unroll
+        for (u32 q = 0; q < 8; q++) dv[q] = q < span ? ld_vol(&dcb[(k + q + 1) & c.NWmask]) : 0u;
+#pragma unroll
+        for (int q = 7; q >= 0; q--) if (dv[q]) best = (u32)q + 1u;
+    }
+    if (best == ASTRA_T_INF)
+#pragma unroll 1
+        for (u32 j = 9; j <= span; j++)
+            if (ld_vol(&dcb[(k + j) & c.NWmask])) { best = j; break; }
     if (best != ASTRA_T_INF) {
         const u64 tw = (u64)(k + best) * c.W;
         atomicMin(hp, tw >= ASTRA_T_INF ? ASTRA_T_INF - 1 : (u32)tw);
@@ -2073,6 +2084,100 @@ __device__ __forceinline__ void set_sync(u32 ws, u32 set) {
     else asm volatile("bar.sync %0, %1;" :: "r"(set + 1u), "r"(ws * 32u) : "memory");
 }
 
+// Link service of one link by all ws warps of a node's set (a GPU's one or two FIFOs of several hundred entries and
+// sixteen warps): warp r takes entries [128 r, 128 r + 128), the blocks' maxima are combined through shared memory.
+// Integer and 1/P bandwidths, single-feeder links, 129 .. 128 ws entries; anything else falls to one warp.
+__device__ void link_service_set(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 e, u32 k, u32 t0, u32 t1, u32 cb,
+                                 u32 lane, u32 sw, u32 ws, u32 set) {
+    const u32 wlen = t1 - t0;
+    const u32 fh = c.fifo_head[e], tl = c.ltail[e], tn = c.run[e];
+    const u32 n_back = tl - fh, n_tot = tn - fh;
+    const u32 lk = c.lkind[e];
+    const u32 kind = lk & 3u, param = lk >> 2;
+    const u32 scan_limit = min(n_tot, c.ceilb[e] * wlen);
+    if (kind == ASTRA_LK_GENERAL || scan_limit > 128u * ws || scan_limit <= 128u || c.dirty[e]) {
+        set_sync(ws, set);                  // every warp has taken this decision before warp 0 moves the link's cursors
+        if (sw == 0) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
+        return;
+    }
+    u64* ring = c.ring + c.ring_off[e];
+    const u32 rmask = c.ring_mask[e];
+    const u32 leff = c.leff[e];
+    const u32 lq = leff / c.W, lr = leff % c.W;
+    const int P = (int)param;
+    const u32 bmagic = 0xffffffffu / param + 1u;
+    int xn_rel = 0;
+    if (kind == ASTRA_LK_PERIOD) { const u32 xn = c.lstate0[e]; xn_rel = xn > t0 ? (int)(xn - t0) : 0; }
+    const u32 warp = threadIdx.x >> 5;
+    // phase 1: the block's entries, running maxima inside the lane, the block's maximum
+    const u32 j0 = 128u * sw + 4u * lane;
+    u64 fl[4]; int val[4]; bool act[4];
+    int m = INT_MIN;
+#pragma unroll
+    for (int q = 0; q < 4; q++) { act[q] = j0 + q < scan_limit; fl[q] = act[q] ? ring[(fh + j0 + q) & rmask] : 0ull; }
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        const u32 j = j0 + q;
+        const int a = (act[q] && j >= n_back) ? (int)((u32)(fl[q] >> ASTRA_FLIT_TIME_SHIFT) & 0x3ffu) : 0;
+        const int v = kind == ASTRA_LK_INT ? P * a - (int)j : a - P * (int)j;
+        m = act[q] ? max(m, v) : m;
+        val[q] = m;
+    }
+    const int incl = warp_incl_max(m, lane);
+    int excl = __shfl_up_sync(FULL, incl, 1);
+    if (lane == 0) excl = INT_MIN;
+    if (lane == 31) ctl.ls_max[warp] = incl;
+    set_sync(ws, set);
+    // phase 2: maxima of the blocks before this one, acceptance cycles, arrival stamps
+    {
+        const int bm = lane < sw ? ctl.ls_max[warp - sw + lane] : INT_MIN;
+        excl = max(excl, (int)__reduce_max_sync(FULL, bm));
+    }
+    u32 xx[4], cnt_acc = 0, xmax = 0;
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+        const u32 j = j0 + q;
+        const int pm = max(excl, val[q]);
+        xx[q] = kind == ASTRA_LK_INT ? (param == 1 ? (u32)((int)j + pm) : __umulhi((u32)((int)j + pm), bmagic)) : (u32)(P * (int)j + max(pm, xn_rel));
+        const bool acc = act[q] && xx[q] < wlen;
+        cnt_acc += acc;
+        if (acc) {
+            xmax = xx[q];
+            ring[(fh + j) & rmask] = (fl[q] & ASTRA_FLIT_PAYLOAD_MASK) | ((u64)((t0 + xx[q] + leff) & ASTRA_TMASK26) << ASTRA_FLIT_TIME_SHIFT);
+        } else xx[q] = 0xffffffffu;
+    }
+    const u32 tot_acc = __reduce_add_sync(FULL, cnt_acc);
+    if (tot_acc) {
+        const u32 x_first = __shfl_sync(FULL, xx[0], 0);       // acceptance is a prefix: the block's first entry is its first accepted one
+        const u32 x_last = __reduce_max_sync(FULL, xmax);
+        const u32 w_first = k + lq + (x_first + lr >= c.W ? 1u : 0u);
+        u32 c0 = 0;
+#pragma unroll
+        for (int q = 0; q < 4; q++) c0 += (xx[q] != 0xffffffffu) && (k + lq + (xx[q] + lr >= c.W ? 1u : 0u)) == w_first;
+        c0 = __reduce_add_sync(FULL, c0);
+        if (lane == 0) {
+            atomicAdd(&c.due_cnt[(size_t)e * c.NW + (w_first & c.NWmask)], c0);
+            if (tot_acc != c0) atomicAdd(&c.due_cnt[(size_t)e * c.NW + ((w_first + 1) & c.NWmask)], tot_acc - c0);
+            atomicAdd(&ctl.ls_acc[set], tot_acc);
+            atomicMax(&ctl.ls_last[set], x_last);
+            if (sw == 0) atomicMin(hp, t0 + x_first + leff);
+        }
+    }
+    set_sync(ws, set);
+    if (sw == 0 && lane == 0) {
+        const u32 n_acc = ctl.ls_acc[set], last_x = ctl.ls_last[set];
+        ctl.ls_acc[set] = 0u; ctl.ls_last[set] = 0u;
+        c.fifo_head[e] = fh + n_acc;
+        c.ltail[e] = tn;
+        if (n_acc) {
+            c.link_lines[e] += n_acc;
+            if (kind == ASTRA_LK_PERIOD) c.lstate0[e] = t0 + last_x + param;
+        }
+        if (n_tot > n_acc) atomicMin(hp, t1);
+        if (tn - ld_vol(&c.pipe_head[e]) > rmask + 1) atomicOr(&ctl.err, 1u);     // ring overflow guard
+    }
+}
+
 // The rest of a node's window after the issue decisions: placement of the window's issues (or the cycle-serial
 // issue path), merge into multi-feeder out-links, link service.  e_l .. fl_l: the node's first 32 in-links, one per
 // lane (id, lines due, read cursor, arrival path), as loaded by stage 1.
@@ -2161,6 +2266,11 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
         }
     }
     #pragma unroll 1
+    if (ws >= 8u * (e_hi - e_lo)) {                              // one or two links and many warps: every link by the whole set
+#pragma unroll 1
+        for (u32 e = e_lo; e < e_hi; e++) link_service_set(c, ctl, hp, e, k, t0, t1, cb, lane, sw, ws, set);
+    } else
+#pragma unroll 1
     for (u32 e = e_lo + sw; e < e_hi; e += ws) link_service(c, ctl, hp, e, k, t0, t1, cb, lane);
     DIAG_CLK(6);
 }
@@ -2390,6 +2500,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
             ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
+            for (int i = 0; i < 32; i++) { ctl.ls_acc[i] = 0u; ctl.ls_last[i] = 0u; }
             ctl.g_hint = ASTRA_T_INF; ctl.g_acked = 0; ctl.g_err = 0; ctl.g_completion = 0;
 #ifdef ASTRA_DIAG
             #pragma unroll 1
