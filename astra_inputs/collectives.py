@@ -264,3 +264,62 @@ def single_transfer(n_gpus: int, src: int, dst: int, lines: int, cu_lo: int, cu_
     b = CollectiveBuilder(n_gpus, f"p2p_{src}_{dst}_{lines}")
     b.add(src, dst, lines, cu_lo, cu_n)
     return b.build()
+
+
+# ---------------------------------------------------------------------------------------------
+# Control-path variants (PAPER.md:L137-138 SemaphoreAcquire / SemaphoreRelease,
+# L165 "only wavefront zero" issues control messages, L279-289 put vs get).  Both are transforms of
+# a step DAG into another step DAG: the control messages become one-line steps of their own, so
+# they queue in the same FIFOs and use the same links as the data (no method arithmetic here).
+# ---------------------------------------------------------------------------------------------
+def put_with_signal(coll: Collective) -> Collective:
+    """put + signal (PAPER.md:L279 "SemaphoreReleaseOp should follow after a remote Store", the
+    receiver "must run SemaphoreAcquireOp before" it goes on): every step p that some step waits
+    for with a DELIVERED dependency gets a SemaphoreRelease step right behind it -- one line from
+    wavefront zero of p's first CU (cu_n = 1: the one line falls to wavefront 0 of that CU, R11)
+    to the same destination, released when p's last line has been issued (ISSUED dependency on p)
+    -- and the waiting steps wait for the DELIVERED stamp of that signal instead of p's.  The
+    acquire is the local observation of the delivered semaphore line."""
+    from .types import DEP_ISSUED
+    S = coll.n_steps
+    waited = set()
+    for s in range(S):
+        for i in range(int(coll.dep_ptr[s]), int(coll.dep_ptr[s + 1])):
+            if int(coll.dep_kind[i]) == DEP_DELIVERED:
+                waited.add(int(coll.dep_step[i]))
+    b = CollectiveBuilder(coll.n_gpus, coll.name + "+signal")
+    new_id, sig_id = {}, {}
+    for s in range(S):
+        deps = []
+        for i in range(int(coll.dep_ptr[s]), int(coll.dep_ptr[s + 1])):
+            p, kind = int(coll.dep_step[i]), int(coll.dep_kind[i])
+            deps.append((sig_id[p], DEP_DELIVERED) if kind == DEP_DELIVERED else (new_id[p], kind))
+        new_id[s] = b.add(coll.owner[s], coll.dst[s], coll.lines[s], coll.cu_lo[s], coll.cu_n[s], deps)
+        if s in waited:
+            sig_id[s] = b.add(coll.owner[s], coll.dst[s], 1, coll.cu_lo[s], 1, [(new_id[s], DEP_ISSUED)])
+    return b.build()
+
+
+def as_get(coll: Collective, chunk_lines: int = 0) -> Collective:
+    """get ("requests to the remote GPU to send data"): every transfer p = (o -> d, n
+    lines) is initiated by its destination.  d sends a one-line request to o from wavefront zero of
+    p's first CU (posted as early as p's own dependencies on d allow: none here, the request is
+    free), and o's response carries the data, released when the request has been DELIVERED at o and
+    p's original dependencies hold.  With chunk_lines > 0 a transfer is cut into chunks of that many
+    lines, one request each (the reading taken: one request per chunk, not per line)."""
+    S = coll.n_steps
+    b = CollectiveBuilder(coll.n_gpus, coll.name + "+get")
+    last_id = {}                                  # original step -> all its response chunk steps
+    for s in range(S):
+        o, d, n = int(coll.owner[s]), int(coll.dst[s]), int(coll.lines[s])
+        base = []
+        for i in range(int(coll.dep_ptr[s]), int(coll.dep_ptr[s + 1])):
+            p, kind = int(coll.dep_step[i]), int(coll.dep_kind[i])
+            base += [(q, kind) for q in last_id[p]]
+        sizes = [n] if chunk_lines <= 0 else [min(chunk_lines, n - x) for x in range(0, n, chunk_lines)]
+        ids = []
+        for m in sizes:
+            req = b.add(d, o, 1, coll.cu_lo[s], 1)
+            ids.append(b.add(o, d, m, coll.cu_lo[s], coll.cu_n[s], base + [(req, DEP_DELIVERED)]))
+        last_id[s] = ids
+    return b.build()
