@@ -1666,16 +1666,28 @@ __device__ void ev_place(const Ctx& __restrict__ c, Ctl& ctl, u32 g, u32 chunk, 
         o = c.first_link[s];
     }
     if (!act) return;
-    // rank among the issues of the same cycle (j) and among those that take the same out-link (jo); a bucket
-    // holds at most H records, each with its wavefront id and out-link (bits 48.. of the record)
+    // rank among the issues of the same cycle (j) and, for a single-feeder out-link of a GPU with several, among those
+    // that take the same out-link (jo); a bucket holds at most H records, each with its wavefront id and out-link
+    // (bits 48.. of the record).  The budget-bound sweep writes its buckets in wavefront order already (nheavy marks it).
     u32 j = 0, jo = 0;
     const u32 oxm = o - e0;
-    #pragma unroll 1
-    for (u32 x = 0; x < n; x++) {
-        const u64 r2 = bucket[x];
-        const bool lower = (((u32)r2 >> 20) & 0xfffu) < wf;
-        j += lower;
-        jo += lower && (u32)(r2 >> 48) == oxm;
+    const bool need_jo = deg > 1 && c.mask_off[o] == ASTRA_NONE32;
+    if (c.nheavy[g] == ASTRA_NONE32) {
+        j = i - st;
+        if (need_jo)
+#pragma unroll 1
+            for (u32 x = 0; x < j; x++) jo += (u32)(bucket[x] >> 48) == oxm;
+    } else if (need_jo) {
+#pragma unroll 1
+        for (u32 x = 0; x < n; x++) {
+            const u64 r2 = bucket[x];
+            const bool lower = (((u32)r2 >> 20) & 0xfffu) < wf;
+            j += lower;
+            jo += lower && (u32)(r2 >> 48) == oxm;
+        }
+    } else {
+#pragma unroll 1
+        for (u32 x = 0; x < n; x++) j += (((u32)bucket[x] >> 20) & 0xfffu) < wf;
     }
     if (deg == 1) jo = j;
     const u32 d = tt + 1;
@@ -2410,7 +2422,7 @@ __device__ void node_window(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v,
                 wf_priority_word(c, ctl, hp, g, wi, k, t0, t1, scr, ws > 1 ? &c.turn[g] : nullptr, lane);
             }
             set_sync(ws, set);
-            if (sw == 0) gpu_finalize(c, g, k, wlen, lane);
+            if (sw == 0) { gpu_finalize(c, g, k, wlen, lane); if (lane == 0) c.nheavy[g] = ASTRA_NONE32; }     // buckets are in wavefront order (ev_place)
         }
         set_sync(ws, set);
         mode = c.gmode[g];

@@ -320,15 +320,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         const double t_run = std::max(t_bw, t_win);
         for (u32 e = 0; e < E; e++) {
             const double cb_ = std::max(1.0, t.bw[e] / 256.0);
-#if defined(ASTRA_X_SPARSE_ALL)
-            sparse_cells[e] = 1;
-#elif defined(ASTRA_X_SPARSE_NONE)
-            sparse_cells[e] = 0;
-#elif defined(ASTRA_X_SPARSE_T)
-            sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < ASTRA_X_SPARSE_T;
-#else
             sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < 0.125;
-#endif
         }
     }
     std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), nz_off(E, ASTRA_NONE32), inj_off(G + 1, 0);
