@@ -323,3 +323,27 @@ def as_get(coll: Collective, chunk_lines: int = 0) -> Collective:
             ids.append(b.add(o, d, m, coll.cu_lo[s], coll.cu_n[s], base + [(req, DEP_DELIVERED)]))
         last_id[s] = ids
     return b.build()
+
+
+def with_barriers(coll: Collective, cus: int, scope: str = "workgroup", kind: int = 2) -> Collective:
+    """NopOp / BarrierOp / memory fence between the operations of a GPU ("halts the
+    execution of a workgroup until all its wavefronts reach this operation", BarrierOp "inter-workgroup
+    synchronization"; L150 MemcpyOp "Waitcnt ... to enforce a memory fence") as dependencies between the
+    steps a GPU owns: every step waits for the previous step on each of its CUs (scope "workgroup": NopOp
+    between the operations of a workgroup) or for the previous step of every CU of the GPU (scope "gpu":
+    BarrierOp).  kind 2 (ISSUED): the wavefronts have dispatched all requests of the previous operation;
+    kind 1 (ACKED): its requests have also completed (Waitcnt 0, a fence).  `cus` = CUs per GPU."""
+    S = coll.n_steps
+    b = CollectiveBuilder(coll.n_gpus, coll.name + f"+{scope}_barriers{kind}")
+    last = [[-1] * cus for _ in range(coll.n_gpus)]        # last step seen on (GPU, CU)
+    for s in range(S):
+        o, lo, cn = int(coll.owner[s]), int(coll.cu_lo[s]), int(coll.cu_n[s])
+        deps = [(int(coll.dep_step[i]), int(coll.dep_kind[i])) for i in range(int(coll.dep_ptr[s]), int(coll.dep_ptr[s + 1]))]
+        rng = range(lo, lo + cn) if scope == "workgroup" else range(cus)
+        prev = sorted({last[o][cu] for cu in rng if last[o][cu] >= 0})
+        deps += [(p, kind) for p in prev if (p, kind) not in deps]
+        sid = b.add(o, coll.dst[s], coll.lines[s], lo, cn, deps)
+        assert sid == s
+        for cu in range(lo, lo + cn):
+            last[o][cu] = s
+    return b.build()

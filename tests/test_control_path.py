@@ -9,7 +9,7 @@ import numpy as np
 import pytest
 
 from astra_inputs import GpuCfg, Workload, collectives as C, configs, topologies as T
-from astra_inputs.types import CollectiveBuilder, DEP_DELIVERED, DEP_ISSUED
+from astra_inputs.types import CollectiveBuilder, DEP_ACKED, DEP_DELIVERED, DEP_ISSUED
 from oracle import oracle
 
 GOLD = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "pins_control_path.json")))
@@ -30,6 +30,21 @@ def _two_step_case():
     return topo, b.build(), GpuCfg(1, 1, 64, 1)
 
 
+def _barrier_cases():
+    """(key in the golden file, variant name, topology, collective, GPU) of the NopOp / BarrierOp / fence hand traces."""
+    topo = T.Topology.from_edges(2, 0, [0, 0], [(0, 1, 1024, 3), (1, 0, 1024, 3)])
+    b = CollectiveBuilder(2, "ab"); b.add(0, 1, 5, 0, 1); b.add(0, 1, 4, 0, 1)
+    ab, g1 = b.build(), GpuCfg(1, 2, 64, 2)
+    b = CollectiveBuilder(2, "xyz"); b.add(0, 1, 4, 0, 1); b.add(0, 1, 2, 1, 1); b.add(0, 1, 2, 1, 1)
+    xyz, g2 = b.build(), GpuCfg(2, 1, 64, 2)
+    return [("S4_nop_and_fence", "plain", topo, ab, g1),
+            ("S4_nop_and_fence", "nop", topo, C.with_barriers(ab, 1, "workgroup", DEP_ISSUED), g1),
+            ("S4_nop_and_fence", "fence", topo, C.with_barriers(ab, 1, "workgroup", DEP_ACKED), g1),
+            ("S5_barrier_scope", "plain", topo, xyz, g2),
+            ("S5_barrier_scope", "workgroup", topo, C.with_barriers(xyz, 2, "workgroup", DEP_ISSUED), g2),
+            ("S5_barrier_scope", "gpu", topo, C.with_barriers(xyz, 2, "gpu", DEP_ISSUED), g2)]
+
+
 def _transformed_workloads():
     """Small workloads for engine-vs-oracle parity: every named family with both transforms."""
     out = []
@@ -43,6 +58,9 @@ def _transformed_workloads():
     for i in range(w4.n_points):
         t4, c4, g4 = w4.point(i)
         out += [_single(t4, C.put_with_signal(c4), g4), _single(t4, C.as_get(c4), g4)]
+    out += [_single(topo, C.with_barriers(coll, gpu.cus, "workgroup", DEP_ISSUED), gpu), _single(topo, C.with_barriers(coll, gpu.cus, "gpu", DEP_ACKED), gpu)]
+    t2, c2, g2 = w2.point(1)
+    out += [_single(t2, C.with_barriers(c2, g2.cus, "workgroup", DEP_ACKED), g2), _single(t2, C.with_barriers(c2, g2.cus, "gpu", DEP_ISSUED), g2)]
     for seed in (3, 4, 5):
         wr = configs.random_workload(seed, n_points=2, max_gpus=6, max_steps=16, max_lines=120)
         for i in range(wr.n_points):
@@ -112,6 +130,13 @@ def test_get_hand_trace():
     assert r.step_ts.astype(np.int64).tolist() == g["step_ts"]
 
 
+def test_barrier_hand_traces():
+    """NopOp (ISSUED), fence (ACKED) and BarrierOp (GPU scope) as dependencies between a GPU's own steps."""
+    for key, name, topo, coll, gpu in _barrier_cases():
+        r = oracle.run_workload(_single(topo, coll, gpu))[0]
+        assert r.status == 0 and r.step_ts.astype(np.int64).tolist() == GOLD[key][name], (key, name)
+
+
 def test_ring_signal_closed_form():
     """T = 14 (350 + n/4) + 13 + 350: one more accept slot per signalled ring step (derivation in the golden file)."""
     w2 = configs.config2(range(6, 10))
@@ -149,6 +174,9 @@ def test_engine_matches_hand_traces():
         summ, ts, _ = simulate_workload(_single(topo, cc, gpu))[0]
         assert summ.status == 0 and summ.completion_cycle == GOLD[key]["completion"]
         assert ts.astype(np.int64).tolist() == GOLD[key]["step_ts"]
+    for key, name, topo, cc, gpu in _barrier_cases():
+        summ, ts, _ = simulate_workload(_single(topo, cc, gpu))[0]
+        assert summ.status == 0 and ts.astype(np.int64).tolist() == GOLD[key][name], (key, name)
 
 
 @pytest.mark.gpu
