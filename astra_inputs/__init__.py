@@ -12,10 +12,10 @@ own workloads are synthetic collectives on a generic power-of-two GPU
 """
 from .types import Topology, Collective, GpuCfg, Workload, DEP_DELIVERED, DEP_ACKED, DEP_ISSUED
 from .rng import SplitMix64, config_seed
-from . import topologies, collectives, configs
+from . import topologies, collectives, configs, noc
 
 __all__ = [
     "Topology", "Collective", "GpuCfg", "Workload",
     "DEP_DELIVERED", "DEP_ACKED", "DEP_ISSUED",
-    "SplitMix64", "config_seed", "topologies", "collectives", "configs",
+    "SplitMix64", "config_seed", "topologies", "collectives", "configs", "noc",
 ]

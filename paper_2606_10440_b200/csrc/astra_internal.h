@@ -29,7 +29,7 @@ typedef uint64_t u64;
 #endif
 #define ASTRA_HOT_BUDGET_SINGLE (48u << 10)  // bytes of shared memory for hot arrays, batches of one-CTA points (the rest of the SM's 256 KB is L1)
 #define ASTRA_HOT_BUDGET_GROUPS (64u << 10)  // ... batches with CTA groups
-#define ASTRA_NW_MAX 256                  // ack window bins per GPU
+#define ASTRA_NW_MAX 4096                 // window bins per GPU and per link (route latency / lookahead window + 2, rounded up to a power of two)
 #define ASTRA_ACK_LIST_CAP 4096u           // ack discovery list entries per (GPU, window bin); beyond: bitmap scan
 #define ASTRA_HEAVY_MIN 8u                // possible issues in a window from which a wavefront gets a warp of its own
 #define ASTRA_HEAVY_MAX_PER_WORD 16        // more such wavefronts among 32 consecutive ones: they stay on their threads
