@@ -2277,7 +2277,6 @@ __device__ void node_tail(const Ctx& __restrict__ c, Ctl& ctl, u32* hp, u32 v, u
             if (fl != 0u) { c.pipe_head[e] += n; c.tl_base[e] = 0; }
         }
     }
-    #pragma unroll 1
     if (ws >= 8u * (e_hi - e_lo)) {                              // one or two links and many warps: every link by the whole set
 #pragma unroll 1
         for (u32 e = e_lo; e < e_hi; e++) link_service_set(c, ctl, hp, e, k, t0, t1, cb, lane, sw, ws, set);

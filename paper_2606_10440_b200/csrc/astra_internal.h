@@ -27,12 +27,19 @@ typedef uint64_t u64;
 #ifndef ASTRA_WMAX
 #define ASTRA_WMAX 512u                   // cap of the lookahead window in cycles (< 1024: 10-bit cycle fields in the flit)
 #endif
+#ifndef ASTRA_HOT_BUDGET_SINGLE
 #define ASTRA_HOT_BUDGET_SINGLE (48u << 10)  // bytes of shared memory for hot arrays, batches of one-CTA points (the rest of the SM's 256 KB is L1)
+#endif
 #define ASTRA_HOT_BUDGET_GROUPS (64u << 10)  // ... batches with CTA groups
 #define ASTRA_NW_MAX 4096                 // window bins per GPU and per link (route latency / lookahead window + 2, rounded up to a power of two)
 #define ASTRA_ACK_LIST_CAP 4096u           // ack discovery list entries per (GPU, window bin); beyond: bitmap scan
+#ifndef ASTRA_HEAVY_MIN
 #define ASTRA_HEAVY_MIN 8u                // possible issues in a window from which a wavefront gets a warp of its own
+#endif
 #define ASTRA_HEAVY_MAX_PER_WORD 16        // more such wavefronts among 32 consecutive ones: they stay on their threads
+#ifndef ASTRA_SPARSE_CELLS_BELOW
+#define ASTRA_SPARSE_CELLS_BELOW 0.125    // expected share of non-empty cells under which a multi-feeder link keeps a bitmap of them
+#endif
 #define ASTRA_LF_DELIVER_ONLY 1u           // lflag: every line over the link terminates at its head
 #define ASTRA_LF_FORWARD_ONLY 2u           // lflag: every line over the link goes on to the single-feeder link lfwd[e]
 #define ASTRA_LF_CELLS 3u                  // lflag: lines terminate at the head or go on to multi-feeder links only (cells)

@@ -320,7 +320,7 @@ int32_t astra_plan_point(const HostTopo& t, const HostColl& c, const HostGpu& g,
         const double t_run = std::max(t_bw, t_win);
         for (u32 e = 0; e < E; e++) {
             const double cb_ = std::max(1.0, t.bw[e] / 256.0);
-            sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < 0.125;
+            sparse_cells[e] = (double)via_tot[e] / (cb_ * t_run) < ASTRA_SPARSE_CELLS_BELOW;
         }
     }
     std::vector<u32> ring_off(E), ring_mask(E), lkind(E), ceilb_v(E), lstate0(E), mask_off(E), pre_off(E), nz_off(E, ASTRA_NONE32), inj_off(G + 1, 0);
