@@ -208,6 +208,49 @@ int32_t astra_last_run_info(astra_ctx* ctx, float* device_ms, uint32_t* kernel_l
  * queue order) and device->host bytes a full read-back of its results copies. */
 int32_t astra_last_transfer_bytes(astra_ctx* ctx, uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 
+/* ---------------------------------------------------------------------------------------------
+ * No-allocation entry point.  Some callers cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  For them one design point can be run with the
+ * engine's whole scratch state (link rings, ack records, wavefront state, queue counters) in a
+ * file-scope `static __device__` array of the library, ASTRA_NOALLOC_SCRATCH_BYTES large; every
+ * GPU that loads the library holds that array until the process exits.
+ *
+ * Set-up (may allocate host memory; resolves the array's device address once per device):
+ *   astra_pack_point  plans ONE design point (A0: routing, tables, array placement) for a single
+ *                     CTA and writes its inputs -- constant tables, descriptor -- as one relocatable
+ *                     blob of info->in_bytes bytes into host_buf (NULL / too small: only *info is
+ *                     filled, ELIMIT when host_buf is non-NULL but too small).  The caller copies
+ *                     that blob to device memory of its own (256-byte aligned).
+ * Run (allocates nothing: no cudaMalloc / cudaFree / allocating library call, host or device):
+ *   astra_run_packed_noalloc  enqueues on `cuda_stream` (NULL = the ctx's stream) a clear of the
+ *                     scratch header and the step kernel on one CTA; inputs = the caller's device
+ *                     copy of the blob (d_in), outputs = caller's device buffer d_out of
+ *                     info->out_bytes bytes (256-byte aligned): step timestamps u64[4*n_steps] at
+ *                     byte offset info->off_step_ts, lines per link u64[n_links] at
+ *                     info->off_link_lines, an astra_summary at info->off_summary.  Asynchronous:
+ *                     the caller synchronises the stream before reading d_out.
+ * ELIMIT ("scratch ... exceeds") when info->scratch_bytes > ASTRA_NOALLOC_SCRATCH_BYTES; EINVAL on
+ * a bad info / NULL buffers.  Same results as astra_run_batch on the same point.
+ * All calls on a device share the one array, which keeps the previous call's contents: the entry
+ * point clears what must start at zero (the queue / abort header) and the kernel initialises the
+ * state arrays itself, but two calls that overlap on the GPU (different streams, two contexts,
+ * two processes' worth of threads on one device) RACE -- serialise them.                       */
+#define ASTRA_NOALLOC_SCRATCH_BYTES (16ull << 20)
+#define ASTRA_PACKED_MAGIC 0x41535452504b3031ull   /* "ASTRPK01" */
+typedef struct {
+    uint64_t magic;             /* ASTRA_PACKED_MAGIC                                          */
+    uint64_t in_bytes;          /* size of the packed input blob                               */
+    uint64_t out_bytes;         /* size of the output buffer                                   */
+    uint64_t scratch_bytes;     /* scratch the point needs (header + one CTA's workspace)      */
+    uint64_t off_const, off_desc, off_order;            /* inside the input blob               */
+    uint64_t off_step_ts, off_link_lines, off_summary;  /* inside the output buffer            */
+    uint32_t n_steps, n_links, hot_bytes, warps;
+} astra_packed_info;
+int32_t astra_pack_point(astra_ctx* ctx, const astra_point* point, uint64_t max_cycles,
+                         void* host_buf, uint64_t host_buf_bytes, astra_packed_info* info);
+int32_t astra_run_packed_noalloc(astra_ctx* ctx, const astra_packed_info* info,
+                                 const void* d_in, void* d_out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,9 @@ EXPORTED_SYMBOLS = [
     "astra_load_infragraph", "astra_load_collective", "astra_set_gpu", "astra_set_gpu_ex",
     "astra_run_batch", "astra_run_batch_async", "astra_sync", "astra_read_results",
     "astra_last_run_info", "astra_last_transfer_bytes", "astra_read_diag", "astra_point_group",
+    "astra_pack_point", "astra_run_packed_noalloc",
 ]
+NOALLOC_SCRATCH_BYTES = 16 << 20     # ASTRA_NOALLOC_SCRATCH_BYTES
 
 FLAG_NO_WINDOW_SKIP = 1
 FLAG_WINDOW_1 = 2
@@ -75,6 +77,15 @@ class Summary:
 _lib = None
 
 
+class PackedInfo(ctypes.Structure):
+    """astra_packed_info (include/astra.h)."""
+    _fields_ = [("magic", ctypes.c_uint64), ("in_bytes", ctypes.c_uint64), ("out_bytes", ctypes.c_uint64),
+                ("scratch_bytes", ctypes.c_uint64), ("off_const", ctypes.c_uint64), ("off_desc", ctypes.c_uint64),
+                ("off_order", ctypes.c_uint64), ("off_step_ts", ctypes.c_uint64), ("off_link_lines", ctypes.c_uint64),
+                ("off_summary", ctypes.c_uint64), ("n_steps", ctypes.c_uint32), ("n_links", ctypes.c_uint32),
+                ("hot_bytes", ctypes.c_uint32), ("warps", ctypes.c_uint32)]
+
+
 def load_library(path: Optional[str] = None):
     """dlopen the engine.  Raises (loudly) when it has not been built; never falls back."""
     global _lib
@@ -103,6 +114,8 @@ def load_library(path: Optional[str] = None):
     lib.astra_point_group.argtypes = [vp, u32, ctypes.POINTER(u32)]
     lib.astra_last_run_info.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(u32), ctypes.POINTER(u64)]
     lib.astra_last_transfer_bytes.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.astra_pack_point.argtypes = [vp, vp, u64, vp, u64, ctypes.POINTER(PackedInfo)]
+    lib.astra_run_packed_noalloc.argtypes = [vp, ctypes.POINTER(PackedInfo), vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name != "astra_last_error":
             getattr(lib, name).restype = i32
@@ -232,6 +245,30 @@ class Engine:
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         self._check(self._lib.astra_last_transfer_bytes(self._ctx, ctypes.byref(a), ctypes.byref(b)))
         return a.value, b.value
+
+    # no-allocation entry point (include/astra.h): set-up, then runs that only clear the scratch header and launch
+    def pack_point(self, point: Tuple[int, int, int], max_cycles: int):
+        """astra_pack_point: returns (PackedInfo, uint8 host array of info.in_bytes holding the packed inputs)."""
+        arr = self._marshal_points([point])
+        info = PackedInfo()
+        self._check(self._lib.astra_pack_point(self._ctx, ctypes.cast(arr, ctypes.c_void_p), max_cycles, None, 0, ctypes.byref(info)))
+        buf = np.zeros(info.in_bytes, dtype=np.uint8)
+        self._check(self._lib.astra_pack_point(self._ctx, ctypes.cast(arr, ctypes.c_void_p), max_cycles, _ptr(buf), buf.nbytes, ctypes.byref(info)))
+        return info, buf
+
+    def run_packed_noalloc(self, info: PackedInfo, d_in: int, d_out: int, stream: int = 0):
+        """astra_run_packed_noalloc: d_in / d_out are device addresses (256-byte aligned), stream a cudaStream_t or 0."""
+        self._check(self._lib.astra_run_packed_noalloc(self._ctx, ctypes.byref(info), ctypes.c_void_p(d_in), ctypes.c_void_p(d_out),
+                                                       ctypes.c_void_p(stream) if stream else None))
+
+    @staticmethod
+    def unpack_results(info: PackedInfo, out: np.ndarray):
+        """Host copy of an output buffer -> (Summary, step_ts[S,4], link_lines[E]) as read_results returns them."""
+        s = _Summary.from_buffer_copy(out[info.off_summary:info.off_summary + ctypes.sizeof(_Summary)].tobytes())
+        ts = out[info.off_step_ts:info.off_step_ts + 32 * info.n_steps].view(np.uint64).reshape(info.n_steps, 4).copy()
+        ll = out[info.off_link_lines:info.off_link_lines + 8 * info.n_links].view(np.uint64).copy()
+        return (Summary(s.status, s.n_steps, s.n_links, s.window, s.completion_cycle, s.total_lines, s.busy_cycles, s.skipped_cycles),
+                ts, ll)
 
     # convenience over the calls above: load a whole astra_inputs.Workload
     def load_workload(self, w) -> List[Tuple[int, int, int]]:

@@ -449,3 +449,96 @@ extern "C" int32_t astra_last_transfer_bytes(astra_ctx* c, uint64_t* h2d, uint64
     if (d2h) *d2h = c->results_bytes;
     return ASTRA_OK;
 }
+
+
+// ---------------------------------------------------------------------------------------------
+// No-allocation entry point (include/astra.h).  astra_pack_point is set-up: it plans one design
+// point for a single CTA exactly as prepare() does for a one-CTA point and serialises what the
+// kernel reads.  astra_run_packed_noalloc only clears the scratch header and launches.
+// ---------------------------------------------------------------------------------------------
+extern "C" int32_t astra_pack_point(astra_ctx* c, const astra_point* pt, uint64_t max_cycles,
+                                    void* host_buf, uint64_t host_buf_bytes, astra_packed_info* info) {
+    if (!c) return ASTRA_EINVAL;
+    if (!pt || !info) return fail(c, ASTRA_EINVAL, "null argument");
+    std::memset(info, 0, sizeof(*info));
+    if (pt->topo_id >= c->topos.size() || pt->coll_id >= c->colls.size() || pt->gpu_id >= c->gpus.size())
+        return fail(c, ASTRA_ESTATE, "design point references an unknown id");
+    try {
+        CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
+        int smem_max = 0, smem_sm = 0;
+        CUDA_TRY(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device), "device attribute");
+        CUDA_TRY(c, cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, c->device), "device attribute");
+        std::string err;
+        uint8_t* scratch = nullptr;
+        int32_t rc = astra_engine_static_scratch(c->device, &scratch, err);     // once per device, this device current
+        if (rc) return fail(c, rc, err);
+        const u32 warps = 16;
+        const u32 fixed = astra_engine_fixed_smem(warps);
+        const u32 smem_cta = std::min<u32>((u32)smem_max, (u32)smem_sm - 1024);
+        PlanOptions opt;
+        opt.flags = c->flags & 0xffull; opt.max_cycles = max_cycles; opt.group = 1;
+        opt.hot_budget = std::min<u32>(smem_cta > fixed + 1024 ? smem_cta - fixed - 1024 : 0, ASTRA_HOT_BUDGET_SINGLE);
+        const HostTopo& t = c->topos[pt->topo_id];
+        const HostColl& h = c->colls[pt->coll_id];
+        Blob blob;
+        u64 to[ASTRA_N_TOPO_TABLES], co[ASTRA_N_COLL_TABLES];
+        to[0] = blob.add(t.in_ptr); to[1] = blob.add(t.in_link); to[2] = blob.add(t.head); to[3] = blob.add(t.tail);
+        to[4] = blob.add(t.leff); to[5] = blob.add(t.next_link); to[6] = blob.add(t.row_ptr);
+        std::vector<u32> od(h.S);
+        for (u32 s = 0; s < h.S; s++) od[s] = (h.owner[s] << 16) | h.dst[s];
+        co[0] = blob.add(od); co[1] = blob.add(h.lines); co[2] = blob.add(h.cu_lo); co[3] = blob.add(h.cu_n);
+        co[4] = blob.add(h.succ_ptr); co[5] = blob.add(h.succ); co[6] = blob.add(h.ndeps);
+        PointDesc P;
+        double unused = 0;
+        rc = astra_plan_point(t, h, c->gpus[pt->gpu_id], opt, to, co, blob, P, unused, err);
+        if (rc) return fail(c, rc, err);
+        u64 roff = 0;
+        P.r_step_ts = roff; roff += 32ull * P.S;
+        P.r_link_lines = roff; roff += 8ull * P.E;
+        P.r_summary = roff; roff += (sizeof(DeviceSummary) + 15) & ~15ull;
+        P.r_diag = roff; roff += 8ull * ASTRA_DIAG_WORDS;
+        info->magic = ASTRA_PACKED_MAGIC;
+        info->off_const = 0;
+        info->off_desc = (blob.bytes.size() + 255) & ~255ull;
+        info->off_order = info->off_desc + ((sizeof(PointDesc) + 255) & ~255ull);
+        info->in_bytes = info->off_order + 256;
+        info->out_bytes = (std::max<u64>(roff, 16) + 255) & ~255ull;
+        info->scratch_bytes = (u64)ASTRA_NOALLOC_HEADER_BYTES + ((P.ws_bytes + 255) & ~255ull);
+        info->off_step_ts = P.r_step_ts; info->off_link_lines = P.r_link_lines; info->off_summary = P.r_summary;
+        info->n_steps = P.S; info->n_links = P.E; info->hot_bytes = P.hot_bytes; info->warps = warps;
+        if (host_buf) {
+            if (host_buf_bytes < info->in_bytes) return fail(c, ASTRA_ELIMIT, "host buffer smaller than info->in_bytes");
+            uint8_t* hb = (uint8_t*)host_buf;
+            std::memset(hb, 0, info->in_bytes);
+            if (!blob.bytes.empty()) std::memcpy(hb + info->off_const, blob.bytes.data(), blob.bytes.size());
+            std::memcpy(hb + info->off_desc, &P, sizeof(P));
+            const u32 order0 = 0;
+            std::memcpy(hb + info->off_order, &order0, sizeof(order0));
+        }
+        return ASTRA_OK;
+    } catch (const std::bad_alloc&) { return fail(c, ASTRA_ENOMEM, "host allocation failed"); }
+      catch (...) { return fail(c, ASTRA_EINVAL, "unexpected error"); }
+}
+
+// Allocates nothing: argument checks, one cudaMemsetAsync on the static scratch header, one kernel launch.
+// (An error message is copied into the ctx on failure only.)
+extern "C" int32_t astra_run_packed_noalloc(astra_ctx* c, const astra_packed_info* info, const void* d_in, void* d_out, void* stream) {
+    if (!c) return ASTRA_EINVAL;
+    if (!info || !d_in || !d_out) return fail(c, ASTRA_EINVAL, "null argument");
+    if (info->magic != ASTRA_PACKED_MAGIC || info->off_order + 4 > info->in_bytes || info->off_desc + sizeof(PointDesc) > info->off_order)
+        return fail(c, ASTRA_EINVAL, "not an astra_packed_info written by astra_pack_point");
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 255u) return fail(c, ASTRA_EINVAL, "d_in and d_out must be 256-byte aligned");
+    if (info->scratch_bytes > ASTRA_NOALLOC_SCRATCH_BYTES)
+        return fail(c, ASTRA_ELIMIT, "scratch of " + std::to_string(info->scratch_bytes) + " bytes exceeds the library's static scratch of " +
+                                     std::to_string((u64)ASTRA_NOALLOC_SCRATCH_BYTES) + " bytes (ASTRA_NOALLOC_SCRATCH_BYTES): use astra_run_batch");
+    if (c->pending) return fail(c, ASTRA_ESTATE, "a batch is still running");
+    CUDA_TRY(c, cudaSetDevice(c->device), "cudaSetDevice");
+    const uint8_t* in = (const uint8_t*)d_in;
+    std::string err;
+    int32_t rc = astra_engine_launch_noalloc(c->device, in + info->off_const, (const PointDesc*)(in + info->off_desc),
+                                             (const u32*)(in + info->off_order), (uint8_t*)d_out,
+                                             info->scratch_bytes - ASTRA_NOALLOC_HEADER_BYTES, info->warps, info->hot_bytes,
+                                             stream ? stream : (void*)c->stream, err);
+    if (rc) return fail(c, rc, err);
+    return ASTRA_OK;
+}

@@ -2825,3 +2825,61 @@ int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& er
     }
     return ASTRA_OK;
 }
+
+
+// ---------------------------------------------------------------------------------------------
+// No-allocation path (include/astra.h: astra_run_packed_noalloc).  The scratch of one single-CTA
+// design point -- queue header + the CTA's workspace -- lives in this file-scope array instead of
+// a cudaMalloc'ed buffer.  In host code the array's name is only a stand-in: its device address
+// is resolved once per device with cudaGetSymbolAddress (that device current) and handed to the
+// kernel as its workspace pointer.  Every call on a device shares the array.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char astra_noalloc_scratch[ASTRA_NOALLOC_SCRATCH_BYTES];
+
+#define ASTRA_NOALLOC_MAX_DEVICES 64
+static uint8_t* g_noalloc_ptr[ASTRA_NOALLOC_MAX_DEVICES];     // device address of the array, per device (nullptr: not resolved yet)
+
+int32_t astra_engine_static_scratch(int device, uint8_t** ptr, std::string& err) {
+    if (device < 0 || device >= ASTRA_NOALLOC_MAX_DEVICES) { err = "device index beyond the static-scratch table"; return ASTRA_ELIMIT; }
+    if (!g_noalloc_ptr[device]) {
+        int cur = -1;
+        cudaError_t e = cudaGetDevice(&cur);
+        if (e == cudaSuccess && cur != device) { err = "static scratch: the device is not current"; return ASTRA_ESTATE; }
+        void* p = nullptr;
+        if (e == cudaSuccess) e = cudaGetSymbolAddress(&p, astra_noalloc_scratch);
+        if (e != cudaSuccess || !p) { (void)cudaGetLastError(); err = std::string("cudaGetSymbolAddress(static scratch): ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+        // the kernel's shared-memory opt-in is set here too, so that the run itself only clears and launches
+        e = cudaFuncSetAttribute((const void*)astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)(astra_engine_fixed_smem(16) + ASTRA_HOT_BUDGET_SINGLE));
+        if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+        g_noalloc_ptr[device] = (uint8_t*)p;
+    }
+    *ptr = g_noalloc_ptr[device];
+    return ASTRA_OK;
+}
+
+// One design point on one CTA: [0, 16) of the array = queue counters + abort flag, [256, 256 + sizeof(GroupCtl)) an
+// (unused) group block, [ASTRA_NOALLOC_HEADER_BYTES, ...) the CTA's workspace.  The header must start at zero.
+int32_t astra_engine_launch_noalloc(int device, const uint8_t* d_const, const PointDesc* d_point, const u32* d_order,
+                                    uint8_t* d_results, u64 ws_bytes, u32 warps_per_cta, u32 hot_bytes, void* stream, std::string& err) {
+    if ((u64)ASTRA_NOALLOC_HEADER_BYTES + ws_bytes > ASTRA_NOALLOC_SCRATCH_BYTES) { err = "scratch exceeds the static scratch array"; return ASTRA_ELIMIT; }
+    if (hot_bytes > ASTRA_HOT_BUDGET_SINGLE || warps_per_cta != 16) { err = "packed point was planned for another CTA shape"; return ASTRA_EINVAL; }
+    uint8_t* scratch = nullptr;
+    int32_t rc = astra_engine_static_scratch(device, &scratch, err);
+    if (rc) return rc;
+    cudaError_t e = cudaMemsetAsync(scratch, 0, ASTRA_NOALLOC_HEADER_BYTES, (cudaStream_t)stream);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("scratch header clear: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+    const u32 fixed = astra_engine_fixed_smem(warps_per_cta);
+    const size_t sm = (size_t)fixed + hot_bytes;
+    // the other path sets this attribute to its own batch's size before each of its launches: set ours (no allocation)
+    e = cudaFuncSetAttribute((const void*)astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+    const uint8_t* a0 = d_const; uint8_t* a1 = scratch + ASTRA_NOALLOC_HEADER_BYTES; uint8_t* a2 = d_results; const PointDesc* a3 = d_point;
+    const u32* a4 = d_order; u32* a5 = (u32*)scratch; GroupCtl* a6 = (GroupCtl*)(scratch + 256);
+    u32 a7 = 1, a8 = 0, a9 = 0, a10 = 1;
+    u64 a11 = 0, a12 = 0, a13 = (ws_bytes + 255) & ~255ull; u32 a14 = fixed;
+    void* args[] = {&a0, &a1, &a2, &a3, &a4, &a5, &a6, &a7, &a8, &a9, &a10, &a11, &a12, &a13, &a14};
+    e = cudaLaunchCooperativeKernel((const void*)astra_step_kernel, dim3(1), dim3(warps_per_cta * 32), args, sm, (cudaStream_t)stream);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("kernel launch: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
+    return ASTRA_OK;
+}
