@@ -11,6 +11,7 @@
 #include <map>
 #include <new>
 #include <numeric>
+#include <thread>
 
 struct astra_ctx {
     int device = 0;
@@ -248,6 +249,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         opt.hot_budget = std::min<u32>(opt.hot_budget, any_big ? ASTRA_HOT_BUDGET_GROUPS : ASTRA_HOT_BUDGET_SINGLE);
     }
     u32 hot_max = 0, n_big = 0;
+    // the tables shared by the points of a topology / a collective go into the blob once
     for (u32 i = 0; i < n; i++) {
         const astra_point& p = pts[i];
         const HostTopo& t = c->topos[p.topo_id];
@@ -266,12 +268,58 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
             o[4] = blob.add(h.succ_ptr); o[5] = blob.add(h.succ); o[6] = blob.add(h.ndeps);
             coll_off[p.coll_id] = o;
         }
-        std::string err;
-        double unused = 0;
-        opt.group = big[i] ? c->group : 1;
-        int32_t rc = astra_plan_point(t, h, c->gpus[p.gpu_id], opt, topo_off[p.topo_id].data(),
-                                      coll_off[p.coll_id].data(), blob, c->descs[i], unused, err);
-        if (rc) return fail(c, rc, "point " + std::to_string(i) + ": " + err);
+    }
+    // A0 per point (routing walk, cell layout, array placement): independent, spread over the host's cores; every
+    // thread appends its points' own tables to a blob of its own, concatenated behind the shared tables afterwards
+    const u32 n_thr = std::max<u32>(1, std::min<u32>({std::thread::hardware_concurrency(), 32u, (n + 15) / 16}));
+    std::vector<Blob> tblob(n_thr);
+    std::vector<int32_t> trc(n_thr, ASTRA_OK);
+    std::vector<std::string> terr(n_thr);
+    std::vector<u32> tfail(n_thr, 0);
+    auto plan_range = [&](u32 th) {
+        const u32 lo = (u32)((u64)n * th / n_thr), hi = (u32)((u64)n * (th + 1) / n_thr);
+        try {
+            for (u32 i = lo; i < hi && trc[th] == ASTRA_OK; i++) {
+                const astra_point& p = pts[i];
+                PlanOptions o2 = opt;
+                o2.group = big[i] ? c->group : 1;
+                double unused = 0;
+                int32_t rc = astra_plan_point(c->topos[p.topo_id], c->colls[p.coll_id], c->gpus[p.gpu_id], o2,
+                                              topo_off.find(p.topo_id)->second.data(), coll_off.find(p.coll_id)->second.data(),
+                                              tblob[th], c->descs[i], unused, terr[th]);
+                if (rc) { trc[th] = rc; tfail[th] = i; }
+            }
+        } catch (const std::bad_alloc&) { trc[th] = ASTRA_ENOMEM; terr[th] = "host allocation failed"; tfail[th] = lo; }
+          catch (...) { trc[th] = ASTRA_EINVAL; terr[th] = "unexpected error"; tfail[th] = lo; }
+    };
+    if (n_thr == 1) plan_range(0);
+    else {
+        std::vector<std::thread> pool;
+        for (u32 th = 0; th < n_thr; th++) pool.emplace_back(plan_range, th);
+        for (auto& th : pool) th.join();
+    }
+    for (u32 th = 0; th < n_thr; th++)
+        if (trc[th]) return fail(c, trc[th], "point " + std::to_string(tfail[th]) + ": " + terr[th]);
+    {
+        // c_off entries of the tables a point shares with others are offsets into the shared part already; the
+        // point's own tables move behind it by the offset of its thread's blob
+        bool shared_table[ASTRA_C_COUNT] = {false};
+        for (u32 q : {ASTRA_C_in_ptr, ASTRA_C_in_link, ASTRA_C_head, ASTRA_C_tail, ASTRA_C_leff, ASTRA_C_next_link, ASTRA_C_row_ptr,
+                      ASTRA_C_step_od, ASTRA_C_lines, ASTRA_C_cu_lo, ASTRA_C_cu_n, ASTRA_C_succ_ptr, ASTRA_C_succ, ASTRA_C_ndeps})
+            shared_table[q] = true;
+        u64 total = blob.bytes.size() + 16;
+        for (u32 th = 0; th < n_thr; th++) total += tblob[th].bytes.size() + 16;
+        blob.bytes.reserve(total);                                  // one allocation, no re-copy of what is there
+        for (u32 th = 0; th < n_thr; th++) {
+            const u64 base = blob.add(tblob[th].bytes.data(), tblob[th].bytes.size());
+            const u32 lo = (u32)((u64)n * th / n_thr), hi = (u32)((u64)n * (th + 1) / n_thr);
+            for (u32 i = lo; i < hi; i++)
+                for (u32 q = 0; q < ASTRA_C_COUNT; q++)
+                    if (!shared_table[q]) c->descs[i].c_off[q] += base;
+            std::vector<uint8_t>().swap(tblob[th].bytes);
+        }
+    }
+    for (u32 i = 0; i < n; i++) {
         PointDesc& P = c->descs[i];
         P.r_step_ts = roff; roff += 32ull * P.S;
         P.r_link_lines = roff; roff += 8ull * P.E;
