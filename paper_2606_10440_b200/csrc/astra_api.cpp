@@ -33,6 +33,7 @@ struct astra_ctx {
     GroupCtl* d_groups = nullptr;
     u64 const_bytes = 0, ws_big_stride = 0, ws_single_stride = 0, ws_single_off = 0, ws_total = 0, results_bytes = 0;
     u32 n_big = 0, n_slots = 0, grid = 1, group = 1, warps = 0, hot_bytes = 0, variant = 1;
+    bool stage = false;
     std::vector<uint8_t> h_results;
     float last_ms = 0.f;
     u32 last_launches = 0;
@@ -235,7 +236,9 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     classify(c, n, pts, (u32)sms * ctas_per_sm, cost, big, &c->group);
     PlanOptions opt;
     opt.flags = c->flags & 0xffull; opt.max_cycles = max_cycles;
-    const u32 fixed = astra_engine_fixed_smem(c->warps);
+    c->stage = false;          // reserve the staging area only when some point's per-step tables fit it (it is taken from L1)
+    for (u32 i = 0; i < n; i++) c->stage = c->stage || astra_engine_stageable(c->warps, c->colls[pts[i].coll_id].S);
+    const u32 fixed = astra_engine_fixed_smem(c->warps, c->stage);
     int smem_sm = 0;
     CUDA_TRY(c, cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev), "device attribute");
     const u32 smem_cta = std::min<u32>((u32)smem_max, (u32)smem_sm / ctas_per_sm - 1024);    // 1 KB per CTA is reserved by the system
@@ -333,7 +336,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
     c->results_bytes = roff ? roff : 16;
     std::string err;
     u32 occ = 0, nsm = 0;
-    int32_t rc = astra_engine_occupancy(c->warps, c->hot_bytes, c->variant, &occ, &nsm, err);
+    int32_t rc = astra_engine_occupancy(c->warps, c->hot_bytes, c->variant, c->stage, &occ, &nsm, err);
     if (rc) return fail(c, rc, err);
     if (occ == 0) return fail(c, ASTRA_ECUDA, "kernel does not fit on an SM");
     // every CTA of the grid must be resident at once (persistent CTAs, group barriers)
@@ -366,7 +369,7 @@ static int32_t prepare(astra_ctx* c, uint32_t n, const astra_point* pts, uint64_
         return cost[a] > cost[b];
     });
 
-    CUDA_TRY(c, cudaMalloc((void**)&c->d_const, std::max<size_t>(16, blob.bytes.size())), "cudaMalloc const");
+    CUDA_TRY(c, cudaMalloc((void**)&c->d_const, blob.bytes.size() + 16), "cudaMalloc const");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_ws, std::max<u64>(16, c->ws_total)), "cudaMalloc workspace");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_results, c->results_bytes), "cudaMalloc results");
     CUDA_TRY(c, cudaMalloc((void**)&c->d_points, std::max<size_t>(16, n * sizeof(PointDesc))), "cudaMalloc points");
@@ -401,7 +404,7 @@ extern "C" int32_t astra_run_batch_async(astra_ctx* c, uint32_t n, const astra_p
             L.d_order = c->d_order; L.d_queue = c->d_queue; L.d_groups = c->d_groups; L.n_points = n;
             L.n_big = c->n_big; L.n_slots = c->n_slots; L.group = c->group; L.grid = c->grid;
             L.ws_big_stride = c->ws_big_stride; L.ws_single_off = c->ws_single_off; L.ws_single_stride = c->ws_single_stride;
-            L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes; L.variant = c->variant;
+            L.warps_per_cta = c->warps; L.hot_bytes = c->hot_bytes; L.variant = c->variant; L.stage = c->stage;
             std::string err;
             int32_t rc = astra_engine_launch(L, (void*)c->stream, err);
             if (rc) return fail(c, rc, err);
@@ -521,7 +524,7 @@ extern "C" int32_t astra_pack_point(astra_ctx* c, const astra_point* pt, uint64_
         int32_t rc = astra_engine_static_scratch(c->device, &scratch, err);     // once per device, this device current
         if (rc) return fail(c, rc, err);
         const u32 warps = 16;
-        const u32 fixed = astra_engine_fixed_smem(warps);
+        const u32 fixed = astra_engine_fixed_smem(warps, astra_engine_stageable(warps, c->colls[pt->coll_id].S));
         const u32 smem_cta = std::min<u32>((u32)smem_max, (u32)smem_sm - 1024);
         PlanOptions opt;
         opt.flags = c->flags & 0xffull; opt.max_cycles = max_cycles; opt.group = 1;
@@ -585,7 +588,7 @@ extern "C" int32_t astra_run_packed_noalloc(astra_ctx* c, const astra_packed_inf
     std::string err;
     int32_t rc = astra_engine_launch_noalloc(c->device, in + info->off_const, (const PointDesc*)(in + info->off_desc),
                                              (const u32*)(in + info->off_order), (uint8_t*)d_out,
-                                             info->scratch_bytes - ASTRA_NOALLOC_HEADER_BYTES, info->warps, info->hot_bytes,
+                                             info->scratch_bytes - ASTRA_NOALLOC_HEADER_BYTES, info->warps, info->hot_bytes, info->n_steps,
                                              stream ? stream : (void*)c->stream, err);
     if (rc) return fail(c, rc, err);
     return ASTRA_OK;

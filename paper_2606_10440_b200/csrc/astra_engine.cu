@@ -40,6 +40,8 @@
 
 #define FULL 0xffffffffu
 #define ASTRA_COLD            // measured: real calls (__noinline__) for the rarely taken paths cost 3 % on every config
+#define STAGE_BYTES (24u << 10)   // shared-memory copy of a point's per-step constant tables (TMA bulk copies at the point's start)
+#define STAGE_TABLES 10u          // step_od, lines, cu_lo, cu_n, step_q, step_r, first_link, step_alpha, step_aq, step_ar
 #define SCR_WORDS 1088u   // per-warp scratch words: 32 lanes x 64 16-bit ack keys (wf_sim, wf_priority_word), 513 counters (ack_sort), 512 (ack_chunk)
 
 struct Ctx {   // resolved pointers of the point a CTA is running; lives in shared memory
@@ -68,6 +70,7 @@ struct Ctl {   // per-CTA control block in shared memory
     u32 shint[32][2];   // next-event hint of node i's current window (slot: window ordinal & 1)
     u32 hint8[8];       // the point's hint per window ordinal & 7
     u32 stop;           // 1 + final status once a node has decided that the run ends
+    u32 stage_phase, stage_wait;   // mbarrier phase of the next / the current point's staged tables
     // link service by all warps of a set (link_service_set)
     int ls_max[32];     // per warp: maximum of its block
     u32 ls_acc[32], ls_last[32];   // per set: lines accepted, last acceptance cycle
@@ -2450,6 +2453,20 @@ __device__ u32 wait_prog(Ctl& ctl, u32 lane, u32 n_nodes, u32 pm, u32 need_pred,
     }
 }
 
+// TMA bulk copy global -> shared memory, completion counted in bytes on an mbarrier (all addresses and the size
+// multiples of 16 bytes).  One thread issues; everybody waits on the barrier's phase.
+__device__ __forceinline__ void bulk_g2s(u32 dst_smem, const void* src, u32 bytes, u32 mbar_smem) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(mbar_smem) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u32 mbar_smem, u32 phase) {
+    u32 ok;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(ok) : "r"(mbar_smem), "r"(phase) : "memory");
+    } while (!ok);
+}
+
 __device__ __forceinline__ void
 step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
@@ -2472,6 +2489,16 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
     uint8_t* ws = in_slot ? ws_base + (size_t)gid * ws_big_stride : ws_base + ws_single_off + (size_t)blockIdx.x * ws_single_stride;
     GroupCtl* gc = groups + gid;
     u32 bar_target = 0;                 // arrivals that complete the next group barrier
+    // staging area of the per-step constant tables and its mbarrier, right below the hot region -- present when the launch
+    // reserved it (astra_engine_fixed_smem): the hot region then starts 128 + STAGE_BYTES above the per-warp scratch
+#define HAS_STAGE (nwarps == 16u && hot_off >= (u32)((((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)) + (size_t)nwarps * SCR_WORDS * sizeof(u32) + 127) & ~size_t(127)) + 128u + STAGE_BYTES)
+#define STAGE_S ((u32)__cvta_generic_to_shared(hot) - STAGE_BYTES)
+#define MBAR_S (STAGE_S - 128u)
+    if (HAS_STAGE && tid == 0) {
+        ctl.stage_phase = 0u;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(MBAR_S) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     if (tid == 0) ctl.abort = 0u;
 
     #pragma unroll 1
@@ -2507,8 +2534,26 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         }
         const u32 pi = order[qi];
         const PointDesc& P = points[pi];
+        // The ten per-step constant tables are looked up on every delivery, issue and ack: where they fit (config 2: 4.5 KB,
+        // config 4: <= 19 KB) one thread copies them to shared memory with TMA bulk copies and the point runs on the copies.
+        const u32 stage_pad = (4u * P.S + 15u) & ~15u;
+        const bool staged = HAS_STAGE && P.S > 0u && STAGE_TABLES * stage_pad <= STAGE_BYTES;
         if (tid == 0) {
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
+            if (staged) {
+                const u32 stage_s = STAGE_S, mbar_s = MBAR_S;
+                uint8_t* const stage = hot - STAGE_BYTES;
+                ctl.stage_wait = ctl.stage_phase; ctl.stage_phase ^= 1u;        // the phase everybody waits for below
+                const u32* src[STAGE_TABLES] = {c.step_od, c.lines, c.cu_lo, c.cu_n, c.step_q, c.step_r, c.first_link, c.step_alpha, c.step_aq, c.step_ar};
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the last point's generic reads of the area are done
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar_s), "r"(STAGE_TABLES * stage_pad) : "memory");
+#pragma unroll
+                for (u32 q = 0; q < STAGE_TABLES; q++) bulk_g2s(stage_s + q * stage_pad, src[q], stage_pad, mbar_s);
+                const u32* const st = (const u32*)stage;
+                const u32 w = stage_pad / 4u;
+                c.step_od = st; c.lines = st + w; c.cu_lo = st + 2 * w; c.cu_n = st + 3 * w; c.step_q = st + 4 * w; c.step_r = st + 5 * w;
+                c.first_link = st + 6 * w; c.step_alpha = st + 7 * w; c.step_aq = st + 8 * w; c.step_ar = st + 9 * w;
+            }
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
             ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
             for (int i = 0; i < 32; i++) { ctl.ls_acc[i] = 0u; ctl.ls_last[i] = 0u; }
@@ -2524,6 +2569,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         long long dck = clock64();
 #endif
         __syncthreads();
+        if (staged) mbar_wait(MBAR_S, ctl.stage_wait);                          // the tables have landed in shared memory
         // ---- state init: shared-memory arrays by their CTA, global arrays split over the group ----
         #pragma unroll 1
         for (u32 a = 0; a < ASTRA_A_COUNT; a++) {
@@ -2782,18 +2828,24 @@ bool astra_engine_has_diag() {
 #endif
 }
 
-u32 astra_engine_fixed_smem(u32 warps) {
+bool astra_engine_stageable(u32 warps, u32 n_steps) {
+    return warps == 16 && n_steps > 0 && (u64)STAGE_TABLES * ((4ull * n_steps + 15) & ~15ull) <= STAGE_BYTES;
+}
+
+u32 astra_engine_fixed_smem(u32 warps, bool stage) {
     size_t s = ((sizeof(Ctx) + 15) & ~size_t(15)) + ((sizeof(Ctl) + 15) & ~size_t(15)) + (size_t)warps * SCR_WORDS * sizeof(u32);
-    return (u32)((s + 127) & ~size_t(127));
+    s = (s + 127) & ~size_t(127);
+    if (stage && warps == 16) s += 128 + STAGE_BYTES;        // mbarrier + staging area of the per-step constant tables, right below the hot region
+    return (u32)s;
 }
 
 static const void* kernel_variant(u32) { return (const void*)astra_step_kernel; }
 
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, u32* ctas_per_sm, u32* n_sms, std::string& err) {
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, bool stage, u32* ctas_per_sm, u32* n_sms, std::string& err) {
     int dev = 0, sms = 0, occ = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    size_t sm = (size_t)astra_engine_fixed_smem(warps_per_cta) + hot_bytes;
+    size_t sm = (size_t)astra_engine_fixed_smem(warps_per_cta, stage) + hot_bytes;
     if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel_variant(variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel_variant(variant), (int)warps_per_cta * 32, sm);
     if (e != cudaSuccess) { err = std::string("occupancy query: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
@@ -2802,7 +2854,7 @@ int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, u3
 }
 
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err) {
-    const u32 fixed = astra_engine_fixed_smem(L.warps_per_cta);
+    const u32 fixed = astra_engine_fixed_smem(L.warps_per_cta, L.stage);
     size_t sm = (size_t)fixed + L.hot_bytes;
     cudaError_t e = cudaFuncSetAttribute(kernel_variant(L.variant), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     if (e != cudaSuccess) { err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
@@ -2850,7 +2902,7 @@ int32_t astra_engine_static_scratch(int device, uint8_t** ptr, std::string& err)
         if (e != cudaSuccess || !p) { (void)cudaGetLastError(); err = std::string("cudaGetSymbolAddress(static scratch): ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
         // the kernel's shared-memory opt-in is set here too, so that the run itself only clears and launches
         e = cudaFuncSetAttribute((const void*)astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)(astra_engine_fixed_smem(16) + ASTRA_HOT_BUDGET_SINGLE));
+                                 (int)(astra_engine_fixed_smem(16, true) + ASTRA_HOT_BUDGET_SINGLE));
         if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("smem attribute: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
         g_noalloc_ptr[device] = (uint8_t*)p;
     }
@@ -2861,7 +2913,7 @@ int32_t astra_engine_static_scratch(int device, uint8_t** ptr, std::string& err)
 // One design point on one CTA: [0, 16) of the array = queue counters + abort flag, [256, 256 + sizeof(GroupCtl)) an
 // (unused) group block, [ASTRA_NOALLOC_HEADER_BYTES, ...) the CTA's workspace.  The header must start at zero.
 int32_t astra_engine_launch_noalloc(int device, const uint8_t* d_const, const PointDesc* d_point, const u32* d_order,
-                                    uint8_t* d_results, u64 ws_bytes, u32 warps_per_cta, u32 hot_bytes, void* stream, std::string& err) {
+                                    uint8_t* d_results, u64 ws_bytes, u32 warps_per_cta, u32 hot_bytes, u32 n_steps, void* stream, std::string& err) {
     if ((u64)ASTRA_NOALLOC_HEADER_BYTES + ws_bytes > ASTRA_NOALLOC_SCRATCH_BYTES) { err = "scratch exceeds the static scratch array"; return ASTRA_ELIMIT; }
     if (hot_bytes > ASTRA_HOT_BUDGET_SINGLE || warps_per_cta != 16) { err = "packed point was planned for another CTA shape"; return ASTRA_EINVAL; }
     uint8_t* scratch = nullptr;
@@ -2869,7 +2921,7 @@ int32_t astra_engine_launch_noalloc(int device, const uint8_t* d_const, const Po
     if (rc) return rc;
     cudaError_t e = cudaMemsetAsync(scratch, 0, ASTRA_NOALLOC_HEADER_BYTES, (cudaStream_t)stream);
     if (e != cudaSuccess) { (void)cudaGetLastError(); err = std::string("scratch header clear: ") + cudaGetErrorString(e); return ASTRA_ECUDA; }
-    const u32 fixed = astra_engine_fixed_smem(warps_per_cta);
+    const u32 fixed = astra_engine_fixed_smem(warps_per_cta, astra_engine_stageable(warps_per_cta, n_steps));
     const size_t sm = (size_t)fixed + hot_bytes;
     // the other path sets this attribute to its own batch's size before each of its launches: set ours (no allocation)
     e = cudaFuncSetAttribute((const void*)astra_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

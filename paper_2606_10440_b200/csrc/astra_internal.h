@@ -190,14 +190,16 @@ struct EngineLaunch {
     u32 n_big, n_slots, group, grid;
     u64 ws_big_stride, ws_single_off, ws_single_stride;
     u32 warps_per_cta, hot_bytes;
+    bool stage;                     // the CTAs carry the staging area for per-step constant tables (some point of the batch fits it)
     u32 variant;                    // 1: one CTA per SM (128 registers per thread), 2: two CTAs per SM (64)
 };
 int32_t astra_engine_launch(const EngineLaunch& L, void* stream, std::string& err);
-int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, u32* ctas_per_sm, u32* n_sms, std::string& err);
-u32 astra_engine_fixed_smem(u32 warps_per_cta);
+int32_t astra_engine_occupancy(u32 warps_per_cta, u32 hot_bytes, u32 variant, bool stage, u32* ctas_per_sm, u32* n_sms, std::string& err);
+u32 astra_engine_fixed_smem(u32 warps_per_cta, bool stage);
+bool astra_engine_stageable(u32 warps_per_cta, u32 n_steps);   // the point's per-step constant tables fit the staging area
 bool astra_engine_has_diag();
 // No-allocation path (include/astra.h, astra_run_packed_noalloc): the library's static device scratch.
 #define ASTRA_NOALLOC_HEADER_BYTES 512u    // queue counters + abort flag, one GroupCtl; cleared by every call
 int32_t astra_engine_static_scratch(int device, uint8_t** ptr, std::string& err);       // set-up: once per device, that device current
 int32_t astra_engine_launch_noalloc(int device, const uint8_t* d_const, const PointDesc* d_point, const u32* d_order,
-                                    uint8_t* d_results, u64 ws_bytes, u32 warps_per_cta, u32 hot_bytes, void* stream, std::string& err);
+                                    uint8_t* d_results, u64 ws_bytes, u32 warps_per_cta, u32 hot_bytes, u32 n_steps, void* stream, std::string& err);
