@@ -2076,11 +2076,11 @@ __device__ __forceinline__ bool group_barrier(GroupCtl* gc, u32 target, u32* abo
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        atomicAdd(&gc->bar, 1u);
+        const u32 mine = atomicAdd(&gc->bar, 1u) + 1u;           // the last to arrive knows it from its own count: no poll
         const long long start = clock64();
         u32 spins = 0;
         #pragma unroll 1
-        while ((int32_t)(*(volatile u32*)&gc->bar - target) < 0) {
+        while ((int32_t)(mine - target) < 0 && (int32_t)(*(volatile u32*)&gc->bar - target) < 0) {
             if ((++spins & 0x3ffu) == 0) {
                 if (*(volatile u32*)abort_flag) { ctl.abort = 1u; break; }
                 if (clock64() - start > ASTRA_SPIN_CLOCKS) { atomicExch(abort_flag, 1u); ctl.abort = 1u; break; }

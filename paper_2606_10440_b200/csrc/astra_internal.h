@@ -124,13 +124,14 @@ struct DeviceSummary {          // mirrors astra_summary, written by the kernel
 
 // Control block of one CTA group in global memory (multi-CTA design points).
 struct GroupCtl {
-    u32 bar;            // monotone barrier counter
+    u32 bar;            // monotone barrier counter; alone in its 128-byte line: every CTA of the group polls it
+    u32 pad0[31];
     u32 point;          // queue index the group is running
     u32 acked;          // steps fully acked, all CTAs
     u32 err;
     u32 completion;     // max t_ack
     u32 hint[3];        // next-event time, rotated per window
-    u32 pad[8];
+    u32 pad[25];
 };
 
 // ---------------------------------------------------------------------------------------------
