@@ -2467,6 +2467,22 @@ __device__ __forceinline__ void mbar_wait(u32 mbar_smem, u32 phase) {
     } while (!ok);
 }
 
+// One thread: the ten per-step constant tables of the point -> the staging area (TMA bulk copies counted on the
+// mbarrier 128 bytes below it); the Ctx then points at the copies.  A call of its own: keeps its registers out of the kernel body.
+__device__ __noinline__ void stage_tables(Ctx& c, Ctl& ctl, uint8_t* stage, u32 stage_pad) {
+    const u32 stage_s = (u32)__cvta_generic_to_shared(stage), mbar_s = stage_s - 128u;
+    ctl.stage_wait = ctl.stage_phase; ctl.stage_phase ^= 1u;        // the phase everybody waits for
+    const u32* src[STAGE_TABLES] = {c.step_od, c.lines, c.cu_lo, c.cu_n, c.step_q, c.step_r, c.first_link, c.step_alpha, c.step_aq, c.step_ar};
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the last point's generic reads of the area are done
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar_s), "r"(STAGE_TABLES * stage_pad) : "memory");
+#pragma unroll
+    for (u32 q = 0; q < STAGE_TABLES; q++) bulk_g2s(stage_s + q * stage_pad, src[q], stage_pad, mbar_s);
+    const u32* const st = (const u32*)stage;
+    const u32 w = stage_pad / 4u;
+    c.step_od = st; c.lines = st + w; c.cu_lo = st + 2 * w; c.cu_n = st + 3 * w; c.step_q = st + 4 * w; c.step_r = st + 5 * w;
+    c.first_link = st + 6 * w; c.step_alpha = st + 7 * w; c.step_aq = st + 8 * w; c.step_ar = st + 9 * w;
+}
+
 __device__ __forceinline__ void
 step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_base, uint8_t* __restrict__ results,
                   const PointDesc* __restrict__ points, const u32* __restrict__ order, u32* queue,
@@ -2540,20 +2556,7 @@ step_kernel_body(const uint8_t* __restrict__ cblob, uint8_t* __restrict__ ws_bas
         const bool staged = HAS_STAGE && P.S > 0u && STAGE_TABLES * stage_pad <= STAGE_BYTES;
         if (tid == 0) {
             resolve_ctx(c, P, cblob, ws, hot, results, rank);
-            if (staged) {
-                const u32 stage_s = STAGE_S, mbar_s = MBAR_S;
-                uint8_t* const stage = hot - STAGE_BYTES;
-                ctl.stage_wait = ctl.stage_phase; ctl.stage_phase ^= 1u;        // the phase everybody waits for below
-                const u32* src[STAGE_TABLES] = {c.step_od, c.lines, c.cu_lo, c.cu_n, c.step_q, c.step_r, c.first_link, c.step_alpha, c.step_aq, c.step_ar};
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the last point's generic reads of the area are done
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar_s), "r"(STAGE_TABLES * stage_pad) : "memory");
-#pragma unroll
-                for (u32 q = 0; q < STAGE_TABLES; q++) bulk_g2s(stage_s + q * stage_pad, src[q], stage_pad, mbar_s);
-                const u32* const st = (const u32*)stage;
-                const u32 w = stage_pad / 4u;
-                c.step_od = st; c.lines = st + w; c.cu_lo = st + 2 * w; c.cu_n = st + 3 * w; c.step_q = st + 4 * w; c.step_r = st + 5 * w;
-                c.first_link = st + 6 * w; c.step_alpha = st + 7 * w; c.step_aq = st + 8 * w; c.step_ar = st + 9 * w;
-            }
+            if (staged) stage_tables(c, ctl, hot - STAGE_BYTES, stage_pad);
             ctl.acked = 0; ctl.completion = 0; ctl.err = 0;
             ctl.hint[0] = ctl.hint[1] = ctl.hint[2] = ASTRA_T_INF;
             for (int i = 0; i < 32; i++) { ctl.ls_acc[i] = 0u; ctl.ls_last[i] = 0u; }
