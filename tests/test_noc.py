@@ -78,3 +78,12 @@ def test_noc_engine_parity():
         b.add(m.cu(0, cu), m.channel(1, 3), 20, 0, 1)
     check_workload(_single(t, b.build(), gpu), oracle_flags=oracle.FLAG_PRUNED_SCAN)
     check_workload(_single(t, b.build(), gpu), flags=0x100, oracle_flags=oracle.FLAG_PRUNED_SCAN)
+
+
+@pytest.mark.gpu
+def test_noc_engine_parity_four_gpus():
+    """Four NoC-level GPUs (1,824 nodes, 4,000 links, 1,536 endpoints): the CU-level all-gather with local loads, every
+    remote store crossing two meshes and one of the 32 scale-up switches."""
+    from tests.parity import check_workload
+    t, m = noc.noc_cluster(4)
+    check_workload(_single(t, noc.noc_all_gather(m, 1024, 32, 4), GpuCfg(1, 4, 64, 4)), oracle_flags=oracle.FLAG_PRUNED_SCAN)
