@@ -185,3 +185,24 @@ def test_engine_parity_on_control_variants():
     for w in _transformed_workloads():
         check_workload(w, oracle_flags=oracle.FLAG_PRUNED_SCAN)
         check_workload(w, flags=0x100, oracle_flags=oracle.FLAG_PRUNED_SCAN)       # one CTA per point
+
+
+@pytest.mark.gpu
+def test_engine_ring_signal_closed_form_all_sizes():
+    """Config 2's ring with signals at all eleven sizes (64 KiB .. 64 MiB) on the engine: T = 14 (350 + n/4) + 13 + 350
+    (the closed form the oracle is pinned to at the four smallest sizes, derivation in the golden file)."""
+    from paper_2606_10440_b200 import simulate_workload
+    w2 = configs.config2()
+    ws = Workload(name="ring+signal", max_cycles=w2.max_cycles)
+    expect = []
+    for i in range(w2.n_points):
+        if w2.meta[i]["algo"] != "ring":
+            continue
+        topo, coll, gpu = w2.point(i)
+        ws.topologies.append(topo); ws.collectives.append(C.put_with_signal(coll)); ws.gpus.append(gpu)
+        ws.points.append((len(ws.topologies) - 1, len(ws.collectives) - 1, len(ws.gpus) - 1)); ws.meta.append({})
+        expect.append(14 * (350 + w2.meta[i]["lines"] // 8 // 4) + 13 + 350)
+    res = simulate_workload(ws)
+    assert len(res) == 11
+    for (summ, _, _), t in zip(res, expect):
+        assert summ.status == 0 and summ.completion_cycle == t
